@@ -1,0 +1,134 @@
+/* tree.h — C ABI of the B200-native Barnes-Hut force library (libbhtree.so).
+ *
+ * What it computes (arxiv 1412.0659, Bedorf et al. 2014, cited as PAPER.md:L<line>):
+ * for N point masses with FP32 positions r_j and masses m_j, the
+ * acceleration a_i and potential phi_i "which we collectively call the force" (L184) by the
+ * Barnes-Hut tree algorithm (L31): Peano-Hilbert keys over the bounding box (L97), sort (Table
+ * II L244), sparse octree with at most `leaf_size` particles per leaf (L31, L246), multipole
+ * moments mass / centre of mass / quadrupole per cell (L65, L190, L247), then a fused tree-walk +
+ * force pass (L67-79, L248) that evaluates particle-particle (23 flop) and particle-cell (65 flop)
+ * interactions, Eqs. (1),(2) (L186-192), with Plummer softening eps and opening angle theta
+ * (L31, L133), and a 2nd-order leapfrog (L121).  G = 1.  Every reading of a point PAPER.md leaves
+ * open is listed in DESIGN.md ("Readings").
+ *
+ * Conventions
+ *  - Plain C, no exceptions, never exits.  Every call returns 0 on success or a negative code:
+ *      TREE_ERR_ARG      -1  bad argument (NULL, N <= 0, N > 2^31-1, theta < 0, eps < 0, NaN ...)
+ *      TREE_ERR_NOMEM    -2  out of device (or pinned host) memory
+ *      TREE_ERR_CUDA     -3  CUDA error; text via tree_last_error()
+ *      TREE_ERR_ORDER    -4  call order (force before build, leapfrog before force/velocities)
+ *      TREE_ERR_NONFINITE -5 non-finite position or mass detected while building
+ *  - Pointers marked DEV are device pointers on the context's device, allocated and owned by the
+ *    caller (e.g. torch tensors); pointers marked HOST are host pointers (pinned memory makes the
+ *    copies faster, pageable works).  The library copies what it needs during the call and never
+ *    keeps a caller pointer.  Its own buffers grow to the largest N seen and are reused.
+ *  - All work is enqueued on the stream given to tree_create (NULL = the legacy default stream).
+ *    tree_build synchronises that stream once (it reads the cell count back to size the cell
+ *    arrays); tree_force / tree_leapfrog return after enqueueing (tree_leapfrog contains a build);
+ *    the *_host variants, tree_get_debug, tree_get_stats and tree_energy synchronise.
+ *  - "Caller order" is the particle order of the arrays given to tree_build.  Outputs are always
+ *    in caller order.  Masses must be > 0.  No two particles may share a position unless eps > 0
+ *    (the self term is skipped by index, "N-1 interactions").
+ */
+#ifndef BHTREE_TREE_H
+#define BHTREE_TREE_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TREE_OK 0
+#define TREE_ERR_ARG (-1)
+#define TREE_ERR_NOMEM (-2)
+#define TREE_ERR_CUDA (-3)
+#define TREE_ERR_ORDER (-4)
+#define TREE_ERR_NONFINITE (-5)
+
+typedef struct tree_ctx tree_ctx; /* opaque; owned by the library */
+
+/* Create a context on CUDA device `device`, working on `cuda_stream` (a cudaStream_t, may be
+ * NULL).  leaf_size: a cell with at most this many particles is a leaf ("we use
+ * 16"); 1..32.  group_size: number of consecutive Peano-Hilbert-sorted particles that share one
+ * tree walk (one warp); 32, 64 or 128 (the paper's unnamed warp-shared lists, L79). */
+int tree_create(tree_ctx **out, int device, void *cuda_stream, int leaf_size, int group_size);
+
+/* Build the tree for N particles: bounding box and PH keys, sort (L244), octree
+ * (L31, L246), groups, multipole moments level by level (L65, L190, L247).
+ * pos: DEV float[N][3] row-major; mass: DEV float[N].  1 <= N <= 2^31-1. */
+int tree_build(tree_ctx *t, const float *pos, const float *mass, long long N);
+
+/* Force pass on the last built tree (Eqs. (1),(2) L186-188): opening radii for
+ * this theta, fused walk + evaluation, results to caller order.
+ * theta >= 0 (0 = open everything = direct summation, L31); eps >= 0 (Plummer softening).
+ * acc: DEV float[N][3] or NULL; pot: DEV float[N] or NULL.  The result is also kept inside the
+ * context for tree_leapfrog / tree_get_state. */
+int tree_force(tree_ctx *t, float theta, float eps, float *acc, float *pot);
+
+/* One kick-drift-kick step of size dt: v += a dt/2; x += v dt; rebuild the tree;
+ * force with the theta, eps of the last tree_force; v += a dt/2.  Needs tree_set_velocity and
+ * one tree_force before.  dt may be negative. */
+int tree_leapfrog(tree_ctx *t, float dt);
+
+int tree_destroy(tree_ctx *t);
+
+/* ---- auxiliary ------------------------------------------------------------------------ */
+
+/* vel: DEV float[N][3], caller order, N of the last tree_build. */
+int tree_set_velocity(tree_ctx *t, const float *vel);
+
+/* Current state in caller order; any pointer may be NULL.  pos, vel, acc: DEV float[N][3];
+ * pot: DEV float[N]. */
+int tree_get_state(tree_ctx *t, float *pos, float *vel, float *acc, float *pot);
+
+/* Same as tree_build / tree_force with HOST buffers: the host<->device copies are part of the
+ * call (this is the end-to-end path bench.py times).  tree_force_host returns after the results
+ * are in acc / pot. */
+int tree_build_host(tree_ctx *t, const float *pos, const float *mass, long long N);
+int tree_force_host(tree_ctx *t, float theta, float eps, float *acc, float *pot);
+
+/* Kinetic energy sum 1/2 m v^2 and potential energy 1/2 sum m phi of the current state, FP64
+ * sums, written to HOST doubles (either may be NULL).  Synchronises. */
+int tree_energy(tree_ctx *t, double *kinetic, double *potential);
+
+/* Internal arrays for the parity tests, copied to HOST memory `dst`.  *count receives the number
+ * of records; with dst == NULL only *count is written.  Synchronises.  `what`: */
+#define TREE_DBG_KEYS 0        /* uint64[N]     PH key per particle, caller order                  */
+#define TREE_DBG_ORDER 1       /* uint32[N]     order[s] = caller index of the particle in slot s  */
+#define TREE_DBG_SORTED_KEYS 2 /* uint64[N]     keys in slot order                                 */
+#define TREE_DBG_CELLS 3       /* int32[n_cells][5] level, first, count, first_child(-1 leaf), n_child; BFS order */
+#define TREE_DBG_MOMENTS 4     /* float[n_cells][11] M, cx,cy,cz, Qxx,Qyy,Qzz,Qxy,Qxz,Qyz, delta    */
+#define TREE_DBG_GROUP_BOXES 5 /* float[n_groups][6] min x,y,z, max x,y,z                          */
+#define TREE_DBG_COUNTS 6      /* uint32[n_groups][2] n_pp, n_pc of the last tree_force            */
+#define TREE_DBG_GRID 7        /* float[10]     bbox lo[3], hi[3], cube origin[3], (float)k with side = 2^k */
+#define TREE_DBG_ROPEN2 8      /* float[n_cells] squared opening radius of the last tree_force     */
+#define TREE_DBG_SORTED_POS 9  /* float[N][4]   x,y,z,m in slot order                              */
+#define TREE_DBG_LEVEL_OFFSETS 10 /* int32[24]  first cell id of each level 0..22, then n_cells   */
+int tree_get_debug(tree_ctx *t, int what, void *dst, long long *count);
+
+/* Timings of the last tree_build / tree_force / tree_leapfrog in milliseconds (CUDA events on the
+ * context's stream) and interaction totals of the last force pass, to HOST memory.
+ * ms[TREE_NPHASE]: see TREE_PH_*.  n_pp / n_pc = sum over groups of group size x list length
+ * ("as recorded during execution").  Synchronises. */
+#define TREE_PH_KEYS 0     /* bbox + grid + keys                 */
+#define TREE_PH_SORT 1     /* radix sort of (key, index)         */
+#define TREE_PH_PERMUTE 2  /* gather particles into slot order   */
+#define TREE_PH_BUILD 3    /* octree construction + linking      */
+#define TREE_PH_MOMENTS 4  /* groups + multipole moments         */
+#define TREE_PH_OPENING 5  /* opening radii for theta            */
+#define TREE_PH_WALK 6     /* the fused walk + force kernel only */
+#define TREE_PH_UNPERMUTE 7 /* results back to caller order      */
+#define TREE_PH_INTEGRATE 8 /* leapfrog kicks + drift            */
+#define TREE_PH_TOTAL 9    /* sum of the above for the last call sequence */
+#define TREE_NPHASE 10
+int tree_get_stats(tree_ctx *t, double *ms, unsigned long long *n_pp, unsigned long long *n_pc);
+
+/* Number of kernels this library launched on the context since tree_create (for accounting). */
+long long tree_launch_count(const tree_ctx *t);
+
+/* Text of the last error on this context ("" if none). Never NULL for a non-NULL context. */
+const char *tree_last_error(const tree_ctx *t);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BHTREE_TREE_H */

@@ -1,0 +1,407 @@
+// C ABI of libbhtree.so (include/tree.h): context, buffer management, call sequencing, debug
+// readback. Every step of the path runs in the kernels of bh_build.cu / bh_force.cu.
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "bh_common.cuh"
+
+namespace bh {
+
+int set_err(tree_ctx *t, int code, const char *what, cudaError_t ce) {
+  if (t) {
+    t->err = what ? what : "";
+    if (ce != cudaSuccess) { t->err += ": "; t->err += cudaGetErrorString(ce); }
+  }
+  return code;
+}
+
+template <typename T>
+static int dev_alloc(tree_ctx *t, T *&p, long long n) {
+  if (p) { cudaFree(p); p = nullptr; }
+  if (n <= 0) n = 1;
+  cudaError_t e = cudaMalloc((void **)&p, (size_t)n * sizeof(T));
+  if (e != cudaSuccess) {
+    p = nullptr;
+    cudaGetLastError();
+    return set_err(t, TREE_ERR_NOMEM, "cudaMalloc", e);
+  }
+  return 0;
+}
+
+#define BH_TRY(x) do { int _rc = (x); if (_rc) return _rc; } while (0)
+
+static int ensure_particles(tree_ctx *t, long long N) {
+  if (N <= t->cap) return 0;
+  long long cap = N;
+  Buffers &b = t->b;
+  BH_TRY(dev_alloc(t, b.posm, cap));
+  BH_TRY(dev_alloc(t, b.vel, cap));
+  BH_TRY(dev_alloc(t, b.acc, cap));
+  for (int k = 0; k < 2; ++k) { BH_TRY(dev_alloc(t, b.key[k], cap)); BH_TRY(dev_alloc(t, b.idx[k], cap)); }
+  BH_TRY(dev_alloc(t, b.spos, cap));
+  BH_TRY(dev_alloc(t, b.sacc, cap));
+  BH_TRY(dev_alloc(t, b.lv, cap));
+  long long ng = (cap + t->group - 1) / t->group;
+  BH_TRY(dev_alloc(t, b.gbox, 6 * ng));
+  BH_TRY(dev_alloc(t, b.gcount, ng));
+  // scan scratch: 256 digits x sort tiles (4096 per tile) or 23 levels x tree tiles (512 per tile)
+  long long s1 = 256 * ((cap + 4095) / 4096), s2 = (long long)NLEVELS * ((cap + 511) / 512);
+  t->scan_cap = (s1 > s2 ? s1 : s2) + 4096;
+  BH_TRY(dev_alloc(t, b.scan_tmp, t->scan_cap));
+  BH_TRY(dev_alloc(t, b.scan_blk, t->scan_cap / 4096 + 16));
+  t->cap = cap;
+  t->have_vel = false;
+  t->have_force = false;
+  t->built = false;
+  return 0;
+}
+
+int ensure_cells(tree_ctx *t, long long nc) {
+  if (nc <= t->cell_cap) return 0;
+  long long cap = nc + nc / 4 + 1024;
+  Buffers &b = t->b;
+  BH_TRY(dev_alloc(t, b.c_level, cap));
+  BH_TRY(dev_alloc(t, b.c_first, cap));
+  BH_TRY(dev_alloc(t, b.c_count, cap));
+  BH_TRY(dev_alloc(t, b.c_fcall, cap + 1));
+  BH_TRY(dev_alloc(t, b.c_link, cap));
+  BH_TRY(dev_alloc(t, b.c_cm, cap));
+  BH_TRY(dev_alloc(t, b.c_qa, cap));
+  BH_TRY(dev_alloc(t, b.c_qb, cap));
+  BH_TRY(dev_alloc(t, b.c_test, cap));
+  t->cell_cap = cap;
+  return 0;
+}
+
+static void free_all(tree_ctx *t) {
+  Buffers &b = t->b;
+  void *ptrs[] = {b.posm, b.vel, b.acc, b.key[0], b.key[1], b.idx[0], b.idx[1], b.scan_tmp, b.scan_blk, b.spos, b.sacc,
+                  b.lv, b.gbox, b.gcount, b.c_level, b.c_first, b.c_count, b.c_fcall, b.c_link, b.c_cm, b.c_qa, b.c_qb,
+                  b.c_test, b.in_pos, b.in_mass, b.out_acc, b.out_pot};
+  for (void *p : ptrs) if (p) cudaFree(p);
+  b = Buffers();
+}
+
+static inline void rec(tree_ctx *t, int e) { if (t->ev_valid[e]) cudaEventRecord(t->ev[e], t->stream); }
+
+static int build_from_posm(tree_ctx *t) {
+  BH_TRY(run_keys(t));
+  rec(t, EV_KEYS);
+  BH_TRY(run_sort(t));
+  rec(t, EV_SORT);
+  BH_TRY(run_permute(t));
+  rec(t, EV_PERM);
+  BH_TRY(run_tree(t));
+  rec(t, EV_BUILD);
+  BH_TRY(run_groups_moments(t));
+  rec(t, EV_MOM);
+  t->built = true;
+  return 0;
+}
+
+static int force_impl(tree_ctx *t, float theta, float eps, float *acc, float *pot) {
+  rec(t, EV_F0);
+  BH_TRY(run_opening(t, theta));
+  BH_TRY(run_walk(t, eps));  // records EV_OPEN before and EV_WALK after the walk kernel
+  BH_TRY(run_unpermute(t, acc, pot));
+  rec(t, EV_UNPERM);
+  t->theta = theta; t->eps = eps;
+  t->have_force = true;
+  return 0;
+}
+
+}  // namespace bh
+
+using namespace bh;
+
+extern "C" {
+
+int tree_create(tree_ctx **out, int device, void *cuda_stream, int leaf_size, int group_size) {
+  if (!out) return TREE_ERR_ARG;
+  *out = nullptr;
+  if (leaf_size < 1 || leaf_size > 32) return TREE_ERR_ARG;
+  if (group_size != 32 && group_size != 64 && group_size != 128) return TREE_ERR_ARG;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) { cudaGetLastError(); return TREE_ERR_CUDA; }
+  tree_ctx *t = new (std::nothrow) tree_ctx();
+  if (!t) return TREE_ERR_NOMEM;
+  t->device = device;
+  t->stream = (cudaStream_t)cuda_stream;
+  t->leaf = leaf_size;
+  t->group = group_size;
+  for (int i = 0; i < 24; ++i) t->ev_valid[i] = false;
+  for (int i = 0; i < TREE_NPHASE; ++i) t->ms[i] = 0.0;
+  if (cudaSetDevice(device) != cudaSuccess) { delete t; return TREE_ERR_CUDA; }
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) t->sm_count = prop.multiProcessorCount;
+  if (cudaMalloc((void **)&t->d_info, sizeof(DevInfo)) != cudaSuccess ||
+      cudaMallocHost((void **)&t->h_info, sizeof(DevInfo)) != cudaSuccess ||
+      cudaMalloc((void **)&t->d_hlut, 24 * 8) != cudaSuccess) {
+    cudaGetLastError();
+    tree_destroy(t);
+    return TREE_ERR_NOMEM;
+  }
+  cudaMemset(t->d_info, 0, sizeof(DevInfo));
+  memset(t->h_info, 0, sizeof(DevInfo));
+  uint8_t lut[24 * 8];
+  build_hilbert_lut(lut);
+  cudaMemcpy(t->d_hlut, lut, sizeof(lut), cudaMemcpyHostToDevice);
+  for (int i = 0; i < EV_COUNT; ++i) t->ev_valid[i] = cudaEventCreate(&t->ev[i]) == cudaSuccess;
+  *out = t;
+  return TREE_OK;
+}
+
+int tree_destroy(tree_ctx *t) {
+  if (!t) return TREE_ERR_ARG;
+  cudaSetDevice(t->device);
+  cudaStreamSynchronize(t->stream);
+  free_all(t);
+  if (t->d_info) cudaFree(t->d_info);
+  if (t->h_info) cudaFreeHost(t->h_info);
+  if (t->d_hlut) cudaFree(t->d_hlut);
+  for (int i = 0; i < EV_COUNT; ++i) if (t->ev_valid[i]) cudaEventDestroy(t->ev[i]);
+  cudaGetLastError();
+  delete t;
+  return TREE_OK;
+}
+
+int tree_build(tree_ctx *t, const float *pos, const float *mass, long long N) {
+  if (!t) return TREE_ERR_ARG;
+  if (!pos || !mass || N <= 0 || N > 2147483647LL) return set_err(t, TREE_ERR_ARG, "tree_build: bad argument");
+  BH_CUDA(cudaSetDevice(t->device));
+  t->built = false;
+  t->have_force = false;
+  if (N != t->N) t->have_vel = false;
+  BH_TRY(ensure_particles(t, N));
+  t->N = N;
+  t->n_groups = (N + t->group - 1) / t->group;
+  rec(t, EV_B0);
+  BH_TRY(run_pack_bbox(t, pos, mass));
+  return build_from_posm(t);
+}
+
+int tree_force(tree_ctx *t, float theta, float eps, float *acc, float *pot) {
+  if (!t) return TREE_ERR_ARG;
+  if (!(theta >= 0.0f) || !(eps >= 0.0f) || !isfinite(theta) || !isfinite(eps))
+    return set_err(t, TREE_ERR_ARG, "tree_force: theta and eps must be finite and >= 0");
+  if (!t->built) return set_err(t, TREE_ERR_ORDER, "tree_force before tree_build");
+  BH_CUDA(cudaSetDevice(t->device));
+  return force_impl(t, theta, eps, acc, pot);
+}
+
+int tree_leapfrog(tree_ctx *t, float dt) {
+  if (!t) return TREE_ERR_ARG;
+  if (!isfinite(dt)) return set_err(t, TREE_ERR_ARG, "tree_leapfrog: dt not finite");
+  if (!t->built || !t->have_force) return set_err(t, TREE_ERR_ORDER, "tree_leapfrog before tree_build + tree_force");
+  if (!t->have_vel) return set_err(t, TREE_ERR_ORDER, "tree_leapfrog before tree_set_velocity");
+  BH_CUDA(cudaSetDevice(t->device));
+  rec(t, EV_I0);
+  BH_TRY(run_kick_drift(t, dt));
+  rec(t, EV_I1);
+  t->built = false;
+  t->have_force = false;
+  rec(t, EV_B0);
+  BH_TRY(run_bbox_only(t));
+  BH_TRY(build_from_posm(t));
+  BH_TRY(force_impl(t, t->theta, t->eps, nullptr, nullptr));
+  rec(t, EV_I2);
+  BH_TRY(run_kick(t, dt));
+  rec(t, EV_I3);
+  return TREE_OK;
+}
+
+int tree_set_velocity(tree_ctx *t, const float *vel) {
+  if (!t) return TREE_ERR_ARG;
+  if (!vel) return set_err(t, TREE_ERR_ARG, "tree_set_velocity: NULL");
+  if (t->N <= 0 || !t->b.vel) return set_err(t, TREE_ERR_ORDER, "tree_set_velocity before tree_build");
+  BH_CUDA(cudaSetDevice(t->device));
+  BH_TRY(run_set_velocity(t, vel));
+  t->have_vel = true;
+  return TREE_OK;
+}
+
+int tree_get_state(tree_ctx *t, float *pos, float *vel, float *acc, float *pot) {
+  if (!t) return TREE_ERR_ARG;
+  if (t->N <= 0) return set_err(t, TREE_ERR_ORDER, "tree_get_state before tree_build");
+  if (vel && !t->have_vel) return set_err(t, TREE_ERR_ORDER, "tree_get_state: no velocities set");
+  if ((acc || pot) && !t->have_force) return set_err(t, TREE_ERR_ORDER, "tree_get_state: no force computed");
+  BH_CUDA(cudaSetDevice(t->device));
+  return run_get_state(t, pos, vel, acc, pot);
+}
+
+int tree_build_host(tree_ctx *t, const float *pos, const float *mass, long long N) {
+  if (!t) return TREE_ERR_ARG;
+  if (!pos || !mass || N <= 0 || N > 2147483647LL) return set_err(t, TREE_ERR_ARG, "tree_build_host: bad argument");
+  BH_CUDA(cudaSetDevice(t->device));
+  if (N > t->staging_cap) {
+    t->staging_cap = 0;
+    BH_TRY(dev_alloc(t, t->b.in_pos, 3 * N));
+    BH_TRY(dev_alloc(t, t->b.in_mass, N));
+    BH_TRY(dev_alloc(t, t->b.out_acc, 3 * N));
+    BH_TRY(dev_alloc(t, t->b.out_pot, N));
+    t->staging_cap = N;
+  }
+  BH_CUDA(cudaMemcpyAsync(t->b.in_pos, pos, (size_t)N * 12, cudaMemcpyHostToDevice, t->stream));
+  BH_CUDA(cudaMemcpyAsync(t->b.in_mass, mass, (size_t)N * 4, cudaMemcpyHostToDevice, t->stream));
+  return tree_build(t, t->b.in_pos, t->b.in_mass, N);
+}
+
+int tree_force_host(tree_ctx *t, float theta, float eps, float *acc, float *pot) {
+  if (!t) return TREE_ERR_ARG;
+  if (t->staging_cap < t->N || t->N <= 0) return set_err(t, TREE_ERR_ORDER, "tree_force_host before tree_build_host");
+  int rc = tree_force(t, theta, eps, acc ? t->b.out_acc : nullptr, pot ? t->b.out_pot : nullptr);
+  if (rc) return rc;
+  if (acc) BH_CUDA(cudaMemcpyAsync(acc, t->b.out_acc, (size_t)t->N * 12, cudaMemcpyDeviceToHost, t->stream));
+  if (pot) BH_CUDA(cudaMemcpyAsync(pot, t->b.out_pot, (size_t)t->N * 4, cudaMemcpyDeviceToHost, t->stream));
+  BH_CUDA(cudaStreamSynchronize(t->stream));
+  return TREE_OK;
+}
+
+int tree_energy(tree_ctx *t, double *kinetic, double *potential) {
+  if (!t) return TREE_ERR_ARG;
+  if (!t->have_force) return set_err(t, TREE_ERR_ORDER, "tree_energy before tree_force");
+  BH_CUDA(cudaSetDevice(t->device));
+  BH_TRY(run_energy(t));
+  BH_CUDA(cudaMemcpyAsync(t->h_info, t->d_info, sizeof(DevInfo), cudaMemcpyDeviceToHost, t->stream));
+  BH_CUDA(cudaStreamSynchronize(t->stream));
+  if (kinetic) *kinetic = t->h_info->ekin;
+  if (potential) *potential = t->h_info->epot;
+  return TREE_OK;
+}
+
+static int copy_out(tree_ctx *t, void *dst, const void *src, size_t bytes) {
+  BH_CUDA(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, t->stream));
+  BH_CUDA(cudaStreamSynchronize(t->stream));
+  return 0;
+}
+
+int tree_get_debug(tree_ctx *t, int what, void *dst, long long *count) {
+  if (!t) return TREE_ERR_ARG;
+  if (!count) return set_err(t, TREE_ERR_ARG, "tree_get_debug: count is NULL");
+  if (!t->built) return set_err(t, TREE_ERR_ORDER, "tree_get_debug before tree_build");
+  BH_CUDA(cudaSetDevice(t->device));
+  const long long N = t->N, nc = t->n_cells, ng = t->n_groups;
+  switch (what) {
+    case TREE_DBG_KEYS: {
+      *count = N;
+      if (!dst) return 0;
+      // keys live in slot order after the sort: scatter back through `order` on the host
+      std::vector<uint64_t> sk(N);
+      std::vector<uint32_t> ord(N);
+      BH_TRY(copy_out(t, sk.data(), t->b.key[t->sorted], N * 8));
+      BH_TRY(copy_out(t, ord.data(), t->b.idx[t->sorted], N * 4));
+      uint64_t *o = (uint64_t *)dst;
+      for (long long s = 0; s < N; ++s) o[ord[s]] = sk[s];
+      return 0;
+    }
+    case TREE_DBG_ORDER: *count = N; return dst ? copy_out(t, dst, t->b.idx[t->sorted], N * 4) : 0;
+    case TREE_DBG_SORTED_KEYS: *count = N; return dst ? copy_out(t, dst, t->b.key[t->sorted], N * 8) : 0;
+    case TREE_DBG_SORTED_POS: *count = N; return dst ? copy_out(t, dst, t->b.spos, N * 16) : 0;
+    case TREE_DBG_CELLS: {
+      *count = nc;
+      if (!dst) return 0;
+      std::vector<uint8_t> lv(nc);
+      std::vector<uint32_t> first(nc), cnt(nc);
+      std::vector<uint2> link(nc);
+      BH_TRY(copy_out(t, lv.data(), t->b.c_level, nc));
+      BH_TRY(copy_out(t, first.data(), t->b.c_first, nc * 4));
+      BH_TRY(copy_out(t, cnt.data(), t->b.c_count, nc * 4));
+      BH_TRY(copy_out(t, link.data(), t->b.c_link, nc * 8));
+      int32_t *o = (int32_t *)dst;
+      for (long long c = 0; c < nc; ++c) {
+        bool internal = link[c].y & LEAF_FLAG;
+        o[5 * c] = lv[c]; o[5 * c + 1] = (int32_t)first[c]; o[5 * c + 2] = (int32_t)cnt[c];
+        o[5 * c + 3] = internal ? (int32_t)link[c].x : -1;
+        o[5 * c + 4] = internal ? (int32_t)(link[c].y & ~LEAF_FLAG) : 0;
+      }
+      return 0;
+    }
+    case TREE_DBG_MOMENTS: {
+      *count = nc;
+      if (!dst) return 0;
+      std::vector<float4> cm(nc), qa(nc), qb(nc);
+      BH_TRY(copy_out(t, cm.data(), t->b.c_cm, nc * 16));
+      BH_TRY(copy_out(t, qa.data(), t->b.c_qa, nc * 16));
+      BH_TRY(copy_out(t, qb.data(), t->b.c_qb, nc * 16));
+      float *o = (float *)dst;
+      for (long long c = 0; c < nc; ++c) {
+        float *r = o + 11 * c;
+        r[0] = cm[c].w; r[1] = cm[c].x; r[2] = cm[c].y; r[3] = cm[c].z;
+        r[4] = qa[c].x; r[5] = qa[c].y; r[6] = qa[c].z; r[7] = qb[c].x; r[8] = qb[c].y; r[9] = qb[c].z;
+        r[10] = qa[c].w;
+      }
+      return 0;
+    }
+    case TREE_DBG_GROUP_BOXES: *count = ng; return dst ? copy_out(t, dst, t->b.gbox, ng * 24) : 0;
+    case TREE_DBG_COUNTS:
+      if (!t->have_force) return set_err(t, TREE_ERR_ORDER, "counts before tree_force");
+      *count = ng;
+      return dst ? copy_out(t, dst, t->b.gcount, ng * 8) : 0;
+    case TREE_DBG_GRID: {
+      *count = 10;
+      if (!dst) return 0;
+      BH_TRY(copy_out(t, t->h_info, t->d_info, sizeof(DevInfo)));
+      float *o = (float *)dst;
+      for (int d = 0; d < 3; ++d) { o[d] = t->h_info->lo[d]; o[3 + d] = t->h_info->hi[d]; o[6 + d] = t->h_info->origin[d]; }
+      o[9] = (float)t->h_info->k;
+      return 0;
+    }
+    case TREE_DBG_ROPEN2: {
+      if (!t->have_force) return set_err(t, TREE_ERR_ORDER, "ropen2 before tree_force");
+      *count = nc;
+      if (!dst) return 0;
+      std::vector<float4> ts(nc);
+      BH_TRY(copy_out(t, ts.data(), t->b.c_test, nc * 16));
+      float *o = (float *)dst;
+      for (long long c = 0; c < nc; ++c) o[c] = ts[c].w;
+      return 0;
+    }
+    case TREE_DBG_LEVEL_OFFSETS: {
+      *count = NLEVELS + 1;
+      if (!dst) return 0;
+      BH_TRY(copy_out(t, t->h_info, t->d_info, sizeof(DevInfo)));
+      memcpy(dst, t->h_info->level_off, sizeof(int) * (NLEVELS + 1));
+      return 0;
+    }
+    default: return set_err(t, TREE_ERR_ARG, "tree_get_debug: unknown selector");
+  }
+}
+
+int tree_get_stats(tree_ctx *t, double *ms, unsigned long long *n_pp, unsigned long long *n_pc) {
+  if (!t) return TREE_ERR_ARG;
+  BH_CUDA(cudaSetDevice(t->device));
+  BH_CUDA(cudaStreamSynchronize(t->stream));
+  auto el = [&](int a, int b) -> double {
+    if (!t->ev_valid[a] || !t->ev_valid[b]) return 0.0;
+    if (cudaEventQuery(t->ev[a]) != cudaSuccess || cudaEventQuery(t->ev[b]) != cudaSuccess) { cudaGetLastError(); return 0.0; }
+    float f = 0.f;
+    if (cudaEventElapsedTime(&f, t->ev[a], t->ev[b]) != cudaSuccess) { cudaGetLastError(); return 0.0; }
+    return f > 0.f ? (double)f : 0.0;
+  };
+  double *m = t->ms;
+  m[TREE_PH_KEYS] = el(EV_B0, EV_KEYS);
+  m[TREE_PH_SORT] = el(EV_KEYS, EV_SORT);
+  m[TREE_PH_PERMUTE] = el(EV_SORT, EV_PERM);
+  m[TREE_PH_BUILD] = el(EV_PERM, EV_BUILD);
+  m[TREE_PH_MOMENTS] = el(EV_BUILD, EV_MOM);
+  m[TREE_PH_OPENING] = t->have_force ? el(EV_F0, EV_OPEN) : 0.0;
+  m[TREE_PH_WALK] = t->have_force ? el(EV_OPEN, EV_WALK) : 0.0;
+  m[TREE_PH_UNPERMUTE] = t->have_force ? el(EV_WALK, EV_UNPERM) : 0.0;
+  m[TREE_PH_INTEGRATE] = el(EV_I0, EV_I1) + el(EV_I2, EV_I3);
+  m[TREE_PH_TOTAL] = 0.0;
+  for (int i = 0; i < TREE_PH_TOTAL; ++i) m[TREE_PH_TOTAL] += m[i];
+  if (ms) memcpy(ms, m, sizeof(double) * TREE_NPHASE);
+  if (n_pp || n_pc) {
+    BH_CUDA(cudaMemcpy(t->h_info, t->d_info, sizeof(DevInfo), cudaMemcpyDeviceToHost));
+    if (n_pp) *n_pp = t->h_info->n_pp;
+    if (n_pc) *n_pc = t->h_info->n_pc;
+  }
+  return TREE_OK;
+}
+
+long long tree_launch_count(const tree_ctx *t) { return t ? t->launches : 0; }
+
+const char *tree_last_error(const tree_ctx *t) { return t ? t->err.c_str() : ""; }
+
+}  // extern "C"

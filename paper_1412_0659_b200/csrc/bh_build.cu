@@ -1,0 +1,724 @@
+// Tree-build kernels (sm_100a): bounding box, Peano-Hilbert keys, radix sort, permutation,
+// octree construction, groups, multipole moments.  HBM-bandwidth-bound phases.
+// Compiled with -fmad=false: every FP operation that feeds an integer decision or a stored moment
+// is a single IEEE operation in a fixed order (S9, S13).
+#include "bh_common.cuh"
+
+namespace bh {
+
+// ------------------------------------------------------------------------------------------
+// small device helpers
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ int enc_f(float f) {  // order-preserving float -> int
+  int i = __float_as_int(f);
+  return i >= 0 ? i : i ^ 0x7fffffff;
+}
+__device__ __forceinline__ float dec_f(int i) { return __int_as_float(i >= 0 ? i : i ^ 0x7fffffff); }
+
+__device__ __forceinline__ unsigned warp_incl_scan(unsigned v, int lane) {
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    unsigned n = __shfl_up_sync(0xffffffffu, v, o);
+    if (lane >= o) v += n;
+  }
+  return v;
+}
+
+// Grid index of one coordinate (reading S9): one FP32 subtraction, exact power-of-two
+// scale, floor, clamp to [0, 2^21).
+__device__ __forceinline__ int grid_coord(float x, float o, float inv) {
+  float t = __fsub_rn(x, o);
+  float u = __fmul_rn(t, inv);
+  float f = floorf(u);
+  return (f < 0.0f) ? 0 : (f >= 2097152.0f ? 2097151 : (int)f);
+}
+
+// ------------------------------------------------------------------------------------------
+// a1: bounding box (+ packing the caller's arrays into float4 x,y,z,m)
+// ------------------------------------------------------------------------------------------
+__global__ void info_reset_kernel(DevInfo *info) {
+  if (threadIdx.x == 0) {
+    for (int d = 0; d < 3; ++d) { info->lo_enc[d] = 0x7fffffff; info->hi_enc[d] = (int)0x80000000; }
+    info->nonfinite = 0;
+  }
+}
+
+template <bool PACK>
+__global__ void __launch_bounds__(256) bbox_kernel(const float *__restrict__ pos, const float *__restrict__ mass,
+                                                   float4 *__restrict__ posm, long long N, DevInfo *info) {
+  float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+  int bad = 0;
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+    float4 p;
+    if (PACK) {
+      p.x = pos[3 * i]; p.y = pos[3 * i + 1]; p.z = pos[3 * i + 2]; p.w = mass[i];
+      posm[i] = p;
+    } else {
+      p = posm[i];
+    }
+    bad |= !(isfinite(p.x) && isfinite(p.y) && isfinite(p.z) && isfinite(p.w));
+    lo[0] = fminf(lo[0], p.x); hi[0] = fmaxf(hi[0], p.x);
+    lo[1] = fminf(lo[1], p.y); hi[1] = fmaxf(hi[1], p.y);
+    lo[2] = fminf(lo[2], p.z); hi[2] = fmaxf(hi[2], p.z);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      lo[d] = fminf(lo[d], __shfl_xor_sync(0xffffffffu, lo[d], o));
+      hi[d] = fmaxf(hi[d], __shfl_xor_sync(0xffffffffu, hi[d], o));
+    }
+    bad |= __shfl_xor_sync(0xffffffffu, bad, o);
+  }
+  __shared__ float s_lo[8][3], s_hi[8][3];
+  __shared__ int s_bad[8];
+  int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (lane == 0) {
+    for (int d = 0; d < 3; ++d) { s_lo[w][d] = lo[d]; s_hi[w][d] = hi[d]; }
+    s_bad[w] = bad;
+  }
+  __syncthreads();
+  if (threadIdx.x < 3) {
+    int d = threadIdx.x;
+    float l = s_lo[0][d], h = s_hi[0][d];
+    for (int k = 1; k < 8; ++k) { l = fminf(l, s_lo[k][d]); h = fmaxf(h, s_hi[k][d]); }
+    atomicMin(&info->lo_enc[d], enc_f(l));
+    atomicMax(&info->hi_enc[d], enc_f(h));
+  }
+  if (threadIdx.x == 3) {
+    int b = 0;
+    for (int k = 0; k < 8; ++k) b |= s_bad[k];
+    if (b) atomicOr(&info->nonfinite, 1);
+  }
+}
+
+// a2 (first half): cube centred on the bbox, side = smallest power of two > extent (S9).
+__global__ void grid_kernel(DevInfo *info) {
+  if (threadIdx.x != 0) return;
+  double ext = 0.0;
+  float lo[3], hi[3];
+  for (int d = 0; d < 3; ++d) {
+    lo[d] = dec_f(info->lo_enc[d]); hi[d] = dec_f(info->hi_enc[d]);
+    info->lo[d] = lo[d]; info->hi[d] = hi[d];
+    double e = (double)hi[d] - (double)lo[d];
+    if (e > ext) ext = e;
+  }
+  int k = 0;
+  if (ext > 0.0) { int e; frexp(ext, &e); k = e; }
+  if (!(ext >= 0.0) || !isfinite(ext)) { info->nonfinite = 1; k = 0; }
+  info->k = k;
+  double S = ldexp(1.0, k);
+  for (int d = 0; d < 3; ++d) {
+    double c = 0.5 * ((double)lo[d] + (double)hi[d]);
+    info->origin[d] = (float)(c - 0.5 * S);
+  }
+  info->inv = ldexpf(1.0f, KEY_BITS - k);
+}
+
+// a2: Peano-Hilbert key by a 24-state x 8-octant table generated on the host from the
+// Gray-code/rotation recurrence (T3). Table entry = digit | next_state << 3.
+__global__ void __launch_bounds__(256) keys_kernel(const float4 *__restrict__ posm, long long N,
+                                                   const DevInfo *__restrict__ info, const uint8_t *__restrict__ lut_g,
+                                                   uint64_t *__restrict__ key, uint32_t *__restrict__ idx) {
+  __shared__ uint8_t lut[24 * 8];
+  if (threadIdx.x < 24 * 8) lut[threadIdx.x] = lut_g[threadIdx.x];
+  __syncthreads();
+  const float ox = info->origin[0], oy = info->origin[1], oz = info->origin[2], inv = info->inv;
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+    float4 p = posm[i];
+    unsigned ix = grid_coord(p.x, ox, inv), iy = grid_coord(p.y, oy, inv), iz = grid_coord(p.z, oz, inv);
+    // interleave to one octant digit per level: bits z y x
+    uint64_t h = 0;
+    unsigned st = 0;
+#pragma unroll
+    for (int b = KEY_BITS - 1; b >= 0; --b) {
+      unsigned l = (((iz >> b) & 1u) << 2) | (((iy >> b) & 1u) << 1) | ((ix >> b) & 1u);
+      unsigned v = lut[st * 8 + l];
+      h = (h << 3) | (v & 7u);
+      st = v >> 3;
+    }
+    key[i] = h;
+    idx[i] = (uint32_t)i;
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// device-wide exclusive scan of uint32 (in place): reduce -> scan block sums -> apply
+// ------------------------------------------------------------------------------------------
+constexpr int SCAN_THREADS = 512;
+constexpr int SCAN_IPT = 8;
+constexpr int SCAN_TILE = SCAN_THREADS * SCAN_IPT;
+
+__device__ __forceinline__ unsigned block_excl_scan(unsigned v, unsigned *total, unsigned *s_w) {
+  // exclusive scan of one value per thread over the block (SCAN_THREADS threads)
+  int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  unsigned inc = warp_incl_scan(v, lane);
+  if (lane == 31) s_w[w] = inc;
+  __syncthreads();
+  if (w == 0) {
+    unsigned x = (lane < SCAN_THREADS / 32) ? s_w[lane] : 0;
+    unsigned xi = warp_incl_scan(x, lane);
+    s_w[lane] = xi - x;
+    if (lane == 31) s_w[32] = xi;
+  }
+  __syncthreads();
+  unsigned r = inc - v + s_w[w];
+  if (total) *total = s_w[32];
+  return r;
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) scan_reduce_kernel(const uint32_t *__restrict__ a, long long n,
+                                                                    uint32_t *__restrict__ blk) {
+  __shared__ unsigned s_w[33];
+  long long base = (long long)blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_IPT;
+  unsigned s = 0;
+#pragma unroll
+  for (int k = 0; k < SCAN_IPT; ++k) if (base + k < n) s += a[base + k];
+  unsigned tot;
+  block_excl_scan(s, &tot, s_w);
+  if (threadIdx.x == 0) blk[blockIdx.x] = tot;
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) scan_blocks_kernel(uint32_t *__restrict__ blk, int nblk,
+                                                                    uint32_t *__restrict__ total_out) {
+  __shared__ unsigned s_w[33];
+  unsigned carry = 0;
+  for (int b0 = 0; b0 < nblk; b0 += SCAN_THREADS) {
+    int i = b0 + threadIdx.x;
+    unsigned v = (i < nblk) ? blk[i] : 0;
+    unsigned tot;
+    unsigned e = block_excl_scan(v, &tot, s_w);
+    if (i < nblk) blk[i] = e + carry;
+    carry += tot;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0 && total_out) *total_out = carry;
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) scan_apply_kernel(uint32_t *__restrict__ a, long long n,
+                                                                   const uint32_t *__restrict__ blk) {
+  __shared__ unsigned s_w[33];
+  long long base = (long long)blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_IPT;
+  unsigned v[SCAN_IPT], s = 0;
+#pragma unroll
+  for (int k = 0; k < SCAN_IPT; ++k) { v[k] = (base + k < n) ? a[base + k] : 0; s += v[k]; }
+  unsigned e = block_excl_scan(s, nullptr, s_w) + blk[blockIdx.x];
+#pragma unroll
+  for (int k = 0; k < SCAN_IPT; ++k) {
+    if (base + k < n) a[base + k] = e;
+    e += v[k];
+  }
+}
+
+static int device_excl_scan(tree_ctx *t, uint32_t *a, long long n, uint32_t *total_out) {
+  int nblk = (int)((n + SCAN_TILE - 1) / SCAN_TILE);
+  scan_reduce_kernel<<<nblk, SCAN_THREADS, 0, t->stream>>>(a, n, t->b.scan_blk);
+  BH_LAUNCH_CHECK("scan_reduce");
+  scan_blocks_kernel<<<1, SCAN_THREADS, 0, t->stream>>>(t->b.scan_blk, nblk, total_out);
+  BH_LAUNCH_CHECK("scan_blocks");
+  scan_apply_kernel<<<nblk, SCAN_THREADS, 0, t->stream>>>(a, n, t->b.scan_blk);
+  BH_LAUNCH_CHECK("scan_apply");
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------
+// a3: stable LSD radix sort of (key 64-bit, index 32-bit), 8 bits per pass.
+// Per pass: tile histograms -> device-wide scan (digit-major) -> stable tile scatter.
+// ------------------------------------------------------------------------------------------
+constexpr int SORT_THREADS = 512;
+constexpr int SORT_IPT = 8;
+constexpr int SORT_TILE = SORT_THREADS * SORT_IPT;  // 4096
+constexpr int SORT_WARPS = SORT_THREADS / 32;
+constexpr int RADIX = 256;
+
+__global__ void __launch_bounds__(SORT_THREADS) sort_hist_kernel(const uint64_t *__restrict__ kin, long long N,
+                                                                  int shift, int ntiles, uint32_t *__restrict__ hist) {
+  __shared__ unsigned h[RADIX];
+  if (threadIdx.x < RADIX) h[threadIdx.x] = 0;
+  __syncthreads();
+  long long base = (long long)blockIdx.x * SORT_TILE;
+#pragma unroll
+  for (int k = 0; k < SORT_IPT; ++k) {
+    long long p = base + k * SORT_THREADS + threadIdx.x;
+    if (p < N) atomicAdd(&h[(unsigned)(kin[p] >> shift) & 255u], 1u);
+  }
+  __syncthreads();
+  if (threadIdx.x < RADIX) hist[(long long)threadIdx.x * ntiles + blockIdx.x] = h[threadIdx.x];
+}
+
+struct SortSmem {
+  uint64_t key[SORT_TILE];
+  uint32_t val[SORT_TILE];
+  unsigned wc[SORT_WARPS][RADIX];
+  unsigned dstart[RADIX];
+  unsigned gbase[RADIX];
+};
+
+__global__ void __launch_bounds__(SORT_THREADS) sort_scatter_kernel(const uint64_t *__restrict__ kin,
+                                                                     const uint32_t *__restrict__ vin,
+                                                                     uint64_t *__restrict__ kout,
+                                                                     uint32_t *__restrict__ vout,
+                                                                     const uint32_t *__restrict__ scanned, int shift,
+                                                                     long long N, int ntiles) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  SortSmem &sm = *reinterpret_cast<SortSmem *>(smem_raw);
+  const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const unsigned lt = (1u << lane) - 1u;
+  const long long base = (long long)blockIdx.x * SORT_TILE;
+  for (int i = lane; i < RADIX; i += 32) sm.wc[w][i] = 0;
+  if (threadIdx.x < RADIX) sm.gbase[threadIdx.x] = scanned[(long long)threadIdx.x * ntiles + blockIdx.x];
+  __syncwarp();
+  uint64_t key[SORT_IPT];
+  uint32_t val[SORT_IPT];
+  unsigned rank[SORT_IPT];
+  // warp-striped: warp w owns items [w*256, w*256+256) of the tile, item k of lane l at k*32+l
+#pragma unroll
+  for (int k = 0; k < SORT_IPT; ++k) {
+    long long p = base + w * (32 * SORT_IPT) + k * 32 + lane;
+    bool valid = p < N;
+    key[k] = valid ? kin[p] : 0;
+    val[k] = valid ? (vin ? vin[p] : (uint32_t)p) : 0;
+  }
+#pragma unroll
+  for (int k = 0; k < SORT_IPT; ++k) {
+    long long p = base + w * (32 * SORT_IPT) + k * 32 + lane;
+    bool valid = p < N;
+    unsigned d = (unsigned)(key[k] >> shift) & 255u;
+    unsigned act = __ballot_sync(0xffffffffu, valid);
+    unsigned peers = 0, c0 = 0;
+    if (valid) {
+      peers = __match_any_sync(act, d);
+      c0 = sm.wc[w][d];
+    }
+    __syncwarp();
+    if (valid && lane == 31 - __clz(peers)) sm.wc[w][d] = c0 + __popc(peers);
+    __syncwarp();
+    rank[k] = c0 + __popc(peers & lt);
+  }
+  __syncthreads();
+  // per digit: exclusive prefix over warps, tile total
+  if (threadIdx.x < RADIX) {
+    unsigned run = 0;
+#pragma unroll
+    for (int ww = 0; ww < SORT_WARPS; ++ww) {
+      unsigned c = sm.wc[ww][threadIdx.x];
+      sm.wc[ww][threadIdx.x] = run;
+      run += c;
+    }
+    sm.dstart[threadIdx.x] = run;
+  }
+  __syncthreads();
+  if (w == 0) {  // exclusive scan of the 256 digit totals
+    unsigned v[8], s = 0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { v[j] = sm.dstart[lane * 8 + j]; s += v[j]; }
+    unsigned e = warp_incl_scan(s, lane) - s;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { sm.dstart[lane * 8 + j] = e; e += v[j]; }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int k = 0; k < SORT_IPT; ++k) {
+    long long p = base + w * (32 * SORT_IPT) + k * 32 + lane;
+    if (p < N) {
+      unsigned d = (unsigned)(key[k] >> shift) & 255u;
+      unsigned q = sm.dstart[d] + sm.wc[w][d] + rank[k];
+      sm.key[q] = key[k];
+      sm.val[q] = val[k];
+    }
+  }
+  __syncthreads();
+  long long rem = N - base;
+  int cnt = rem < SORT_TILE ? (int)rem : SORT_TILE;
+  for (int j = threadIdx.x; j < cnt; j += SORT_THREADS) {
+    uint64_t kk = sm.key[j];
+    unsigned d = (unsigned)(kk >> shift) & 255u;
+    long long dst = (long long)sm.gbase[d] + (j - sm.dstart[d]);
+    kout[dst] = kk;
+    vout[dst] = sm.val[j];
+  }
+}
+
+// a4: gather the particles into slot order
+__global__ void __launch_bounds__(256) permute_kernel(const float4 *__restrict__ posm, const uint32_t *__restrict__ order,
+                                                      float4 *__restrict__ spos, long long N) {
+  long long s = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (s < N) spos[s] = posm[order[s]];
+}
+
+// ------------------------------------------------------------------------------------------
+// a5: octree from the sorted keys, without a per-level pass over the particles.
+// cd(p) = number of leading 3-bit digits shared by key[p-1] and key[p] (-1 at the ends).
+// Slot s starts cells at levels L0(s) = cd(s)+1 .. Lleaf(s), where Lleaf(s) = 1 + (leaf_size-th
+// largest "common digits with s" among the other particles), capped at 21: the level at which
+// the cell around s first holds <= leaf_size particles (DESIGN.md §Tree construction).
+// ------------------------------------------------------------------------------------------
+constexpr int TREE_THREADS = 512;
+constexpr int TREE_HALO = 32;  // >= max leaf_size
+
+__device__ __forceinline__ int common_digits(const uint64_t *__restrict__ key, long long p, long long N) {
+  if (p <= 0 || p >= N) return -1;
+  uint64_t x = key[p - 1] ^ key[p];
+  if (x == 0) return KEY_BITS;
+  return (__clzll((long long)x) - 1) / 3;
+}
+
+__global__ void __launch_bounds__(TREE_THREADS) tree_levels_kernel(const uint64_t *__restrict__ skey, long long N,
+                                                                    int leaf, int ntiles, uint16_t *__restrict__ lv,
+                                                                    uint32_t *__restrict__ tilecnt) {
+  __shared__ signed char cd[TREE_THREADS + 2 * TREE_HALO + 1];
+  __shared__ unsigned cnt[NLEVELS];
+  const long long base = (long long)blockIdx.x * TREE_THREADS;
+  if (threadIdx.x < NLEVELS) cnt[threadIdx.x] = 0;
+  for (int i = threadIdx.x; i < TREE_THREADS + 2 * TREE_HALO + 1; i += TREE_THREADS)
+    cd[i] = (signed char)common_digits(skey, base - TREE_HALO + i, N);
+  __syncthreads();
+  long long s = base + threadIdx.x;
+  if (s < N) {
+    int i = threadIdx.x + TREE_HALO;
+    int L0 = cd[i] + 1;
+    int lmin = KEY_BITS, rmin = KEY_BITS, li = i, ri = i + 1, v = KEY_BITS;
+    for (int it = 0; it < leaf; ++it) {
+      int cl = min(lmin, (int)cd[li]), cr = min(rmin, (int)cd[ri]);
+      if (cl >= cr) { v = cl; lmin = cl; --li; } else { v = cr; rmin = cr; ++ri; }
+    }
+    int Ll = min(MAX_LEVEL, v + 1);
+    lv[s] = (uint16_t)(L0 | (Ll << 5));
+    for (int l = L0; l <= Ll; ++l) atomicAdd(&cnt[l], 1u);
+  }
+  __syncthreads();
+  if (threadIdx.x < NLEVELS) tilecnt[(long long)threadIdx.x * ntiles + blockIdx.x] = cnt[threadIdx.x];
+}
+
+__global__ void tree_offsets_kernel(const uint32_t *__restrict__ scanned, int ntiles, const uint32_t *__restrict__ total,
+                                    DevInfo *info) {
+  int l = threadIdx.x;
+  if (l < NLEVELS) info->level_off[l] = (int)scanned[(long long)l * ntiles];
+  if (l == NLEVELS) info->level_off[NLEVELS] = (int)*total;
+}
+
+__global__ void __launch_bounds__(TREE_THREADS) tree_emit_kernel(const uint16_t *__restrict__ lv, long long N,
+                                                                  int ntiles, const uint32_t *__restrict__ scanned,
+                                                                  uint8_t *__restrict__ c_level,
+                                                                  uint32_t *__restrict__ c_first,
+                                                                  uint32_t *__restrict__ c_count,
+                                                                  uint32_t *__restrict__ c_fcall) {
+  constexpr int NW = TREE_THREADS / 32;
+  __shared__ uint16_t lvs[TREE_THREADS + TREE_HALO + 1];
+  __shared__ unsigned wbase[NLEVELS][NW];
+  const long long base = (long long)blockIdx.x * TREE_THREADS;
+  const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const unsigned lt = (1u << lane) - 1u;
+  for (int i = threadIdx.x; i < TREE_THREADS + TREE_HALO + 1; i += TREE_THREADS) {
+    long long p = base + i;
+    lvs[i] = (p < N) ? lv[p] : (uint16_t)0;  // L0 = 0 terminates every rightward scan
+  }
+  __syncthreads();
+  const long long s = base + threadIdx.x;
+  const bool valid = s < N;
+  const int me = lvs[threadIdx.x];
+  const int L0 = valid ? (me & 31) : 99, Ll = valid ? (me >> 5) : -1;
+  for (int l = 0; l < NLEVELS; ++l) {
+    unsigned b = __ballot_sync(0xffffffffu, L0 <= l && l <= Ll);
+    if (lane == 0) wbase[l][w] = __popc(b);
+  }
+  __syncthreads();
+  if (threadIdx.x < NLEVELS) {
+    unsigned run = scanned[(long long)threadIdx.x * ntiles + blockIdx.x];
+    for (int ww = 0; ww < NW; ++ww) { unsigned c = wbase[threadIdx.x][ww]; wbase[threadIdx.x][ww] = run; run += c; }
+  }
+  __syncthreads();
+  int lo = L0, hi = Ll;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+    hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+  }
+  if (hi < 0) return;  // whole warp past the end (warp-uniform)
+  if (lo > hi) return;
+  unsigned bcur = __ballot_sync(0xffffffffu, L0 <= lo && lo <= Ll);
+  for (int l = lo; l <= hi; ++l) {
+    unsigned bnext = __ballot_sync(0xffffffffu, L0 <= l + 1 && l + 1 <= Ll);
+    if (L0 <= l && l <= Ll) {
+      unsigned id = wbase[l][w] + __popc(bcur & lt);
+      unsigned child = wbase[l + 1][w] + __popc(bnext & lt);  // level 22 is empty: = n_cells
+      unsigned cnt = 0;
+      if (l == Ll) {  // leaf: extent = up to the next slot that starts a cell at a level <= l
+        long long e = s + 1;
+        int i = threadIdx.x + 1;
+        while (e < N) {
+          int l0 = (i <= TREE_THREADS + TREE_HALO) ? (lvs[i] & 31) : (lv[e] & 31);
+          if (l0 <= l) break;
+          ++e; ++i;
+        }
+        cnt = (unsigned)(e - s);
+      }
+      c_level[id] = (uint8_t)l;
+      c_first[id] = (uint32_t)s;
+      c_count[id] = cnt;
+      c_fcall[id] = child;
+    }
+    bcur = bnext;
+  }
+}
+
+// child links: n_child(c) = fcall[c+1] - fcall[c]; 0 = leaf.
+__global__ void __launch_bounds__(256) tree_link_kernel(long long n_cells, const uint32_t *__restrict__ c_first,
+                                                        const uint32_t *__restrict__ c_count,
+                                                        const uint32_t *__restrict__ c_fcall, uint2 *__restrict__ c_link) {
+  long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (c >= n_cells) return;
+  unsigned f = c_fcall[c];
+  unsigned nx = (c + 1 < n_cells) ? c_fcall[c + 1] : (unsigned)n_cells;
+  unsigned nch = nx - f;
+  c_link[c] = nch ? make_uint2(f, nch | LEAF_FLAG) : make_uint2(c_first[c], c_count[c]);
+}
+
+// ------------------------------------------------------------------------------------------
+// a6: groups = runs of `group` consecutive slots, tight AABB. One warp per group.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) groups_kernel(const float4 *__restrict__ spos, long long N, int group,
+                                                     long long n_groups, float *__restrict__ gbox) {
+  long long g = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5;
+  int lane = threadIdx.x & 31;
+  if (g >= n_groups) return;
+  float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+  for (int j = lane; j < group; j += 32) {
+    long long s = g * group + j;
+    if (s < N) {
+      float4 p = spos[s];
+      lo[0] = fminf(lo[0], p.x); hi[0] = fmaxf(hi[0], p.x);
+      lo[1] = fminf(lo[1], p.y); hi[1] = fmaxf(hi[1], p.y);
+      lo[2] = fminf(lo[2], p.z); hi[2] = fmaxf(hi[2], p.z);
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      lo[d] = fminf(lo[d], __shfl_xor_sync(0xffffffffu, lo[d], o));
+      hi[d] = fmaxf(hi[d], __shfl_xor_sync(0xffffffffu, hi[d], o));
+    }
+  if (lane == 0) {
+    float *o = gbox + 6 * g;
+    o[0] = lo[0]; o[1] = lo[1]; o[2] = lo[2]; o[3] = hi[0]; o[4] = hi[1]; o[5] = hi[2];
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// a7: multipole moments of one level (leaves from particles, internal cells from their children,
+// which are one level deeper and already done).  FP64 accumulation in slot order, one rounding to
+// FP32 per stored value (S13).  Q = sum m d d^T about the FP32-rounded centre of mass (S4).
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) moments_level_kernel(int c0, int c1, int level, const DevInfo *__restrict__ info,
+                                                            const float4 *__restrict__ spos,
+                                                            const uint2 *__restrict__ c_link,
+                                                            const uint32_t *__restrict__ c_first,
+                                                            uint32_t *__restrict__ c_count, float4 *__restrict__ c_cm,
+                                                            float4 *__restrict__ c_qa, float4 *__restrict__ c_qb) {
+  int c = c0 + blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= c1) return;
+  const uint2 lk = c_link[c];
+  double M = 0, s0 = 0, s1 = 0, s2 = 0;
+  double Q0 = 0, Q1 = 0, Q2 = 0, Q3 = 0, Q4 = 0, Q5 = 0;
+  float cx, cy, cz;
+  if (!(lk.y & LEAF_FLAG)) {
+    const unsigned f = lk.x, n = lk.y;
+    for (unsigned p = f; p < f + n; ++p) {
+      float4 q = spos[p];
+      double m = (double)q.w;
+      M = __dadd_rn(M, m);
+      s0 = __dadd_rn(s0, __dmul_rn(m, (double)q.x));
+      s1 = __dadd_rn(s1, __dmul_rn(m, (double)q.y));
+      s2 = __dadd_rn(s2, __dmul_rn(m, (double)q.z));
+    }
+    cx = (float)(s0 / M); cy = (float)(s1 / M); cz = (float)(s2 / M);
+    for (unsigned p = f; p < f + n; ++p) {
+      float4 q = spos[p];
+      double m = (double)q.w;
+      double dx = __dsub_rn((double)q.x, (double)cx), dy = __dsub_rn((double)q.y, (double)cy),
+             dz = __dsub_rn((double)q.z, (double)cz);
+      double mx = __dmul_rn(m, dx), my = __dmul_rn(m, dy), mz = __dmul_rn(m, dz);
+      Q0 = __dadd_rn(Q0, __dmul_rn(mx, dx)); Q1 = __dadd_rn(Q1, __dmul_rn(my, dy)); Q2 = __dadd_rn(Q2, __dmul_rn(mz, dz));
+      Q3 = __dadd_rn(Q3, __dmul_rn(mx, dy)); Q4 = __dadd_rn(Q4, __dmul_rn(mx, dz)); Q5 = __dadd_rn(Q5, __dmul_rn(my, dz));
+    }
+  } else {
+    const unsigned f = lk.x, n = lk.y & ~LEAF_FLAG;
+    unsigned cnt = 0;
+    for (unsigned ch = f; ch < f + n; ++ch) {
+      float4 a = c_cm[ch];
+      double m = (double)a.w;
+      M = __dadd_rn(M, m);
+      s0 = __dadd_rn(s0, __dmul_rn(m, (double)a.x));
+      s1 = __dadd_rn(s1, __dmul_rn(m, (double)a.y));
+      s2 = __dadd_rn(s2, __dmul_rn(m, (double)a.z));
+      cnt += c_count[ch];
+    }
+    c_count[c] = cnt;
+    cx = (float)(s0 / M); cy = (float)(s1 / M); cz = (float)(s2 / M);
+    for (unsigned ch = f; ch < f + n; ++ch) {
+      float4 a = c_cm[ch], qa = c_qa[ch], qb = c_qb[ch];
+      double m = (double)a.w;
+      double dx = __dsub_rn((double)a.x, (double)cx), dy = __dsub_rn((double)a.y, (double)cy),
+             dz = __dsub_rn((double)a.z, (double)cz);
+      double mx = __dmul_rn(m, dx), my = __dmul_rn(m, dy), mz = __dmul_rn(m, dz);
+      Q0 = __dadd_rn(Q0, __dadd_rn((double)qa.x, __dmul_rn(mx, dx)));
+      Q1 = __dadd_rn(Q1, __dadd_rn((double)qa.y, __dmul_rn(my, dy)));
+      Q2 = __dadd_rn(Q2, __dadd_rn((double)qa.z, __dmul_rn(mz, dz)));
+      Q3 = __dadd_rn(Q3, __dadd_rn((double)qb.x, __dmul_rn(mx, dy)));
+      Q4 = __dadd_rn(Q4, __dadd_rn((double)qb.y, __dmul_rn(mx, dz)));
+      Q5 = __dadd_rn(Q5, __dadd_rn((double)qb.z, __dmul_rn(my, dz)));
+    }
+  }
+  // geometric centre of the octant from the grid coordinates of the first particle (T6)
+  const float4 pf = spos[c_first[c]];
+  const float inv = info->inv;
+  const double lc = ldexp(1.0, info->k - level);
+  const int sh = KEY_BITS - level;
+  double qx = (double)(grid_coord(pf.x, info->origin[0], inv) >> sh);
+  double qy = (double)(grid_coord(pf.y, info->origin[1], inv) >> sh);
+  double qz = (double)(grid_coord(pf.z, info->origin[2], inv) >> sh);
+  double gx = __dadd_rn((double)info->origin[0], __dmul_rn(__dadd_rn(qx, 0.5), lc));
+  double gy = __dadd_rn((double)info->origin[1], __dmul_rn(__dadd_rn(qy, 0.5), lc));
+  double gz = __dadd_rn((double)info->origin[2], __dmul_rn(__dadd_rn(qz, 0.5), lc));
+  double ex = __dsub_rn((double)cx, gx), ey = __dsub_rn((double)cy, gy), ez = __dsub_rn((double)cz, gz);
+  double del = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)), __dmul_rn(ez, ez)));
+  float q0 = (float)Q0, q1 = (float)Q1, q2 = (float)Q2;
+  c_cm[c] = make_float4(cx, cy, cz, (float)M);
+  c_qa[c] = make_float4(q0, q1, q2, (float)del);
+  c_qb[c] = make_float4((float)Q3, (float)Q4, (float)Q5, __fadd_rn(__fadd_rn(q0, q1), q2));
+}
+
+// ------------------------------------------------------------------------------------------
+// host launchers
+// ------------------------------------------------------------------------------------------
+static inline int grid_for(tree_ctx *t, long long n, int threads, int per_sm) {
+  long long need = (n + threads - 1) / threads;
+  long long cap = (long long)t->sm_count * per_sm;
+  return (int)(need < cap ? (need > 0 ? need : 1) : cap);
+}
+
+int run_pack_bbox(tree_ctx *t, const float *pos, const float *mass) {
+  info_reset_kernel<<<1, 32, 0, t->stream>>>(t->d_info);
+  BH_LAUNCH_CHECK("info_reset");
+  bbox_kernel<true><<<grid_for(t, t->N, 256, 8), 256, 0, t->stream>>>(pos, mass, t->b.posm, t->N, t->d_info);
+  BH_LAUNCH_CHECK("bbox_pack");
+  return 0;
+}
+
+int run_bbox_only(tree_ctx *t) {
+  info_reset_kernel<<<1, 32, 0, t->stream>>>(t->d_info);
+  BH_LAUNCH_CHECK("info_reset");
+  bbox_kernel<false><<<grid_for(t, t->N, 256, 8), 256, 0, t->stream>>>(nullptr, nullptr, t->b.posm, t->N, t->d_info);
+  BH_LAUNCH_CHECK("bbox");
+  return 0;
+}
+
+int run_keys(tree_ctx *t) {
+  grid_kernel<<<1, 32, 0, t->stream>>>(t->d_info);
+  BH_LAUNCH_CHECK("grid");
+  keys_kernel<<<grid_for(t, t->N, 256, 8), 256, 0, t->stream>>>(t->b.posm, t->N, t->d_info, t->d_hlut, t->b.key[0],
+                                                                 t->b.idx[0]);
+  BH_LAUNCH_CHECK("keys");
+  return 0;
+}
+
+int run_sort(tree_ctx *t) {
+  static bool attr_set = false;
+  if (!attr_set) {
+    BH_CUDA(cudaFuncSetAttribute(sort_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem)));
+    attr_set = true;
+  }
+  const int ntiles = (int)((t->N + SORT_TILE - 1) / SORT_TILE);
+  int cur = 0;
+  for (int pass = 0; pass < 8; ++pass) {
+    const int shift = 8 * pass;
+    sort_hist_kernel<<<ntiles, SORT_THREADS, 0, t->stream>>>(t->b.key[cur], t->N, shift, ntiles, t->b.scan_tmp);
+    BH_LAUNCH_CHECK("sort_hist");
+    int rc = device_excl_scan(t, t->b.scan_tmp, (long long)RADIX * ntiles, nullptr);
+    if (rc) return rc;
+    sort_scatter_kernel<<<ntiles, SORT_THREADS, sizeof(SortSmem), t->stream>>>(
+        t->b.key[cur], pass == 0 ? nullptr : t->b.idx[cur], t->b.key[cur ^ 1], t->b.idx[cur ^ 1], t->b.scan_tmp, shift,
+        t->N, ntiles);
+    BH_LAUNCH_CHECK("sort_scatter");
+    cur ^= 1;
+  }
+  t->sorted = cur;
+  return 0;
+}
+
+int run_permute(tree_ctx *t) {
+  permute_kernel<<<(unsigned)((t->N + 255) / 256), 256, 0, t->stream>>>(t->b.posm, t->b.idx[t->sorted], t->b.spos, t->N);
+  BH_LAUNCH_CHECK("permute");
+  return 0;
+}
+
+int run_tree(tree_ctx *t) {
+  const int ntiles = (int)((t->N + TREE_THREADS - 1) / TREE_THREADS);
+  const uint64_t *skey = t->b.key[t->sorted];
+  tree_levels_kernel<<<ntiles, TREE_THREADS, 0, t->stream>>>(skey, t->N, t->leaf, ntiles, t->b.lv, t->b.scan_tmp);
+  BH_LAUNCH_CHECK("tree_levels");
+  uint32_t *total = t->b.scan_blk + (t->scan_cap / SCAN_TILE + 8);  // spare slot behind the block sums
+  int rc = device_excl_scan(t, t->b.scan_tmp, (long long)NLEVELS * ntiles, total);
+  if (rc) return rc;
+  tree_offsets_kernel<<<1, 32, 0, t->stream>>>(t->b.scan_tmp, ntiles, total, t->d_info);
+  BH_LAUNCH_CHECK("tree_offsets");
+  BH_CUDA(cudaMemcpyAsync(t->h_info, t->d_info, sizeof(DevInfo), cudaMemcpyDeviceToHost, t->stream));
+  BH_CUDA(cudaStreamSynchronize(t->stream));
+  if (t->h_info->nonfinite) return set_err(t, TREE_ERR_NONFINITE, "non-finite position or mass");
+  const long long nc = t->h_info->level_off[NLEVELS];
+  if (nc <= 0 || nc >= (1ll << 28)) return set_err(t, TREE_ERR_ARG, "cell count out of range (needs < 2^28 cells)");
+  rc = ensure_cells(t, nc);
+  if (rc) return rc;
+  t->n_cells = nc;
+  tree_emit_kernel<<<ntiles, TREE_THREADS, 0, t->stream>>>(t->b.lv, t->N, ntiles, t->b.scan_tmp, t->b.c_level,
+                                                           t->b.c_first, t->b.c_count, t->b.c_fcall);
+  BH_LAUNCH_CHECK("tree_emit");
+  tree_link_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, t->stream>>>(nc, t->b.c_first, t->b.c_count, t->b.c_fcall,
+                                                                        t->b.c_link);
+  BH_LAUNCH_CHECK("tree_link");
+  return 0;
+}
+
+int run_groups_moments(tree_ctx *t) {
+  const long long thr = t->n_groups * 32;
+  groups_kernel<<<(unsigned)((thr + 255) / 256), 256, 0, t->stream>>>(t->b.spos, t->N, t->group, t->n_groups, t->b.gbox);
+  BH_LAUNCH_CHECK("groups");
+  const int *off = t->h_info->level_off;
+  for (int l = MAX_LEVEL; l >= 0; --l) {
+    int c0 = off[l], c1 = off[l + 1];
+    if (c1 <= c0) continue;
+    moments_level_kernel<<<(c1 - c0 + 127) / 128, 128, 0, t->stream>>>(c0, c1, l, t->d_info, t->b.spos, t->b.c_link,
+                                                                       t->b.c_first, t->b.c_count, t->b.c_cm, t->b.c_qa,
+                                                                       t->b.c_qb);
+    BH_LAUNCH_CHECK("moments_level");
+  }
+  return 0;
+}
+
+// Hilbert state table from the Gray-code / rotation recurrence (T3), state = e*3 + d.
+void build_hilbert_lut(uint8_t out[24 * 8]) {
+  auto rot_r = [](unsigned x, unsigned k) { k %= 3; return ((x >> k) | (x << (3 - k))) & 7u; };
+  auto rot_l = [](unsigned x, unsigned k) { k %= 3; return ((x << k) | (x >> (3 - k))) & 7u; };
+  auto ones_tail = [](unsigned i) { unsigned n = 0; for (; i & 1u; i >>= 1) ++n; return n; };
+  for (unsigned e = 0; e < 8; ++e)
+    for (unsigned d = 0; d < 3; ++d)
+      for (unsigned l = 0; l < 8; ++l) {
+        unsigned g = rot_r(l ^ e, d + 1);
+        unsigned w = g;  // inverse Gray code on 3 bits
+        w ^= w >> 1;
+        w ^= w >> 2;
+        w &= 7u;
+        unsigned ent = 0, dir = 0;
+        if (w) {
+          unsigned b = 2u * ((w - 1u) >> 1);
+          ent = b ^ (b >> 1);
+          dir = ((w & 1u) ? ones_tail(w) : ones_tail(w - 1u)) % 3u;
+        }
+        unsigned e2 = e ^ rot_l(ent, d + 1);
+        unsigned d2 = (d + dir + 1u) % 3u;
+        out[(e * 3 + d) * 8 + l] = (uint8_t)(w | ((e2 * 3 + d2) << 3));
+      }
+}
+
+}  // namespace bh

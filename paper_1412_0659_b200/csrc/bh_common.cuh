@@ -1,0 +1,127 @@
+// Shared declarations of the CUDA Barnes-Hut library (sm_100a). Product code: nothing here is
+// shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <cstdio>
+#include <string>
+
+#include "../../include/tree.h"
+
+namespace bh {
+
+constexpr int KEY_BITS = 21;      // bits per dimension -> 63-bit Peano-Hilbert key (S8)
+constexpr int MAX_LEVEL = KEY_BITS;
+constexpr int NLEVELS = MAX_LEVEL + 2;  // levels 0..21 exist; level 22 is an always-empty sentinel
+constexpr uint32_t LEAF_FLAG = 0x80000000u;
+
+// Device-resident scalars of one build.
+struct DevInfo {
+  int lo_enc[3], hi_enc[3];  // order-preserving integer encodings of the bbox (atomicMin/Max)
+  int nonfinite;             // set if a non-finite position or mass was seen
+  int k;                     // cube side S = 2^k
+  float lo[3], hi[3], origin[3];
+  float inv;                 // 2^(21-k): grid cells per unit length
+  int level_off[NLEVELS + 1];  // first BFS cell id of each level, then n_cells
+  unsigned long long n_pp, n_pc;  // interaction totals of the last force pass
+  unsigned int group_ticket;      // dynamic group fetch counter of the walk kernel
+  unsigned int pad;
+  double ekin, epot;
+};
+
+struct Buffers {
+  // caller order
+  float4 *posm = nullptr;   // x,y,z,m
+  float4 *vel = nullptr;    // vx,vy,vz,0
+  float4 *acc = nullptr;    // ax,ay,az,phi
+  // sort
+  uint64_t *key[2] = {nullptr, nullptr};
+  uint32_t *idx[2] = {nullptr, nullptr};
+  uint32_t *scan_tmp = nullptr;  // tile histograms / tile level counts (scanned in place)
+  uint32_t *scan_blk = nullptr;  // block sums for the device-wide scan
+  // slot (sorted) order
+  float4 *spos = nullptr;
+  float4 *sacc = nullptr;
+  uint16_t *lv = nullptr;   // per slot: L0 | Lleaf << 5
+  // groups
+  float *gbox = nullptr;    // [n_groups][6]
+  uint2 *gcount = nullptr;  // [n_groups] n_pp, n_pc
+  // cells (BFS order)
+  uint8_t *c_level = nullptr;
+  uint32_t *c_first = nullptr, *c_count = nullptr, *c_fcall = nullptr;
+  uint2 *c_link = nullptr;    // leaf: (first, count); internal: (first_child, n_child | LEAF_FLAG.. see bh_build.cu)
+  float4 *c_cm = nullptr;     // cx,cy,cz,M
+  float4 *c_qa = nullptr;     // Qxx,Qyy,Qzz,delta
+  float4 *c_qb = nullptr;     // Qxy,Qxz,Qyz,tr(Q)
+  float4 *c_test = nullptr;   // cx,cy,cz,r_open^2 (per force call)
+  // host-call staging
+  float *in_pos = nullptr, *in_mass = nullptr, *out_acc = nullptr, *out_pot = nullptr;
+};
+
+}  // namespace bh
+
+struct tree_ctx {
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  int leaf = 16, group = 64;
+  long long N = 0, cap = 0;          // particles, particle capacity
+  long long n_cells = 0, cell_cap = 0;
+  long long n_groups = 0;
+  long long scan_cap = 0;
+  int sorted = 0;                    // which of key[]/idx[] holds the sorted result
+  bool built = false, have_vel = false, have_force = false;
+  long long staging_cap = 0;         // capacity of the host-call staging buffers
+  float theta = 0.f, eps = 0.f;
+  int sm_count = 148;
+  bh::Buffers b;
+  bh::DevInfo *d_info = nullptr;
+  bh::DevInfo *h_info = nullptr;     // pinned
+  uint8_t *d_hlut = nullptr;         // Hilbert state table (device copy)
+  cudaEvent_t ev[24];
+  bool ev_valid[24];
+  double ms[TREE_NPHASE];
+  long long launches = 0;
+  std::string err;
+};
+
+namespace bh {
+
+// event slots
+enum { EV_B0 = 0, EV_KEYS, EV_SORT, EV_PERM, EV_BUILD, EV_MOM, EV_F0, EV_OPEN, EV_WALK, EV_UNPERM,
+       EV_I0, EV_I1, EV_I2, EV_I3, EV_COUNT };
+
+int set_err(tree_ctx *t, int code, const char *what, cudaError_t ce = cudaSuccess);
+
+#define BH_CUDA(call)                                                      \
+  do {                                                                     \
+    cudaError_t _e = (call);                                               \
+    if (_e != cudaSuccess) return bh::set_err(t, TREE_ERR_CUDA, #call, _e); \
+  } while (0)
+
+#define BH_LAUNCH_CHECK(name)                                                   \
+  do {                                                                          \
+    cudaError_t _e = cudaGetLastError();                                        \
+    if (_e != cudaSuccess) return bh::set_err(t, TREE_ERR_CUDA, name, _e);      \
+    t->launches++;                                                              \
+  } while (0)
+
+// phases implemented in bh_build.cu / bh_force.cu (host launchers; all enqueue on t->stream)
+int run_pack_bbox(tree_ctx *t, const float *pos, const float *mass);  // caller arrays -> posm + bbox
+int run_bbox_only(tree_ctx *t);                                        // bbox of posm (leapfrog rebuild)
+int run_keys(tree_ctx *t);
+int run_sort(tree_ctx *t);
+int run_permute(tree_ctx *t);
+int run_tree(tree_ctx *t);      // octree construction; synchronises once (cell count)
+int run_groups_moments(tree_ctx *t);
+int run_opening(tree_ctx *t, float theta);
+int run_walk(tree_ctx *t, float eps);
+int run_unpermute(tree_ctx *t, float *acc, float *pot);
+int run_kick_drift(tree_ctx *t, float dt);
+int run_kick(tree_ctx *t, float dt);
+int run_energy(tree_ctx *t);
+int run_set_velocity(tree_ctx *t, const float *vel);
+int run_get_state(tree_ctx *t, float *pos, float *vel, float *acc, float *pot);
+int ensure_cells(tree_ctx *t, long long n_cells);
+void build_hilbert_lut(uint8_t out[24 * 8]);
+
+}  // namespace bh

@@ -1,0 +1,506 @@
+// Force-pass kernels (sm_100a): opening radii, the fused tree-walk + force kernel, un-permute,
+// leapfrog and energy.  The walk+force kernel is bound by the FP32 FMA pipe;
+// it is not a dense contraction, so no tensor cores (north_star).
+#include "bh_common.cuh"
+
+namespace bh {
+
+__device__ __forceinline__ unsigned warp_incl_scan_u(unsigned v, int lane) {
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    unsigned n = __shfl_up_sync(0xffffffffu, v, o);
+    if (lane >= o) v += n;
+  }
+  return v;
+}
+
+// ------------------------------------------------------------------------------------------
+// a8: opening radius per cell for this theta, packed with the centre of mass into the 16-byte
+// test record (T9): r = l_c / theta; r = r + delta; r_open^2 = r * r, each one IEEE op.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) opening_kernel(long long n_cells, const DevInfo *__restrict__ info, float theta,
+                                                      const uint8_t *__restrict__ c_level,
+                                                      const float4 *__restrict__ c_cm, const float4 *__restrict__ c_qa,
+                                                      float4 *__restrict__ c_test) {
+  long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (c >= n_cells) return;
+  float lc = ldexpf(1.0f, info->k - (int)c_level[c]);
+  float r = __fdiv_rn(lc, theta);
+  r = __fadd_rn(r, c_qa[c].w);
+  float4 cm = c_cm[c];
+  c_test[c] = make_float4(cm.x, cm.y, cm.z, __fmul_rn(r, r));
+}
+
+// ------------------------------------------------------------------------------------------
+// a9 + a10: fused walk + force. One warp per group of 32*TPL consecutive slots.
+//
+// Walk: a per-warp stack of child RANGES (first_cell << 3 | n-1) in shared memory. Each step pops
+// exactly min(32, cells on the stack) cells (splitting the straddling range), tests one cell per
+// lane against the group's AABB, and by ballot/prefix compaction appends accepted cells to the
+// p-c queue, opened leaves (as particle ranges) to the p-p queue and the child ranges of opened
+// internal cells to the stack (deeper ranges on top, so each level holds at most 32 ranges and
+// the stack never exceeds 32 * 22 entries: DESIGN.md §Walk).
+// Evaluate: whenever a queue holds >= 32 sources, 32 of them are staged in shared memory as float4
+// and every lane evaluates them against its TPL targets with broadcast LDS.128 loads.
+// ------------------------------------------------------------------------------------------
+constexpr int WALK_WARPS = 4;
+constexpr int STACK_CAP = 32 * (MAX_LEVEL + 1);
+
+struct __align__(16) WarpSmem {
+  float4 pc0[32], pc1[32], pc2[32];  // cx,cy,cz,M | Qxx,Qyy,Qzz,T/2 | Qxy,Qxz,Qyz,-3T/2
+  float4 pp[32];                     // x,y,z,m
+  uint32_t ppidx[32];                // slot of each staged p-p source (self-skip by index, S2)
+  uint2 ppq[64];                     // pending particle ranges (first, count)
+  uint32_t pcq[64];                  // pending accepted cells
+  uint32_t stack[STACK_CAP];
+};
+
+struct WalkParams {
+  const float4 *spos;
+  const float4 *c_test;
+  const uint2 *c_link;
+  const float4 *c_cm, *c_qa, *c_qb;
+  const float *gbox;
+  float4 *sacc;
+  uint2 *gcount;
+  DevInfo *info;
+  long long N;
+  unsigned n_groups;
+  float eps2;
+};
+
+template <int TPL>
+struct Targets {
+  float x[TPL], y[TPL], z[TPL];
+  float ax[TPL], ay[TPL], az[TPL], ph[TPL];
+  uint32_t slot[TPL];
+};
+
+template <int TPL, bool MASK>
+__device__ __forceinline__ void pp_one(const float4 s, uint32_t sidx, Targets<TPL> &T, float eps2) {
+#pragma unroll
+  for (int t = 0; t < TPL; ++t) {
+    float dx = s.x - T.x[t], dy = s.y - T.y[t], dz = s.z - T.z[t];
+    float r2 = fmaf(dx, dx, eps2);
+    r2 = fmaf(dy, dy, r2);
+    r2 = fmaf(dz, dz, r2);
+    float m = s.w;
+    if (MASK) {
+      if (sidx == T.slot[t]) { m = 0.0f; r2 = 1.0f; }
+    }
+    float ri = rsqrtf(r2);
+    float ri2 = ri * ri;
+    float mr = m * ri;
+    float mr3 = mr * ri2;
+    T.ax[t] = fmaf(mr3, dx, T.ax[t]);
+    T.ay[t] = fmaf(mr3, dy, T.ay[t]);
+    T.az[t] = fmaf(mr3, dz, T.az[t]);
+    T.ph[t] -= mr;
+  }
+}
+
+template <int TPL>
+__device__ __forceinline__ void pc_one(const float4 a, const float4 b, const float4 c, Targets<TPL> &T, float eps2) {
+#pragma unroll
+  for (int t = 0; t < TPL; ++t) {
+    float dx = a.x - T.x[t], dy = a.y - T.y[t], dz = a.z - T.z[t];
+    float r2 = fmaf(dx, dx, eps2);
+    r2 = fmaf(dy, dy, r2);
+    r2 = fmaf(dz, dz, r2);
+    float ri = rsqrtf(r2);
+    float ri2 = ri * ri;
+    float vx = fmaf(c.y, dz, fmaf(c.x, dy, b.x * dx));
+    float vy = fmaf(c.z, dz, fmaf(b.y, dy, c.x * dx));
+    float vz = fmaf(b.z, dz, fmaf(c.z, dy, c.y * dx));
+    float q = fmaf(dz, vz, fmaf(dy, vy, dx * vx));
+    float ri3 = ri * ri2;
+    float ri5 = ri3 * ri2;
+    float u = q * ri5;
+    float mr = a.w * ri;
+    float p = fmaf(b.w, ri3, -mr);   // -M rho + T/2 rho^3
+    p = fmaf(-1.5f, u, p);           // - 3/2 q rho^5
+    T.ph[t] += p;
+    float g = a.w * ri3;             // M rho^3
+    g = fmaf(c.w, ri5, g);           // - 3/2 T rho^5
+    float w7 = u * ri2;              // q rho^7
+    g = fmaf(7.5f, w7, g);
+    float k = -3.0f * ri5;
+    T.ax[t] = fmaf(k, vx, fmaf(g, dx, T.ax[t]));
+    T.ay[t] = fmaf(k, vy, fmaf(g, dy, T.ay[t]));
+    T.az[t] = fmaf(k, vz, fmaf(g, dz, T.az[t]));
+  }
+}
+
+template <int TPL>
+__device__ __forceinline__ void eval_pp_tile(const WarpSmem &ws, int cnt, bool mask, Targets<TPL> &T, float eps2) {
+  if (!mask && cnt == 32) {
+#pragma unroll 8
+    for (int j = 0; j < 32; ++j) pp_one<TPL, false>(ws.pp[j], 0u, T, eps2);
+  } else if (!mask) {
+    for (int j = 0; j < cnt; ++j) pp_one<TPL, false>(ws.pp[j], 0u, T, eps2);
+  } else {
+#pragma unroll 2
+    for (int j = 0; j < cnt; ++j) pp_one<TPL, true>(ws.pp[j], ws.ppidx[j], T, eps2);
+  }
+}
+
+template <int TPL>
+__device__ __forceinline__ void eval_pc_tile(const WarpSmem &ws, int cnt, Targets<TPL> &T, float eps2) {
+  if (cnt == 32) {
+#pragma unroll 4
+    for (int j = 0; j < 32; ++j) pc_one<TPL>(ws.pc0[j], ws.pc1[j], ws.pc2[j], T, eps2);
+  } else {
+    for (int j = 0; j < cnt; ++j) pc_one<TPL>(ws.pc0[j], ws.pc1[j], ws.pc2[j], T, eps2);
+  }
+}
+
+// Take `want` (<= 32) particles from the back of the p-p range queue and stage them.
+// Returns true if any staged source is one of this group's own slots.
+__device__ __forceinline__ bool stage_pp(WarpSmem &ws, int lane, int &entries, int want, const float4 *__restrict__ spos,
+                                         uint32_t g0, uint32_t gsize) {
+  const bool have = lane < entries;
+  uint2 e = have ? ws.ppq[entries - 1 - lane] : make_uint2(0u, 0u);
+  const unsigned n = have ? min(e.y, 33u) : 0u;  // clamp: only "more than 32" matters
+  const unsigned incl = warp_incl_scan_u(n, lane), excl = incl - n;
+  const bool take = have && excl < (unsigned)want;
+  const bool full = incl <= (unsigned)want;
+  if (take && !full) {
+    unsigned k = (unsigned)want - excl;
+    ws.ppq[entries - 1 - lane] = make_uint2(e.x + k, e.y - k);
+  }
+  entries -= __popc(__ballot_sync(0xffffffffu, take && full));
+  const unsigned head = __reduce_or_sync(0xffffffffu, take ? (1u << excl) : 0u);
+  const int ei = __popc(head & (0xffffffffu >> (31 - lane))) - 1;
+  const unsigned fx = __shfl_sync(0xffffffffu, e.x, ei & 31);
+  const unsigned ex = __shfl_sync(0xffffffffu, excl, ei & 31);
+  const unsigned pidx = fx + ((unsigned)lane - ex);
+  const bool valid = lane < want;
+  if (valid) {
+    ws.pp[lane] = spos[pidx];
+    ws.ppidx[lane] = pidx;
+  }
+  const bool own = valid && (pidx - g0) < gsize;
+  const bool any_own = __any_sync(0xffffffffu, own);
+  __syncwarp();
+  return any_own;
+}
+
+__device__ __forceinline__ void stage_pc(WarpSmem &ws, int lane, int cnt, const WalkParams &P) {
+  if (lane < cnt) {
+    const unsigned c = ws.pcq[lane];
+    const float4 a = P.c_cm[c], qa = P.c_qa[c], qb = P.c_qb[c];
+    ws.pc0[lane] = a;
+    ws.pc1[lane] = make_float4(qa.x, qa.y, qa.z, 0.5f * qb.w);
+    ws.pc2[lane] = make_float4(qb.x, qb.y, qb.z, -1.5f * qb.w);
+  }
+  __syncwarp();
+}
+
+template <int TPL>
+__global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const WalkParams P) {
+  __shared__ WarpSmem smem[WALK_WARPS];
+  WarpSmem &ws = smem[threadIdx.x >> 5];
+  const int lane = threadIdx.x & 31;
+  const unsigned lt = (1u << lane) - 1u;
+  const unsigned gt = ~((lt << 1) | 1u);
+  constexpr unsigned GS = 32u * TPL;
+
+  for (;;) {
+    unsigned g = 0;
+    if (lane == 0) g = atomicAdd(&P.info->group_ticket, 1u);
+    g = __shfl_sync(0xffffffffu, g, 0);
+    if (g >= P.n_groups) break;
+
+    const long long g0 = (long long)g * GS;
+    const long long rem = P.N - g0;
+    const unsigned gsize = rem < (long long)GS ? (unsigned)rem : GS;
+    Targets<TPL> T;
+#pragma unroll
+    for (int t = 0; t < TPL; ++t) {
+      unsigned j = lane + 32u * t;
+      T.slot[t] = (uint32_t)(g0 + j);
+      float4 p = P.spos[g0 + (j < gsize ? j : gsize - 1)];  // padded lanes copy a real target
+      T.x[t] = p.x; T.y[t] = p.y; T.z[t] = p.z;
+      T.ax[t] = T.ay[t] = T.az[t] = T.ph[t] = 0.0f;
+      if (j >= gsize) T.slot[t] = 0xffffffffu;
+    }
+    const float *gb = P.gbox + 6ll * g;
+    const float bx0 = gb[0], by0 = gb[1], bz0 = gb[2], bx1 = gb[3], by1 = gb[4], bz1 = gb[5];
+
+    int sp = 1;
+    if (lane == 0) ws.stack[0] = 0u;  // root: cell 0, one cell
+    __syncwarp();
+    int pp_entries = 0, pp_pending = 0, pc_pending = 0;
+    unsigned n_pp = 0, n_pc = 0;
+
+    while (sp > 0) {
+      // ---- pop exactly min(32, cells on stack) cells
+      const bool have = lane < sp;
+      const unsigned e = have ? ws.stack[sp - 1 - lane] : 0u;
+      const unsigned n = have ? (e & 7u) + 1u : 0u;
+      const unsigned incl = warp_incl_scan_u(n, lane), excl = incl - n;
+      const bool take = have && excl < 32u;
+      const bool full = incl <= 32u;
+      if (take && !full) {
+        unsigned k = 32u - excl;
+        ws.stack[sp - 1 - lane] = (((e >> 3) + k) << 3) | (n - k - 1u);
+      }
+      sp -= __popc(__ballot_sync(0xffffffffu, take && full));
+      const unsigned tot_all = __shfl_sync(0xffffffffu, incl, 31);
+      const unsigned total = tot_all < 32u ? tot_all : 32u;
+      const unsigned head = __reduce_or_sync(0xffffffffu, take ? (1u << excl) : 0u);
+      const int ei = __popc(head & (0xffffffffu >> (31 - lane))) - 1;
+      const unsigned fx = __shfl_sync(0xffffffffu, e >> 3, ei & 31);
+      const unsigned ex = __shfl_sync(0xffffffffu, excl, ei & 31);
+      const bool valid = (unsigned)lane < total;
+      const unsigned cell = fx + ((unsigned)lane - ex);
+
+      // ---- multipole acceptance test (T10), exact op sequence
+      bool accept = false, open_leaf = false, open_int = false;
+      uint2 lk = make_uint2(0u, 0u);
+      if (valid) {
+        const float4 tr = P.c_test[cell];
+        lk = P.c_link[cell];
+        float ux = fmaxf(0.0f, fmaxf(__fsub_rn(bx0, tr.x), __fsub_rn(tr.x, bx1)));
+        float uy = fmaxf(0.0f, fmaxf(__fsub_rn(by0, tr.y), __fsub_rn(tr.y, by1)));
+        float uz = fmaxf(0.0f, fmaxf(__fsub_rn(bz0, tr.z), __fsub_rn(tr.z, bz1)));
+        float d2 = __fmaf_rn(uz, uz, __fmaf_rn(uy, uy, __fmul_rn(ux, ux)));
+        accept = d2 > tr.w;
+        const bool leaf = !(lk.y & LEAF_FLAG);
+        open_leaf = !accept && leaf;
+        open_int = !accept && !leaf;
+      }
+      // ---- opened internal cells: push child ranges, deeper levels on top
+      {
+        const unsigned m = __ballot_sync(0xffffffffu, open_int);
+        if (open_int) ws.stack[sp + __popc(m & gt)] = (lk.x << 3) | ((lk.y & 0xfu) - 1u);
+        sp += __popc(m);
+      }
+      // ---- accepted cells -> p-c queue
+      {
+        const unsigned m = __ballot_sync(0xffffffffu, accept);
+        if (accept) ws.pcq[pc_pending + __popc(m & lt)] = cell;
+        const int c = __popc(m);
+        pc_pending += c;
+        n_pc += c;
+      }
+      // ---- opened leaves -> p-p range queue
+      {
+        const unsigned m = __ballot_sync(0xffffffffu, open_leaf);
+        if (open_leaf) ws.ppq[pp_entries + __popc(m & lt)] = lk;
+        pp_entries += __popc(m);
+        const unsigned c = __reduce_add_sync(0xffffffffu, open_leaf ? lk.y : 0u);
+        pp_pending += (int)c;
+        n_pp += c;
+      }
+      __syncwarp();
+      // ---- evaluate full tiles
+      if (pc_pending >= 32) {
+        stage_pc(ws, lane, 32, P);
+        eval_pc_tile<TPL>(ws, 32, T, P.eps2);
+        __syncwarp();
+        const unsigned mv = (lane + 32 < pc_pending) ? ws.pcq[lane + 32] : 0u;
+        __syncwarp();
+        ws.pcq[lane] = mv;
+        pc_pending -= 32;
+        __syncwarp();
+      }
+      while (pp_pending >= 32) {
+        const bool own = stage_pp(ws, lane, pp_entries, 32, P.spos, (uint32_t)g0, gsize);
+        eval_pp_tile<TPL>(ws, 32, own, T, P.eps2);
+        pp_pending -= 32;
+        __syncwarp();
+      }
+    }
+    // ---- flush partial tiles
+    if (pc_pending > 0) {
+      stage_pc(ws, lane, pc_pending, P);
+      eval_pc_tile<TPL>(ws, pc_pending, T, P.eps2);
+      __syncwarp();
+    }
+    if (pp_pending > 0) {
+      const bool own = stage_pp(ws, lane, pp_entries, pp_pending, P.spos, (uint32_t)g0, gsize);
+      eval_pp_tile<TPL>(ws, pp_pending, own, T, P.eps2);
+      __syncwarp();
+    }
+#pragma unroll
+    for (int t = 0; t < TPL; ++t) {
+      unsigned j = lane + 32u * t;
+      if (j < gsize) P.sacc[g0 + j] = make_float4(T.ax[t], T.ay[t], T.az[t], T.ph[t]);
+    }
+    if (lane == 0) {
+      P.gcount[g] = make_uint2(n_pp, n_pc);
+      atomicAdd(&P.info->n_pp, (unsigned long long)n_pp * gsize);
+      atomicAdd(&P.info->n_pc, (unsigned long long)n_pc * gsize);
+    }
+  }
+}
+
+__global__ void walk_reset_kernel(DevInfo *info) {
+  if (threadIdx.x == 0) { info->group_ticket = 0; info->n_pp = 0; info->n_pc = 0; }
+}
+
+// a11: results back to caller order
+__global__ void __launch_bounds__(256) unpermute_kernel(const float4 *__restrict__ sacc, const uint32_t *__restrict__ order,
+                                                        long long N, float4 *__restrict__ acc4, float *__restrict__ acc,
+                                                        float *__restrict__ pot) {
+  long long s = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (s >= N) return;
+  const float4 a = sacc[s];
+  const long long i = order[s];
+  acc4[i] = a;
+  if (acc) { acc[3 * i] = a.x; acc[3 * i + 1] = a.y; acc[3 * i + 2] = a.z; }
+  if (pot) pot[i] = a.w;
+}
+
+// a12: leapfrog (T12): v = fma(a, dt/2, v); x = fma(v, dt, x)
+__global__ void __launch_bounds__(256) kick_drift_kernel(float4 *__restrict__ posm, float4 *__restrict__ vel,
+                                                         const float4 *__restrict__ acc, long long N, float hdt, float dt) {
+  long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  float4 p = posm[i], v = vel[i];
+  const float4 a = acc[i];
+  v.x = __fmaf_rn(a.x, hdt, v.x); v.y = __fmaf_rn(a.y, hdt, v.y); v.z = __fmaf_rn(a.z, hdt, v.z);
+  p.x = __fmaf_rn(v.x, dt, p.x); p.y = __fmaf_rn(v.y, dt, p.y); p.z = __fmaf_rn(v.z, dt, p.z);
+  vel[i] = v;
+  posm[i] = p;
+}
+
+__global__ void __launch_bounds__(256) kick_kernel(float4 *__restrict__ vel, const float4 *__restrict__ acc, long long N,
+                                                   float hdt) {
+  long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  float4 v = vel[i];
+  const float4 a = acc[i];
+  v.x = __fmaf_rn(a.x, hdt, v.x); v.y = __fmaf_rn(a.y, hdt, v.y); v.z = __fmaf_rn(a.z, hdt, v.z);
+  vel[i] = v;
+}
+
+__global__ void energy_reset_kernel(DevInfo *info) {
+  if (threadIdx.x == 0) { info->ekin = 0.0; info->epot = 0.0; }
+}
+
+__global__ void __launch_bounds__(256) energy_kernel(const float4 *__restrict__ posm, const float4 *__restrict__ vel,
+                                                     const float4 *__restrict__ acc, long long N, bool have_vel,
+                                                     DevInfo *info) {
+  double ke = 0.0, pe = 0.0;
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+    const double m = (double)posm[i].w;
+    if (have_vel) {
+      const float4 v = vel[i];
+      ke += 0.5 * m * ((double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z);
+    }
+    pe += 0.5 * m * (double)acc[i].w;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    ke += __shfl_xor_sync(0xffffffffu, ke, o);
+    pe += __shfl_xor_sync(0xffffffffu, pe, o);
+  }
+  __shared__ double s_k[8], s_p[8];
+  if ((threadIdx.x & 31) == 0) { s_k[threadIdx.x >> 5] = ke; s_p[threadIdx.x >> 5] = pe; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double a = 0, b = 0;
+    for (int k = 0; k < 8; ++k) { a += s_k[k]; b += s_p[k]; }
+    atomicAdd(&info->ekin, a);
+    atomicAdd(&info->epot, b);
+  }
+}
+
+__global__ void __launch_bounds__(256) set_vel_kernel(const float *__restrict__ v3, float4 *__restrict__ vel, long long N) {
+  long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (i < N) vel[i] = make_float4(v3[3 * i], v3[3 * i + 1], v3[3 * i + 2], 0.0f);
+}
+
+__global__ void __launch_bounds__(256) get_state_kernel(const float4 *__restrict__ posm, const float4 *__restrict__ vel,
+                                                        const float4 *__restrict__ acc4, long long N,
+                                                        float *__restrict__ pos, float *__restrict__ v3,
+                                                        float *__restrict__ acc, float *__restrict__ pot) {
+  long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  if (pos) { float4 p = posm[i]; pos[3 * i] = p.x; pos[3 * i + 1] = p.y; pos[3 * i + 2] = p.z; }
+  if (v3) { float4 v = vel[i]; v3[3 * i] = v.x; v3[3 * i + 1] = v.y; v3[3 * i + 2] = v.z; }
+  if (acc || pot) {
+    float4 a = acc4[i];
+    if (acc) { acc[3 * i] = a.x; acc[3 * i + 1] = a.y; acc[3 * i + 2] = a.z; }
+    if (pot) pot[i] = a.w;
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// host launchers
+// ------------------------------------------------------------------------------------------
+static inline unsigned blocks_for(long long n, int threads) { return (unsigned)((n + threads - 1) / threads); }
+
+int run_opening(tree_ctx *t, float theta) {
+  opening_kernel<<<blocks_for(t->n_cells, 256), 256, 0, t->stream>>>(t->n_cells, t->d_info, theta, t->b.c_level,
+                                                                     t->b.c_cm, t->b.c_qa, t->b.c_test);
+  BH_LAUNCH_CHECK("opening");
+  return 0;
+}
+
+int run_walk(tree_ctx *t, float eps) {
+  WalkParams P;
+  P.spos = t->b.spos; P.c_test = t->b.c_test; P.c_link = t->b.c_link;
+  P.c_cm = t->b.c_cm; P.c_qa = t->b.c_qa; P.c_qb = t->b.c_qb;
+  P.gbox = t->b.gbox; P.sacc = t->b.sacc; P.gcount = t->b.gcount; P.info = t->d_info;
+  P.N = t->N; P.n_groups = (unsigned)t->n_groups; P.eps2 = eps * eps;
+  walk_reset_kernel<<<1, 32, 0, t->stream>>>(t->d_info);
+  BH_LAUNCH_CHECK("walk_reset");
+  long long want = (t->n_groups + WALK_WARPS - 1) / WALK_WARPS;
+  long long cap = (long long)t->sm_count * 4;
+  unsigned grid = (unsigned)(want < cap ? want : cap);
+  if (t->ev_valid[EV_OPEN]) cudaEventRecord(t->ev[EV_OPEN], t->stream);
+  switch (t->group) {
+    case 32: walk_force_kernel<1><<<grid, WALK_WARPS * 32, 0, t->stream>>>(P); break;
+    case 64: walk_force_kernel<2><<<grid, WALK_WARPS * 32, 0, t->stream>>>(P); break;
+    case 128: walk_force_kernel<4><<<grid, WALK_WARPS * 32, 0, t->stream>>>(P); break;
+    default: return set_err(t, TREE_ERR_ARG, "group size");
+  }
+  BH_LAUNCH_CHECK("walk_force");
+  if (t->ev_valid[EV_WALK]) cudaEventRecord(t->ev[EV_WALK], t->stream);
+  return 0;
+}
+
+int run_unpermute(tree_ctx *t, float *acc, float *pot) {
+  unpermute_kernel<<<blocks_for(t->N, 256), 256, 0, t->stream>>>(t->b.sacc, t->b.idx[t->sorted], t->N, t->b.acc, acc, pot);
+  BH_LAUNCH_CHECK("unpermute");
+  return 0;
+}
+
+int run_kick_drift(tree_ctx *t, float dt) {
+  kick_drift_kernel<<<blocks_for(t->N, 256), 256, 0, t->stream>>>(t->b.posm, t->b.vel, t->b.acc, t->N, 0.5f * dt, dt);
+  BH_LAUNCH_CHECK("kick_drift");
+  return 0;
+}
+
+int run_kick(tree_ctx *t, float dt) {
+  kick_kernel<<<blocks_for(t->N, 256), 256, 0, t->stream>>>(t->b.vel, t->b.acc, t->N, 0.5f * dt);
+  BH_LAUNCH_CHECK("kick");
+  return 0;
+}
+
+int run_energy(tree_ctx *t) {
+  energy_reset_kernel<<<1, 32, 0, t->stream>>>(t->d_info);
+  BH_LAUNCH_CHECK("energy_reset");
+  long long want = (t->N + 255) / 256, cap = (long long)t->sm_count * 8;
+  energy_kernel<<<(unsigned)(want < cap ? want : cap), 256, 0, t->stream>>>(t->b.posm, t->b.vel, t->b.acc, t->N,
+                                                                          t->have_vel, t->d_info);
+  BH_LAUNCH_CHECK("energy");
+  return 0;
+}
+
+int run_set_velocity(tree_ctx *t, const float *vel) {
+  set_vel_kernel<<<blocks_for(t->N, 256), 256, 0, t->stream>>>(vel, t->b.vel, t->N);
+  BH_LAUNCH_CHECK("set_velocity");
+  return 0;
+}
+
+int run_get_state(tree_ctx *t, float *pos, float *vel, float *acc, float *pot) {
+  get_state_kernel<<<blocks_for(t->N, 256), 256, 0, t->stream>>>(t->b.posm, t->b.vel, t->b.acc, t->N, pos, vel, acc, pot);
+  BH_LAUNCH_CHECK("get_state");
+  return 0;
+}
+
+}  // namespace bh
