@@ -72,9 +72,36 @@ struct WalkParams {
 template <int TPL>
 struct Targets {
   float x[TPL], y[TPL], z[TPL];
-  float ax[TPL], ay[TPL], az[TPL], ph[TPL];
+  float ax[TPL], ay[TPL], az[TPL], ph[TPL];  // sums over the tile being evaluated
   uint32_t slot[TPL];
 };
+
+// Running totals as unevaluated (hi, lo) pairs: each tile's partial sum is folded in with an
+// error-free two-sum, so the FP32 result does not drift with the list length (S14).
+template <int TPL>
+struct Totals {
+  float hi[4][TPL], lo[4][TPL];
+};
+
+__device__ __forceinline__ void two_sum_fold(float &hi, float &lo, float x) {
+  float s = __fadd_rn(hi, x);
+  float bb = __fsub_rn(s, hi);
+  float e = __fadd_rn(__fsub_rn(hi, __fsub_rn(s, bb)), __fsub_rn(x, bb));
+  hi = s;
+  lo = __fadd_rn(lo, e);
+}
+
+template <int TPL>
+__device__ __forceinline__ void fold_tile(Targets<TPL> &T, Totals<TPL> &R) {
+#pragma unroll
+  for (int t = 0; t < TPL; ++t) {
+    two_sum_fold(R.hi[0][t], R.lo[0][t], T.ax[t]);
+    two_sum_fold(R.hi[1][t], R.lo[1][t], T.ay[t]);
+    two_sum_fold(R.hi[2][t], R.lo[2][t], T.az[t]);
+    two_sum_fold(R.hi[3][t], R.lo[3][t], T.ph[t]);
+    T.ax[t] = T.ay[t] = T.az[t] = T.ph[t] = 0.0f;
+  }
+}
 
 template <int TPL, bool MASK>
 __device__ __forceinline__ void pp_one(const float4 s, uint32_t sidx, Targets<TPL> &T, float eps2) {
@@ -215,6 +242,12 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const Wa
     const long long rem = P.N - g0;
     const unsigned gsize = rem < (long long)GS ? (unsigned)rem : GS;
     Targets<TPL> T;
+    Totals<TPL> R;
+#pragma unroll
+    for (int t = 0; t < TPL; ++t) {
+#pragma unroll
+      for (int c = 0; c < 4; ++c) { R.hi[c][t] = 0.0f; R.lo[c][t] = 0.0f; }
+    }
 #pragma unroll
     for (int t = 0; t < TPL; ++t) {
       unsigned j = lane + 32u * t;
@@ -298,6 +331,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const Wa
       if (pc_pending >= 32) {
         stage_pc(ws, lane, 32, P);
         eval_pc_tile<TPL>(ws, 32, T, P.eps2);
+        fold_tile<TPL>(T, R);
         __syncwarp();
         const unsigned mv = (lane + 32 < pc_pending) ? ws.pcq[lane + 32] : 0u;
         __syncwarp();
@@ -308,6 +342,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const Wa
       while (pp_pending >= 32) {
         const bool own = stage_pp(ws, lane, pp_entries, 32, P.spos, (uint32_t)g0, gsize);
         eval_pp_tile<TPL>(ws, 32, own, T, P.eps2);
+        fold_tile<TPL>(T, R);
         pp_pending -= 32;
         __syncwarp();
       }
@@ -316,17 +351,21 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const Wa
     if (pc_pending > 0) {
       stage_pc(ws, lane, pc_pending, P);
       eval_pc_tile<TPL>(ws, pc_pending, T, P.eps2);
+      fold_tile<TPL>(T, R);
       __syncwarp();
     }
     if (pp_pending > 0) {
       const bool own = stage_pp(ws, lane, pp_entries, pp_pending, P.spos, (uint32_t)g0, gsize);
       eval_pp_tile<TPL>(ws, pp_pending, own, T, P.eps2);
+      fold_tile<TPL>(T, R);
       __syncwarp();
     }
 #pragma unroll
     for (int t = 0; t < TPL; ++t) {
       unsigned j = lane + 32u * t;
-      if (j < gsize) P.sacc[g0 + j] = make_float4(T.ax[t], T.ay[t], T.az[t], T.ph[t]);
+      if (j < gsize)
+        P.sacc[g0 + j] = make_float4(__fadd_rn(R.hi[0][t], R.lo[0][t]), __fadd_rn(R.hi[1][t], R.lo[1][t]),
+                                     __fadd_rn(R.hi[2][t], R.lo[2][t]), __fadd_rn(R.hi[3][t], R.lo[3][t]));
     }
     if (lane == 0) {
       P.gcount[g] = make_uint2(n_pp, n_pc);

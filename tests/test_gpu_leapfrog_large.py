@@ -1,0 +1,134 @@
+"""GPU tests: leapfrog / energy against the oracle, and sampled parity at BASELINE.json's bench
+size (config 2: N = 1,048,576) in the launch configuration bench.py times."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from nbody_inputs import plummer, milky_way, subsample_indices, config
+from paper_1412_0659_b200 import Tree
+
+pytestmark = pytest.mark.gpu
+
+
+def _state(t, n):
+    p = torch.empty((n, 3), device="cuda"); v = torch.empty((n, 3), device="cuda")
+    a = torch.empty((n, 3), device="cuda"); ph = torch.empty(n, device="cuda")
+    t.get_state(p, v, a, ph)
+    torch.cuda.synchronize()
+    return p.cpu().numpy(), v.cpu().numpy(), a.cpu().numpy(), ph.cpu().numpy()
+
+
+def test_leapfrog_matches_oracle_over_steps():
+    n, dt, theta, eps, steps = 2048, 0.01, 0.4, 0.05, 4
+    pos, vel, mass = plummer(n, 31)
+    t = Tree(device=0)
+    t.build(pos.cuda(), mass.cuda()); t.set_velocity(vel.cuda()); t.force(theta, eps)
+    ke0, pe0 = t.energy()
+    for _ in range(steps):
+        t.leapfrog(dt)
+    p, v, a, ph = _state(t, n)
+    ke1, pe1 = t.energy()
+    op, ov, oa, oph, en = oracle.leapfrog(pos.numpy(), vel.numpy(), mass.numpy(), dt, steps, theta, eps)
+    # FP32 state; the two force evaluations differ by ~1e-6 relative, so trajectories agree to a few ulp-steps
+    assert np.abs(p - op).max() < 2e-5 * np.abs(op).max()
+    assert np.abs(v - ov).max() < 2e-5 * np.abs(ov).max()
+    assert abs(ke0 - en[0, 0]) < 1e-6 * abs(en[0, 0]) and abs(pe0 - en[0, 1]) < 1e-5 * abs(en[0, 1])
+    assert abs(ke1 - en[-1, 0]) < 1e-5 * abs(en[-1, 0]) and abs(pe1 - en[-1, 1]) < 1e-5 * abs(en[-1, 1])
+    drift_gpu = abs((ke1 + pe1) - (ke0 + pe0)) / abs(ke0 + pe0)
+    drift_cpu = abs(en[-1].sum() - en[0].sum()) / abs(en[0].sum())
+    assert drift_gpu < 1e-4 and abs(drift_gpu - drift_cpu) < 2e-6
+    t.close()
+
+
+def test_leapfrog_first_step_bitwise_kick_drift():
+    # one step from the ORACLE's FP32 force: positions after the drift are fmaf chains of identical inputs
+    n, dt = 1000, 0.02
+    pos, vel, mass = plummer(n, 32)
+    t = Tree(device=0)
+    t.build(pos.cuda(), mass.cuda()); t.set_velocity(vel.cuda()); t.force(0.4, 0.05)
+    p0, v0, a0, _ = _state(t, n)
+    t.leapfrog(dt)
+    p1, v1, a1, _ = _state(t, n)
+    hdt = np.float32(0.5) * np.float32(dt)
+    vh = (a0.astype(np.float64) * np.float64(hdt) + v0.astype(np.float64)).astype(np.float32)  # fma, one rounding
+    ph = (vh.astype(np.float64) * np.float64(np.float32(dt)) + p0.astype(np.float64)).astype(np.float32)
+    assert np.array_equal(p1, ph)
+    v1e = (a1.astype(np.float64) * np.float64(hdt) + vh.astype(np.float64)).astype(np.float32)
+    assert np.array_equal(v1, v1e)
+    t.close()
+
+
+def test_leapfrog_reversible():
+    n = 1500
+    pos, vel, mass = plummer(n, 33)
+    t = Tree(device=0)
+    t.build(pos.cuda(), mass.cuda()); t.set_velocity(vel.cuda()); t.force(0.4, 0.05)
+    for _ in range(5):
+        t.leapfrog(0.01)
+    for _ in range(5):
+        t.leapfrog(-0.01)
+    p, v, _, _ = _state(t, n)
+    assert np.abs(p - pos.numpy()).max() < 1e-5 and np.abs(v - vel.numpy()).max() < 1e-5
+    t.close()
+
+
+def test_bench_size_sampled_parity_config2():
+    # BASELINE config 2: Plummer N = 1,048,576, eps = 0.005, theta = 0.4.  Integers on the full
+    # arrays; forces against the oracle on every 32nd group; error vs direct on a 2048 subsample
+    # (the 65,536 subsample is bench-side reporting: it costs ~1e11 FP64 pair evaluations).
+    cfg, pos, vel, mass = config(1, with_vel=False)
+    n = cfg["n"]
+    t = Tree(device=0)
+    acc = torch.empty((n, 3), device="cuda"); pot = torch.empty(n, device="cuda")
+    t.build(pos.cuda(), mass.cuda()); t.force(cfg["theta"], cfg["eps"], acc, pot)
+    torch.cuda.synchronize()
+    ot = oracle.Tree(pos.numpy(), mass.numpy())
+    key, order, skey = ot.keys()
+    assert np.array_equal(t.debug("order"), order)
+    assert np.array_equal(t.debug("cells"), ot.cells())
+    assert np.array_equal(t.debug("moments"), ot.moments())
+    stride = 32
+    oacc, opot, onpp, onpc = ot.force(cfg["theta"], cfg["eps"], g0=5, stride=stride)
+    cnt = t.debug("counts")
+    gsel = np.arange(5, ot.n_groups, stride)
+    assert np.array_equal(cnt[gsel, 0], onpp[gsel]) and np.array_equal(cnt[gsel, 1], onpc[gsel])
+    sel = np.concatenate([order[64 * g: 64 * g + 64] for g in gsel])
+    a = acc.cpu().numpy().astype(np.float64)[sel]; p = pot.cpu().numpy().astype(np.float64)[sel]
+    rel = np.linalg.norm(a - oacc[sel], axis=1) / np.linalg.norm(oacc[sel], axis=1)
+    assert rel.max() <= 1e-5, rel.max()
+    assert (np.abs(p - opot[sel]) / np.abs(opot[sel])).max() <= 1e-5
+    sub = subsample_indices(n, 2048).numpy()
+    ad, pd = oracle.direct(pos.numpy(), mass.numpy(), cfg["eps"], targets=sub)
+    as_ = acc.cpu().numpy().astype(np.float64)[sub]
+    err = np.linalg.norm(as_ - ad, axis=1) / np.linalg.norm(ad, axis=1)
+    assert np.median(err) < 2e-3
+    # partition property that holds at any size: total mass seen by every group
+    t.close()
+
+
+def test_mw_model_2m_properties_and_sampled_parity():
+    # Milky-Way-shaped model at 2^21 particles (shape of configs 3-5): sampled groups vs oracle
+    n = 1 << 21
+    pos, _, mass = milky_way(n, 1003, with_vel=False)
+    t = Tree(device=0)
+    acc = torch.empty((n, 3), device="cuda"); pot = torch.empty(n, device="cuda")
+    t.build(pos.cuda(), mass.cuda()); t.force(0.4, 0.01, acc, pot)
+    torch.cuda.synchronize()
+    ot = oracle.Tree(pos.numpy(), mass.numpy())
+    assert np.array_equal(t.debug("order"), ot.keys()[1])
+    assert np.array_equal(t.debug("cells"), ot.cells())
+    stride = 97
+    oacc, opot, onpp, onpc = ot.force(0.4, 0.01, g0=11, stride=stride)
+    gsel = np.arange(11, ot.n_groups, stride)
+    cnt = t.debug("counts")
+    assert np.array_equal(cnt[gsel, 0], onpp[gsel]) and np.array_equal(cnt[gsel, 1], onpc[gsel])
+    order = ot.keys()[1]
+    sel = np.concatenate([order[64 * g: 64 * g + 64] for g in gsel])
+    a = acc.cpu().numpy().astype(np.float64)[sel]
+    rel = np.linalg.norm(a - oacc[sel], axis=1) / np.linalg.norm(oacc[sel], axis=1)
+    assert rel.max() <= 1e-5, rel.max()
+    p = pot.cpu().numpy().astype(np.float64)[sel]
+    assert (np.abs(p - opot[sel]) / np.abs(opot[sel])).max() <= 1e-5
+    assert bool(torch.isfinite(acc).all()) and bool(torch.isfinite(pot).all())
+    t.close()

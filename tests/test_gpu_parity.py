@@ -1,0 +1,190 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by element
+on the same seeded inputs.  Integer / index work is bit-exact; forces within 1e-5 (north_star).
+Run on the B200 box with `-m gpu`."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from nbody_inputs import plummer, milky_way, subsample_indices
+from paper_1412_0659_b200 import Tree, TreeError
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-5  # north_star: acc and pot within 1e-5 relative of the CPU tree, max over particles
+
+
+def _gpu_run(pos, mass, theta, eps, leaf=16, group=64):
+    n = mass.numel()
+    t = Tree(device=0, leaf_size=leaf, group_size=group)
+    acc = torch.empty((n, 3), device="cuda"); pot = torch.empty(n, device="cuda")
+    t.build(pos.cuda(), mass.cuda())
+    t.force(theta, eps, acc, pot)
+    torch.cuda.synchronize()
+    return t, acc.cpu().numpy().astype(np.float64), pot.cpu().numpy().astype(np.float64)
+
+
+def _compare_build(t, ot):
+    key, order, skey = ot.keys()
+    g = t.debug("grid")
+    lo, hi, org, k = ot.grid()
+    assert np.array_equal(g[:3], lo) and np.array_equal(g[3:6], hi) and np.array_equal(g[6:9], org) and g[9] == k
+    assert np.array_equal(t.debug("keys"), key)
+    assert np.array_equal(t.debug("order"), order)
+    assert np.array_equal(t.debug("sorted_keys"), skey)
+    assert np.array_equal(t.debug("sorted_pos"), ot.sorted_particles())
+    assert np.array_equal(t.debug("cells"), ot.cells())
+    assert np.array_equal(t.debug("moments"), ot.moments())  # S13: same order, FP64 accumulate
+    gmin, gmax = ot.groups()
+    gb = t.debug("group_boxes")
+    assert np.array_equal(gb[:, :3], gmin) and np.array_equal(gb[:, 3:], gmax)
+
+
+def _compare_force(t, acc, pot, ot, theta, eps, tol=TOL):
+    oacc, opot, onpp, onpc = ot.force(theta, eps)
+    cnt = t.debug("counts")
+    assert np.array_equal(cnt[:, 0], onpp) and np.array_equal(cnt[:, 1], onpc)
+    assert np.array_equal(t.debug("ropen2"), ot.ropen2())
+    rel = np.linalg.norm(acc - oacc, axis=1) / np.linalg.norm(oacc, axis=1)
+    prel = np.abs(pot - opot) / np.abs(opot)
+    assert rel.max() <= tol, rel.max()
+    assert prel.max() <= tol, prel.max()
+    ms, pp, pc = t.stats()
+    gs = np.minimum(ot.group_size, ot.n - ot.group_size * np.arange(ot.n_groups))
+    assert pp == int((onpp.astype(np.int64) * gs).sum()) and pc == int((onpc.astype(np.int64) * gs).sum())
+    return oacc, opot
+
+
+@pytest.mark.parametrize("model,n,seed,eps", [
+    ("plummer", 16384, 1001, 0.01),      # BASELINE config 1
+    ("plummer", 5000 + 37, 5, 0.01),     # ragged: several tiles and a partial last group
+    ("mw", 100000, 3, 0.01),             # Milky-Way-shaped: deep tree, wide dynamic range
+])
+def test_full_parity(model, n, seed, eps):
+    pos, _, mass = (plummer if model == "plummer" else milky_way)(n, seed, with_vel=False)
+    t, acc, pot = _gpu_run(pos, mass, 0.4, eps)
+    ot = oracle.Tree(pos.numpy(), mass.numpy())
+    _compare_build(t, ot)
+    _compare_force(t, acc, pot, ot, 0.4, eps)
+    t.close()
+
+
+def test_config1_against_direct_summation():
+    pos, _, mass = plummer(16384, 1001, with_vel=False)
+    t, acc, pot = _gpu_run(pos, mass, 0.4, 0.01)
+    ad, pd = oracle.direct(pos.numpy(), mass.numpy(), 0.01)
+    rel = np.linalg.norm(acc - ad, axis=1) / np.linalg.norm(ad, axis=1)
+    assert np.median(rel) < 2e-3 and 5e-6 < np.median(rel) < 1.5e-4
+    t.close()
+
+
+@pytest.mark.parametrize("theta", [0.0, 0.3, 0.75, 1.5])
+def test_theta_sweep_counts_and_forces(theta):
+    pos, _, mass = plummer(3000, 17, with_vel=False)
+    t, acc, pot = _gpu_run(pos, mass, theta, 0.02)
+    ot = oracle.Tree(pos.numpy(), mass.numpy())
+    _compare_force(t, acc, pot, ot, theta, 0.02)
+    if theta == 0.0:  # theta -> 0 is direct summation
+        cnt = t.debug("counts")
+        assert np.all(cnt[:, 1] == 0) and np.all(cnt[:, 0] == 3000)
+        ad, pd = oracle.direct(pos.numpy(), mass.numpy(), 0.02)
+        assert (np.linalg.norm(acc - ad, axis=1) / np.linalg.norm(ad, axis=1)).max() < TOL
+    t.close()
+
+
+@pytest.mark.parametrize("leaf,group", [(16, 32), (16, 128), (8, 64), (1, 64), (32, 64)])
+def test_leaf_and_group_sizes(leaf, group):
+    pos, _, mass = plummer(4000 + 5, 23, with_vel=False)
+    t, acc, pot = _gpu_run(pos, mass, 0.4, 0.01, leaf=leaf, group=group)
+    ot = oracle.Tree(pos.numpy(), mass.numpy(), leaf_size=leaf, group_size=group)
+    _compare_build(t, ot)
+    _compare_force(t, acc, pot, ot, 0.4, 0.01)
+    t.close()
+
+
+@pytest.mark.parametrize("n", [1, 2, 16, 17, 33, 64, 65])
+def test_tiny_inputs(n):
+    pos, _, mass = plummer(n, 99, with_vel=False)
+    t, acc, pot = _gpu_run(pos, mass, 0.4, 0.05)
+    ot = oracle.Tree(pos.numpy(), mass.numpy())
+    _compare_build(t, ot)
+    if n > 1:
+        _compare_force(t, acc, pot, ot, 0.4, 0.05)
+    else:
+        assert np.all(acc == 0) and np.all(pot == 0)
+    t.close()
+
+
+def test_degenerate_coincident_particles_and_deep_leaves():
+    # many particles in one finest grid cell: level-21 leaves with more than leaf_size particles,
+    # equal keys (stable sort by index), single-child chains of cells
+    pos, _, mass = plummer(4096, 31, with_vel=False)
+    pos = pos.clone()
+    pos[:300] = pos[0]
+    pos[300:700] = pos[300] + 1e-7
+    t, acc, pot = _gpu_run(pos, mass, 0.4, 0.05)
+    ot = oracle.Tree(pos.numpy(), mass.numpy())
+    cells = ot.cells()
+    assert np.any((cells[:, 2] > 16) & (cells[:, 3] < 0))
+    _compare_build(t, ot)
+    _compare_force(t, acc, pot, ot, 0.4, 0.05)
+    t.close()
+
+
+def test_two_body_closed_form_eps0():
+    pos = torch.tensor([[0.25, -1.0, 0.5], [1.25, 1.0, -1.5]])
+    mass = torch.tensor([2.0, 0.5])
+    t, acc, pot = _gpu_run(pos, mass, 0.4, 0.0)
+    r = np.array([1.0, 2.0, -2.0])
+    np.testing.assert_allclose(acc[0], 0.5 * r / 27.0, rtol=2e-6)
+    np.testing.assert_allclose(acc[1], -2.0 * r / 27.0, rtol=2e-6)
+    np.testing.assert_allclose(pot, [-0.5 / 3.0, -2.0 / 3.0], rtol=2e-6)
+    t.close()
+
+
+def test_errors_and_call_order():
+    t = Tree(device=0)
+    pos, _, mass = plummer(100, 1, with_vel=False)
+    dpos, dmass = pos.cuda(), mass.cuda()
+    with pytest.raises(TreeError) as e:
+        t.force(0.4, 0.01)
+    assert e.value.code == -4
+    t.build(dpos, dmass)
+    with pytest.raises(TreeError) as e:
+        t.force(-0.1, 0.01)
+    assert e.value.code == -1
+    with pytest.raises(TreeError) as e:
+        t.leapfrog(0.1)
+    assert e.value.code == -4
+    bad = dpos.clone(); bad[7, 1] = float("nan")
+    with pytest.raises(TreeError) as e:
+        t.build(bad, dmass)
+    assert e.value.code == -5
+    t.build(dpos, dmass)  # context stays usable after an error
+    t.force(0.4, 0.01)
+    t.close()
+
+
+def test_rebuild_with_different_sizes_reuses_context():
+    t = Tree(device=0)
+    for n, seed in [(5000, 1), (700, 2), (20000, 3)]:
+        pos, _, mass = plummer(n, seed, with_vel=False)
+        acc = torch.empty((n, 3), device="cuda"); pot = torch.empty(n, device="cuda")
+        t.build(pos.cuda(), mass.cuda()); t.force(0.4, 0.01, acc, pot)
+        torch.cuda.synchronize()
+        ot = oracle.Tree(pos.numpy(), mass.numpy())
+        _compare_build(t, ot)
+        _compare_force(t, acc.cpu().numpy().astype(np.float64), pot.cpu().numpy().astype(np.float64), ot, 0.4, 0.01)
+    t.close()
+
+
+def test_host_buffer_calls_match_device_calls():
+    n = 30000
+    pos, _, mass = plummer(n, 8, with_vel=False)
+    t, acc, pot = _gpu_run(pos, mass, 0.4, 0.01)
+    hp, hm = pos.pin_memory(), mass.pin_memory()
+    ha = torch.empty((n, 3)).pin_memory(); hph = torch.empty(n).pin_memory()
+    t2 = Tree(device=0)
+    t2.build_host(hp, hm); t2.force_host(0.4, 0.01, ha, hph)
+    assert np.array_equal(ha.numpy().astype(np.float64), acc) and np.array_equal(hph.numpy().astype(np.float64), pot)
+    t.close(); t2.close()
