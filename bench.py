@@ -246,6 +246,7 @@ def run_ours(args):
     barrier()
     e2e_s = 0.0
     e_pp = e_pc = 0
+    e_phase = {}
     for k in range(args.steps):
         flush.fill_(k & 0xff)
         torch.cuda.synchronize(dev)
@@ -253,7 +254,9 @@ def run_ours(args):
         t2.build_host(h_pos, h_mass)
         t2.force_host(cfg["theta"], cfg["eps"], h_acc, h_pot)  # returns after the D2H copies
         e2e_s += time.perf_counter() - t0
-        _, pp, pc = t2.stats()
+        ems, pp, pc = t2.stats()
+        for key, v in ems.items():
+            e_phase[key] = e_phase.get(key, 0.0) + v / args.steps
         e_pp += pp; e_pc += pc
     te = torch.tensor([e2e_s, float(e_pp + e_pc)], dtype=torch.float64, device=dev)
     if world > 1:
@@ -294,7 +297,7 @@ def run_ours(args):
             "roofline": roof,
             "cpu_baseline": cpu,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 16 * n,
-                    "ms_per_step": 1e3 * e2e_s / args.steps,
+                    "ms_per_step": 1e3 * e2e_s / args.steps, "phase_ms": e_phase,
                     "call": "tree_build_host + tree_force_host (pinned host buffers)"},
             "gpu_launches": launches, "clocks": clocks, "wall_s_timed_region": wall,
         }

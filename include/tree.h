@@ -103,6 +103,8 @@ int tree_energy(tree_ctx *t, double *kinetic, double *potential);
 #define TREE_DBG_ROPEN2 8      /* float[n_cells] squared opening radius of the last tree_force     */
 #define TREE_DBG_SORTED_POS 9  /* float[N][4]   x,y,z,m in slot order                              */
 #define TREE_DBG_LEVEL_OFFSETS 10 /* int32[24]  first cell id of each level 0..22, then n_cells   */
+#define TREE_DBG_TASK_TRACE 11 /* uint32[n_tasks][4] per task of the last force pass: start ns since the
+                                  pass began, duration ns, SM id, group | part << 26 (scheduling trace) */
 int tree_get_debug(tree_ctx *t, int what, void *dst, long long *count);
 
 /* Timings of the last tree_build / tree_force / tree_leapfrog in milliseconds (CUDA events on the
@@ -118,8 +120,9 @@ int tree_get_debug(tree_ctx *t, int what, void *dst, long long *count);
 #define TREE_PH_WALK 6     /* the fused walk + force kernel only */
 #define TREE_PH_UNPERMUTE 7 /* results back to caller order      */
 #define TREE_PH_INTEGRATE 8 /* leapfrog kicks + drift            */
-#define TREE_PH_TOTAL 9    /* sum of the above for the last call sequence */
-#define TREE_NPHASE 10
+#define TREE_PH_SCHED 9    /* counting walk + task list (cost-aware scheduling of the force walk) */
+#define TREE_PH_TOTAL 10   /* sum of the above for the last call sequence */
+#define TREE_NPHASE 11
 int tree_get_stats(tree_ctx *t, double *ms, unsigned long long *n_pp, unsigned long long *n_pc);
 
 /* Number of kernels this library launched on the context since tree_create (for accounting). */

@@ -18,10 +18,10 @@ _lib = None
 FLOP_PP = 23
 FLOP_PC = 65
 
-PHASES = ("keys", "sort", "permute", "build", "moments", "opening", "walk", "unpermute", "integrate", "total")
+PHASES = ("keys", "sort", "permute", "build", "moments", "opening", "walk", "unpermute", "integrate", "sched", "total")
 
 DBG = dict(keys=0, order=1, sorted_keys=2, cells=3, moments=4, group_boxes=5, counts=6, grid=7, ropen2=8,
-           sorted_pos=9, level_offsets=10)
+           sorted_pos=9, level_offsets=10, task_trace=11)
 
 _SIGS = {
     "tree_create": (C.c_int, [C.POINTER(C.c_void_p), C.c_int, C.c_void_p, C.c_int, C.c_int]),
@@ -203,6 +203,7 @@ class Tree:
             "cells": ((n, 5), np.int32), "moments": ((n, 11), np.float32), "group_boxes": ((n, 6), np.float32),
             "counts": ((n, 2), np.uint32), "grid": ((n,), np.float32), "ropen2": ((n,), np.float32),
             "sorted_pos": ((n, 4), np.float32), "level_offsets": ((n,), np.int32),
+            "task_trace": ((n, 4), np.uint32),
         }[what]
         out = np.zeros(shape, dt)
         _check(self.h, load_library().tree_get_debug(self.h, code, _ptr(out), C.byref(cnt)))

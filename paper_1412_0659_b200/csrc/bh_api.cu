@@ -45,6 +45,15 @@ static int ensure_particles(tree_ctx *t, long long N) {
   long long ng = (cap + t->group - 1) / t->group;
   BH_TRY(dev_alloc(t, b.gbox, 6 * ng));
   BH_TRY(dev_alloc(t, b.gcount, ng));
+  if (ng >= (1ll << 26)) return set_err(t, TREE_ERR_ARG, "too many groups (needs < 2^26)");
+  t->part_cap = ng / 8 + 1024;
+  BH_TRY(dev_alloc(t, b.sched_a, ng));
+  BH_TRY(dev_alloc(t, b.sched_b, ng));
+  BH_TRY(dev_alloc(t, b.gdone, ng));
+  BH_TRY(dev_alloc(t, b.gparts, ng));
+  BH_TRY(dev_alloc(t, b.tasks, ng + t->part_cap));
+  BH_TRY(dev_alloc(t, b.part, t->part_cap * t->group));
+  BH_TRY(dev_alloc(t, b.trace, ng + t->part_cap));
   // scan scratch: 256 digits x sort tiles (4096 per tile) or 23 levels x tree tiles (512 per tile)
   long long s1 = 256 * ((cap + 4095) / 4096), s2 = (long long)NLEVELS * ((cap + 511) / 512);
   t->scan_cap = (s1 > s2 ? s1 : s2) + 4096;
@@ -77,7 +86,7 @@ int ensure_cells(tree_ctx *t, long long nc) {
 static void free_all(tree_ctx *t) {
   Buffers &b = t->b;
   void *ptrs[] = {b.posm, b.vel, b.acc, b.key[0], b.key[1], b.idx[0], b.idx[1], b.scan_tmp, b.scan_blk, b.spos, b.sacc,
-                  b.lv, b.gbox, b.gcount, b.c_level, b.c_first, b.c_count, b.c_fcall, b.c_link, b.c_cm, b.c_qa, b.c_qb,
+                  b.lv, b.gbox, b.gcount, b.sched_a, b.sched_b, b.gdone, b.gparts, b.tasks, b.part, b.trace, b.c_level, b.c_first, b.c_count, b.c_fcall, b.c_link, b.c_cm, b.c_qa, b.c_qb,
                   b.c_test, b.in_pos, b.in_mass, b.out_acc, b.out_pot};
   for (void *p : ptrs) if (p) cudaFree(p);
   b = Buffers();
@@ -364,6 +373,12 @@ int tree_get_debug(tree_ctx *t, int what, void *dst, long long *count) {
       memcpy(dst, t->h_info->level_off, sizeof(int) * (NLEVELS + 1));
       return 0;
     }
+    case TREE_DBG_TASK_TRACE: {
+      if (!t->have_force) return set_err(t, TREE_ERR_ORDER, "task trace before tree_force");
+      BH_TRY(copy_out(t, t->h_info, t->d_info, sizeof(DevInfo)));
+      *count = t->h_info->n_tasks;
+      return dst ? copy_out(t, dst, t->b.trace, (size_t)t->h_info->n_tasks * 16) : 0;
+    }
     default: return set_err(t, TREE_ERR_ARG, "tree_get_debug: unknown selector");
   }
 }
@@ -386,7 +401,8 @@ int tree_get_stats(tree_ctx *t, double *ms, unsigned long long *n_pp, unsigned l
   m[TREE_PH_BUILD] = el(EV_PERM, EV_BUILD);
   m[TREE_PH_MOMENTS] = el(EV_BUILD, EV_MOM);
   m[TREE_PH_OPENING] = t->have_force ? el(EV_F0, EV_OPEN) : 0.0;
-  m[TREE_PH_WALK] = t->have_force ? el(EV_OPEN, EV_WALK) : 0.0;
+  m[TREE_PH_SCHED] = t->have_force ? el(EV_OPEN, EV_SCHED) : 0.0;
+  m[TREE_PH_WALK] = t->have_force ? el(EV_SCHED, EV_WALK) : 0.0;
   m[TREE_PH_UNPERMUTE] = t->have_force ? el(EV_WALK, EV_UNPERM) : 0.0;
   m[TREE_PH_INTEGRATE] = el(EV_I0, EV_I1) + el(EV_I2, EV_I3);
   m[TREE_PH_TOTAL] = 0.0;

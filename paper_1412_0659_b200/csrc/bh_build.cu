@@ -210,7 +210,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) scan_apply_kernel(uint32_t *__re
   }
 }
 
-static int device_excl_scan(tree_ctx *t, uint32_t *a, long long n, uint32_t *total_out) {
+int device_excl_scan(tree_ctx *t, uint32_t *a, long long n, uint32_t *total_out) {
   int nblk = (int)((n + SCAN_TILE - 1) / SCAN_TILE);
   scan_reduce_kernel<<<nblk, SCAN_THREADS, 0, t->stream>>>(a, n, t->b.scan_blk);
   BH_LAUNCH_CHECK("scan_reduce");

@@ -24,8 +24,12 @@ struct DevInfo {
   float inv;                 // 2^(21-k): grid cells per unit length
   int level_off[NLEVELS + 1];  // first BFS cell id of each level, then n_cells
   unsigned long long n_pp, n_pc;  // interaction totals of the last force pass
-  unsigned int group_ticket;      // dynamic group fetch counter of the walk kernel
-  unsigned int pad;
+  unsigned long long t0_ns;       // globaltimer at the start of the last force pass (task trace origin)
+  unsigned long long sched_cost;  // sum of the per-group cost estimates of the counting walk
+  unsigned int group_ticket;      // dynamic group fetch counter of the counting walk
+  unsigned int task_ticket;       // dynamic task fetch counter of the force walk
+  unsigned int n_tasks, n_tasks_a;  // tasks in the list; of which parts of split groups (listed first)
+  unsigned int sched_tot[2];      // totals of the two scheduling scans
   double ekin, epot;
 };
 
@@ -46,6 +50,13 @@ struct Buffers {
   // groups
   float *gbox = nullptr;    // [n_groups][6]
   uint2 *gcount = nullptr;  // [n_groups] n_pp, n_pc
+  // scheduling of the force walk
+  uint32_t *sched_a = nullptr, *sched_b = nullptr;  // [n_groups] part counts -> offsets (scanned in place)
+  uint32_t *gdone = nullptr;   // [n_groups]
+  uint8_t *gparts = nullptr;   // [n_groups]
+  uint32_t *tasks = nullptr;   // [n_groups + part_cap]
+  float4 *part = nullptr;      // [part_cap][group]
+  uint4 *trace = nullptr;      // [n_groups + part_cap] per-task trace of the last force pass
   // cells (BFS order)
   uint8_t *c_level = nullptr;
   uint32_t *c_first = nullptr, *c_count = nullptr, *c_fcall = nullptr;
@@ -68,6 +79,7 @@ struct tree_ctx {
   long long n_cells = 0, cell_cap = 0;
   long long n_groups = 0;
   long long scan_cap = 0;
+  long long part_cap = 0;            // tasks that fit the partial-sum buffer
   int sorted = 0;                    // which of key[]/idx[] holds the sorted result
   bool built = false, have_vel = false, have_force = false;
   long long staging_cap = 0;         // capacity of the host-call staging buffers
@@ -87,7 +99,7 @@ struct tree_ctx {
 namespace bh {
 
 // event slots
-enum { EV_B0 = 0, EV_KEYS, EV_SORT, EV_PERM, EV_BUILD, EV_MOM, EV_F0, EV_OPEN, EV_WALK, EV_UNPERM,
+enum { EV_B0 = 0, EV_KEYS, EV_SORT, EV_PERM, EV_BUILD, EV_MOM, EV_F0, EV_OPEN, EV_SCHED, EV_WALK, EV_UNPERM,
        EV_I0, EV_I1, EV_I2, EV_I3, EV_COUNT };
 
 int set_err(tree_ctx *t, int code, const char *what, cudaError_t ce = cudaSuccess);
@@ -123,5 +135,6 @@ int run_set_velocity(tree_ctx *t, const float *vel);
 int run_get_state(tree_ctx *t, float *pos, float *vel, float *acc, float *pot);
 int ensure_cells(tree_ctx *t, long long n_cells);
 void build_hilbert_lut(uint8_t out[24 * 8]);
+int device_excl_scan(tree_ctx *t, uint32_t *a, long long n, uint32_t *total_out);
 
 }  // namespace bh

@@ -44,6 +44,7 @@ __global__ void __launch_bounds__(256) opening_kernel(long long n_cells, const D
 // and every lane evaluates them against its TPL targets with broadcast LDS.128 loads.
 // ------------------------------------------------------------------------------------------
 constexpr int WALK_WARPS = 4;
+constexpr unsigned COUNT_TRUNC = 256;  // the counting walk treats cells this small as opened leaves
 constexpr int STACK_CAP = 32 * (MAX_LEVEL + 1);
 
 struct __align__(16) WarpSmem {
@@ -64,10 +65,19 @@ struct WalkParams {
   float4 *sacc;
   uint2 *gcount;
   DevInfo *info;
+  const uint32_t *c_count; // particles per cell (counting walk only)
+  const uint32_t *tasks;   // task = group | part << TASK_GROUP_BITS
+  const uint8_t *gparts;   // parts per group (1 = not split)
+  uint32_t *gdone;         // finished parts per split group
+  float4 *part;            // partial sums of split groups, [task][group size]
+  uint4 *trace;            // per task: start ns (lo 32), duration ns, SM id, task word (tracing aid)
   long long N;
   unsigned n_groups;
   float eps2;
 };
+
+constexpr unsigned TASK_GROUP_BITS = 26;
+constexpr unsigned TASK_GROUP_MASK = (1u << TASK_GROUP_BITS) - 1u;
 
 template <int TPL>
 struct Targets {
@@ -103,6 +113,14 @@ __device__ __forceinline__ void fold_tile(Targets<TPL> &T, Totals<TPL> &R) {
   }
 }
 
+// MUFU.RSQ without the denormal range fix-up of rsqrtf(): the argument is r^2 + eps^2 of FP32
+// coordinates, never subnormal unless the particles coincide with eps = 0 (excluded by the ABI).
+__device__ __forceinline__ float rsqrt_fast(float x) {
+  float y;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
 template <int TPL, bool MASK>
 __device__ __forceinline__ void pp_one(const float4 s, uint32_t sidx, Targets<TPL> &T, float eps2) {
 #pragma unroll
@@ -115,7 +133,7 @@ __device__ __forceinline__ void pp_one(const float4 s, uint32_t sidx, Targets<TP
     if (MASK) {
       if (sidx == T.slot[t]) { m = 0.0f; r2 = 1.0f; }
     }
-    float ri = rsqrtf(r2);
+    float ri = rsqrt_fast(r2);
     float ri2 = ri * ri;
     float mr = m * ri;
     float mr3 = mr * ri2;
@@ -134,7 +152,7 @@ __device__ __forceinline__ void pc_one(const float4 a, const float4 b, const flo
     float r2 = fmaf(dx, dx, eps2);
     r2 = fmaf(dy, dy, r2);
     r2 = fmaf(dz, dz, r2);
-    float ri = rsqrtf(r2);
+    float ri = rsqrt_fast(r2);
     float ri2 = ri * ri;
     float vx = fmaf(c.y, dz, fmaf(c.x, dy, b.x * dx));
     float vy = fmaf(c.z, dz, fmaf(b.y, dy, c.x * dx));
@@ -181,10 +199,10 @@ __device__ __forceinline__ void eval_pc_tile(const WarpSmem &ws, int cnt, Target
   }
 }
 
-// Take `want` (<= 32) particles from the back of the p-p range queue and stage them.
+// Take `want` (<= 32) particles from the back of the p-p range queue; if `load`, stage them.
 // Returns true if any staged source is one of this group's own slots.
-__device__ __forceinline__ bool stage_pp(WarpSmem &ws, int lane, int &entries, int want, const float4 *__restrict__ spos,
-                                         uint32_t g0, uint32_t gsize) {
+__device__ __forceinline__ bool stage_pp(WarpSmem &ws, int lane, int &entries, int want, bool load,
+                                         const float4 *__restrict__ spos, uint32_t g0, uint32_t gsize) {
   const bool have = lane < entries;
   uint2 e = have ? ws.ppq[entries - 1 - lane] : make_uint2(0u, 0u);
   const unsigned n = have ? min(e.y, 33u) : 0u;  // clamp: only "more than 32" matters
@@ -196,18 +214,20 @@ __device__ __forceinline__ bool stage_pp(WarpSmem &ws, int lane, int &entries, i
     ws.ppq[entries - 1 - lane] = make_uint2(e.x + k, e.y - k);
   }
   entries -= __popc(__ballot_sync(0xffffffffu, take && full));
-  const unsigned head = __reduce_or_sync(0xffffffffu, take ? (1u << excl) : 0u);
-  const int ei = __popc(head & (0xffffffffu >> (31 - lane))) - 1;
-  const unsigned fx = __shfl_sync(0xffffffffu, e.x, ei & 31);
-  const unsigned ex = __shfl_sync(0xffffffffu, excl, ei & 31);
-  const unsigned pidx = fx + ((unsigned)lane - ex);
-  const bool valid = lane < want;
-  if (valid) {
-    ws.pp[lane] = spos[pidx];
-    ws.ppidx[lane] = pidx;
+  bool any_own = false;
+  if (load) {  // warp-uniform
+    const unsigned head = __reduce_or_sync(0xffffffffu, take ? (1u << excl) : 0u);
+    const int ei = __popc(head & (0xffffffffu >> (31 - lane))) - 1;
+    const unsigned fx = __shfl_sync(0xffffffffu, e.x, ei & 31);
+    const unsigned ex = __shfl_sync(0xffffffffu, excl, ei & 31);
+    const unsigned pidx = fx + ((unsigned)lane - ex);
+    const bool valid = lane < want;
+    if (valid) {
+      ws.pp[lane] = spos[pidx];
+      ws.ppidx[lane] = pidx;
+    }
+    any_own = __any_sync(0xffffffffu, valid && (pidx - g0) < gsize);
   }
-  const bool own = valid && (pidx - g0) < gsize;
-  const bool any_own = __any_sync(0xffffffffu, own);
   __syncwarp();
   return any_own;
 }
@@ -223,7 +243,14 @@ __device__ __forceinline__ void stage_pc(WarpSmem &ws, int lane, int cnt, const 
   __syncwarp();
 }
 
-template <int TPL>
+// One kernel, two modes.
+//  COUNT = true : walk only; writes the per-group list lengths (n_pp, n_pc) — the exact cost of
+//                 every group, from which the task list is built (see task kernels below).
+//  COUNT = false: work items are TASKS (group g, part j of s): every part of a group repeats the
+//                 (cheap) walk and evaluates only the source tiles k with k mod s == j, so an
+//                 expensive group is spread over s warps; the parts' partial sums are combined
+//                 in fixed order by the part that finishes last (deterministic).
+template <int TPL, bool COUNT>
 __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const WalkParams P) {
   __shared__ WarpSmem smem[WALK_WARPS];
   WarpSmem &ws = smem[threadIdx.x >> 5];
@@ -231,12 +258,22 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const Wa
   const unsigned lt = (1u << lane) - 1u;
   const unsigned gt = ~((lt << 1) | 1u);
   constexpr unsigned GS = 32u * TPL;
+  const unsigned n_items = COUNT ? P.n_groups : P.info->n_tasks;
 
   for (;;) {
-    unsigned g = 0;
-    if (lane == 0) g = atomicAdd(&P.info->group_ticket, 1u);
-    g = __shfl_sync(0xffffffffu, g, 0);
-    if (g >= P.n_groups) break;
+    unsigned item = 0;
+    if (lane == 0) item = atomicAdd(COUNT ? &P.info->group_ticket : &P.info->task_ticket, 1u);
+    item = __shfl_sync(0xffffffffu, item, 0);
+    if (item >= n_items) break;
+    unsigned g = item, part = 0, nparts = 1;
+    unsigned long long t_start = 0;
+    if (!COUNT) {
+      asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_start));
+      const unsigned tk = P.tasks[item];
+      g = tk & TASK_GROUP_MASK;
+      part = tk >> TASK_GROUP_BITS;
+      nparts = P.gparts[g];
+    }
 
     const long long g0 = (long long)g * GS;
     const long long rem = P.N - g0;
@@ -252,7 +289,8 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const Wa
     for (int t = 0; t < TPL; ++t) {
       unsigned j = lane + 32u * t;
       T.slot[t] = (uint32_t)(g0 + j);
-      float4 p = P.spos[g0 + (j < gsize ? j : gsize - 1)];  // padded lanes copy a real target
+      float4 p = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (!COUNT) p = P.spos[g0 + (j < gsize ? j : gsize - 1)];  // padded lanes copy a real target
       T.x[t] = p.x; T.y[t] = p.y; T.z[t] = p.z;
       T.ax[t] = T.ay[t] = T.az[t] = T.ph[t] = 0.0f;
       if (j >= gsize) T.slot[t] = 0xffffffffu;
@@ -265,6 +303,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const Wa
     __syncwarp();
     int pp_entries = 0, pp_pending = 0, pc_pending = 0;
     unsigned n_pp = 0, n_pc = 0;
+    unsigned tile_wait = part;  // tiles to skip before the next one this part evaluates
 
     while (sp > 0) {
       // ---- pop exactly min(32, cells on stack) cells
@@ -299,7 +338,11 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const Wa
         float uz = fmaxf(0.0f, fmaxf(__fsub_rn(bz0, tr.z), __fsub_rn(tr.z, bz1)));
         float d2 = __fmaf_rn(uz, uz, __fmaf_rn(uy, uy, __fmul_rn(ux, ux)));
         accept = d2 > tr.w;
-        const bool leaf = !(lk.y & LEAF_FLAG);
+        bool leaf = !(lk.y & LEAF_FLAG);
+        if (COUNT && !leaf && !accept) {  // cost estimate: do not descend below small cells
+          const unsigned cc = P.c_count[cell];
+          if (cc <= COUNT_TRUNC) { leaf = true; lk.y = cc; }
+        }
         open_leaf = !accept && leaf;
         open_int = !accept && !leaf;
       }
@@ -312,7 +355,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const Wa
       // ---- accepted cells -> p-c queue
       {
         const unsigned m = __ballot_sync(0xffffffffu, accept);
-        if (accept) ws.pcq[pc_pending + __popc(m & lt)] = cell;
+        if (!COUNT) { if (accept) ws.pcq[pc_pending + __popc(m & lt)] = cell; }
         const int c = __popc(m);
         pc_pending += c;
         n_pc += c;
@@ -320,19 +363,24 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const Wa
       // ---- opened leaves -> p-p range queue
       {
         const unsigned m = __ballot_sync(0xffffffffu, open_leaf);
-        if (open_leaf) ws.ppq[pp_entries + __popc(m & lt)] = lk;
+        if (!COUNT) { if (open_leaf) ws.ppq[pp_entries + __popc(m & lt)] = lk; }
         pp_entries += __popc(m);
         const unsigned c = __reduce_add_sync(0xffffffffu, open_leaf ? lk.y : 0u);
         pp_pending += (int)c;
         n_pp += c;
       }
       __syncwarp();
-      // ---- evaluate full tiles
+      if (COUNT) { pc_pending = 0; pp_pending = 0; pp_entries = 0; continue; }
+      // ---- evaluate full tiles (only those that belong to this part)
       if (pc_pending >= 32) {
-        stage_pc(ws, lane, 32, P);
-        eval_pc_tile<TPL>(ws, 32, T, P.eps2);
-        fold_tile<TPL>(T, R);
-        __syncwarp();
+        const bool mine = tile_wait == 0;
+        tile_wait = mine ? nparts - 1 : tile_wait - 1;
+        if (mine) {
+          stage_pc(ws, lane, 32, P);
+          eval_pc_tile<TPL>(ws, 32, T, P.eps2);
+          fold_tile<TPL>(T, R);
+          __syncwarp();
+        }
         const unsigned mv = (lane + 32 < pc_pending) ? ws.pcq[lane + 32] : 0u;
         __syncwarp();
         ws.pcq[lane] = mv;
@@ -340,43 +388,165 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const Wa
         __syncwarp();
       }
       while (pp_pending >= 32) {
-        const bool own = stage_pp(ws, lane, pp_entries, 32, P.spos, (uint32_t)g0, gsize);
-        eval_pp_tile<TPL>(ws, 32, own, T, P.eps2);
-        fold_tile<TPL>(T, R);
+        const bool mine = tile_wait == 0;
+        tile_wait = mine ? nparts - 1 : tile_wait - 1;
+        const bool own = stage_pp(ws, lane, pp_entries, 32, mine, P.spos, (uint32_t)g0, gsize);
+        if (mine) {
+          eval_pp_tile<TPL>(ws, 32, own, T, P.eps2);
+          fold_tile<TPL>(T, R);
+        }
         pp_pending -= 32;
         __syncwarp();
       }
     }
-    // ---- flush partial tiles
-    if (pc_pending > 0) {
-      stage_pc(ws, lane, pc_pending, P);
-      eval_pc_tile<TPL>(ws, pc_pending, T, P.eps2);
-      fold_tile<TPL>(T, R);
-      __syncwarp();
+    if (COUNT) {
+      if (lane == 0) {
+        const unsigned long long c = 13ull * n_pp + 37ull * n_pc;
+        P.gdone[g] = c > 0xffffffffull ? 0xffffffffu : (unsigned)c;  // read and cleared by task_cost_kernel
+        atomicAdd(&P.info->sched_cost, c);
+      }
+      continue;
     }
-    if (pp_pending > 0) {
-      const bool own = stage_pp(ws, lane, pp_entries, pp_pending, P.spos, (uint32_t)g0, gsize);
-      eval_pp_tile<TPL>(ws, pp_pending, own, T, P.eps2);
-      fold_tile<TPL>(T, R);
-      __syncwarp();
-    }
-#pragma unroll
-    for (int t = 0; t < TPL; ++t) {
-      unsigned j = lane + 32u * t;
-      if (j < gsize)
-        P.sacc[g0 + j] = make_float4(__fadd_rn(R.hi[0][t], R.lo[0][t]), __fadd_rn(R.hi[1][t], R.lo[1][t]),
-                                     __fadd_rn(R.hi[2][t], R.lo[2][t]), __fadd_rn(R.hi[3][t], R.lo[3][t]));
-    }
-    if (lane == 0) {
+    if (part == 0 && lane == 0) {
       P.gcount[g] = make_uint2(n_pp, n_pc);
       atomicAdd(&P.info->n_pp, (unsigned long long)n_pp * gsize);
       atomicAdd(&P.info->n_pc, (unsigned long long)n_pc * gsize);
     }
+    // ---- flush partial tiles
+    if (pc_pending > 0) {
+      const bool mine = tile_wait == 0;
+      tile_wait = mine ? nparts - 1 : tile_wait - 1;
+      if (mine) {
+        stage_pc(ws, lane, pc_pending, P);
+        eval_pc_tile<TPL>(ws, pc_pending, T, P.eps2);
+        fold_tile<TPL>(T, R);
+        __syncwarp();
+      }
+    }
+    if (pp_pending > 0) {
+      const bool mine = tile_wait == 0;
+      if (mine) {
+        const bool own = stage_pp(ws, lane, pp_entries, pp_pending, true, P.spos, (uint32_t)g0, gsize);
+        eval_pp_tile<TPL>(ws, pp_pending, own, T, P.eps2);
+        fold_tile<TPL>(T, R);
+        __syncwarp();
+      }
+    }
+    if (lane == 0) {
+      unsigned long long t_end;
+      unsigned smid;
+      asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_end));
+      asm volatile("mov.u32 %0, %smid;" : "=r"(smid));
+      P.trace[item] = make_uint4((unsigned)(t_start - P.info->t0_ns), (unsigned)(t_end - t_start), smid, P.tasks[item]);
+    }
+    // ---- results
+    float4 res[TPL];
+#pragma unroll
+    for (int t = 0; t < TPL; ++t)
+      res[t] = make_float4(__fadd_rn(R.hi[0][t], R.lo[0][t]), __fadd_rn(R.hi[1][t], R.lo[1][t]),
+                           __fadd_rn(R.hi[2][t], R.lo[2][t]), __fadd_rn(R.hi[3][t], R.lo[3][t]));
+    if (nparts == 1) {
+#pragma unroll
+      for (int t = 0; t < TPL; ++t) {
+        unsigned j = lane + 32u * t;
+        if (j < gsize) P.sacc[g0 + j] = res[t];
+      }
+    } else {
+      // split group: tasks of one group are consecutive and all lie in the partial-sum buffer
+      float4 *mine = P.part + (size_t)item * GS;
+#pragma unroll
+      for (int t = 0; t < TPL; ++t) __stcg(&mine[lane + 32u * t], res[t]);
+      __threadfence();
+      unsigned prev = 0;
+      if (lane == 0) prev = atomicAdd(&P.gdone[g], 1u);
+      prev = __shfl_sync(0xffffffffu, prev, 0);
+      if (prev == nparts - 1) {  // last part to finish: combine in fixed order 0..s-1
+        __threadfence();
+        const float4 *base = P.part + (size_t)(item - part) * GS;
+#pragma unroll
+        for (int t = 0; t < TPL; ++t) {
+          float hi[4] = {0.f, 0.f, 0.f, 0.f}, lo[4] = {0.f, 0.f, 0.f, 0.f};
+          for (unsigned q = 0; q < nparts; ++q) {
+            const float4 v = __ldcg(&base[(size_t)q * GS + lane + 32u * t]);
+            two_sum_fold(hi[0], lo[0], v.x); two_sum_fold(hi[1], lo[1], v.y);
+            two_sum_fold(hi[2], lo[2], v.z); two_sum_fold(hi[3], lo[3], v.w);
+          }
+          unsigned j = lane + 32u * t;
+          if (j < gsize)
+            P.sacc[g0 + j] = make_float4(__fadd_rn(hi[0], lo[0]), __fadd_rn(hi[1], lo[1]), __fadd_rn(hi[2], lo[2]),
+                                         __fadd_rn(hi[3], lo[3]));
+        }
+      }
+    }
   }
 }
 
+// ------------------------------------------------------------------------------------------
+// Task list (scheduling only; results do not depend on it beyond the fixed-order partial sums).
+// cost(g) = 13 n_pp + 37 n_pc (FP32 instructions per target of the two evaluators). A group
+// costing more than SPLIT_AT x mean is cut into s = ceil(cost / (mean x SPLIT_TO)) parts, capped
+// at MAX_PARTS and by the room left in the partial-sum buffer. Split groups come first in the
+// task list (longest work first), the rest follows in Peano-Hilbert order (L1/L2 locality).
+// ------------------------------------------------------------------------------------------
+constexpr unsigned MAX_PARTS = 63;
+
 __global__ void walk_reset_kernel(DevInfo *info) {
-  if (threadIdx.x == 0) { info->group_ticket = 0; info->n_pp = 0; info->n_pc = 0; }
+  if (threadIdx.x == 0) { info->group_ticket = 0; info->task_ticket = 0; info->n_pp = 0; info->n_pc = 0; info->n_tasks = 0; info->sched_cost = 0;
+    unsigned long long now; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(now)); info->t0_ns = now; }
+}
+
+__global__ void __launch_bounds__(256) task_cost_kernel(unsigned n_groups, const DevInfo *__restrict__ info,
+                                                        uint32_t *__restrict__ a_cnt, uint32_t *__restrict__ gdone) {
+  unsigned g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= n_groups) return;
+  const double mean = (double)info->sched_cost / (double)n_groups;
+  const double cost = (double)gdone[g];
+  unsigned s = 0;
+  if (cost > 2.0 * mean && mean > 0.0) {
+    double want = ceil(cost / mean);
+    s = want > (double)MAX_PARTS ? MAX_PARTS : (unsigned)want;
+    if (s < 2) s = 0;
+  }
+  a_cnt[g] = s;
+  gdone[g] = 0;
+}
+
+// after the exclusive scan of a_cnt (in place -> a_off): split groups that do not fit the partial-sum
+// buffer (a suffix of them, offsets are monotone) fall back to one part; writes the class-B counts
+__global__ void __launch_bounds__(256) task_class_kernel(unsigned n_groups, const uint32_t *__restrict__ a_off,
+                                                         const uint32_t *a_total, unsigned part_cap,
+                                                         uint8_t *__restrict__ gparts, uint32_t *__restrict__ b_cnt,
+                                                         DevInfo *info) {
+  unsigned g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= n_groups) return;
+  const unsigned tot = *a_total;
+  const unsigned off = a_off[g];
+  const unsigned nxt = (g + 1 < n_groups) ? a_off[g + 1] : tot;
+  unsigned s = nxt - off;
+  if (s && nxt > part_cap) {
+    if (off <= part_cap) info->n_tasks_a = off;  // the first split group that does not fit
+    s = 0;
+  }
+  gparts[g] = (uint8_t)(s ? s : 1);
+  b_cnt[g] = s ? 0u : 1u;
+  if (g == 0 && tot <= part_cap) info->n_tasks_a = tot;
+}
+
+__global__ void __launch_bounds__(256) task_fill_kernel(unsigned n_groups, const uint32_t *__restrict__ a_off,
+                                                        const uint32_t *__restrict__ b_off, const uint32_t *b_total,
+                                                        const uint8_t *__restrict__ gparts, uint32_t *__restrict__ tasks,
+                                                        DevInfo *info) {
+  unsigned g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= n_groups) return;
+  const unsigned a_end = info->n_tasks_a;
+  const unsigned s = gparts[g];
+  if (s > 1) {
+    const unsigned off = a_off[g];
+    for (unsigned j = 0; j < s; ++j) tasks[off + j] = g | (j << TASK_GROUP_BITS);
+  } else {
+    tasks[a_end + b_off[g]] = g;
+  }
+  if (g == 0) info->n_tasks = a_end + *b_total;
 }
 
 // a11: results back to caller order
@@ -479,11 +649,38 @@ int run_opening(tree_ctx *t, float theta) {
   return 0;
 }
 
+template <int TPL>
+static int launch_walk(tree_ctx *t, const WalkParams &P, unsigned grid) {
+  const unsigned ng = P.n_groups, gb = (ng + 255) / 256;
+  DevInfo *info = t->d_info;
+  uint32_t *tot = info->sched_tot;
+  // 1. exact cost of every group: the walk without the evaluation
+  walk_force_kernel<TPL, true><<<grid, WALK_WARPS * 32, 0, t->stream>>>(P);
+  BH_LAUNCH_CHECK("walk_count");
+  // 2. task list: split expensive groups, longest work first
+  task_cost_kernel<<<gb, 256, 0, t->stream>>>(ng, info, t->b.sched_a, t->b.gdone);
+  BH_LAUNCH_CHECK("task_cost");
+  int rc = device_excl_scan(t, t->b.sched_a, ng, tot);
+  if (rc) return rc;
+  task_class_kernel<<<gb, 256, 0, t->stream>>>(ng, t->b.sched_a, tot, (unsigned)t->part_cap, t->b.gparts, t->b.sched_b, info);
+  BH_LAUNCH_CHECK("task_class");
+  rc = device_excl_scan(t, t->b.sched_b, ng, tot + 1);
+  if (rc) return rc;
+  task_fill_kernel<<<gb, 256, 0, t->stream>>>(ng, t->b.sched_a, t->b.sched_b, tot + 1, t->b.gparts, t->b.tasks, info);
+  BH_LAUNCH_CHECK("task_fill");
+  if (t->ev_valid[EV_SCHED]) cudaEventRecord(t->ev[EV_SCHED], t->stream);
+  // 3. the fused walk + force over the task list
+  walk_force_kernel<TPL, false><<<grid, WALK_WARPS * 32, 0, t->stream>>>(P);
+  BH_LAUNCH_CHECK("walk_force");
+  return 0;
+}
+
 int run_walk(tree_ctx *t, float eps) {
   WalkParams P;
   P.spos = t->b.spos; P.c_test = t->b.c_test; P.c_link = t->b.c_link;
   P.c_cm = t->b.c_cm; P.c_qa = t->b.c_qa; P.c_qb = t->b.c_qb;
   P.gbox = t->b.gbox; P.sacc = t->b.sacc; P.gcount = t->b.gcount; P.info = t->d_info;
+  P.c_count = t->b.c_count; P.trace = t->b.trace; P.tasks = t->b.tasks; P.gparts = t->b.gparts; P.gdone = t->b.gdone; P.part = t->b.part;
   P.N = t->N; P.n_groups = (unsigned)t->n_groups; P.eps2 = eps * eps;
   walk_reset_kernel<<<1, 32, 0, t->stream>>>(t->d_info);
   BH_LAUNCH_CHECK("walk_reset");
@@ -491,13 +688,14 @@ int run_walk(tree_ctx *t, float eps) {
   long long cap = (long long)t->sm_count * 4;
   unsigned grid = (unsigned)(want < cap ? want : cap);
   if (t->ev_valid[EV_OPEN]) cudaEventRecord(t->ev[EV_OPEN], t->stream);
+  int rc;
   switch (t->group) {
-    case 32: walk_force_kernel<1><<<grid, WALK_WARPS * 32, 0, t->stream>>>(P); break;
-    case 64: walk_force_kernel<2><<<grid, WALK_WARPS * 32, 0, t->stream>>>(P); break;
-    case 128: walk_force_kernel<4><<<grid, WALK_WARPS * 32, 0, t->stream>>>(P); break;
+    case 32: rc = launch_walk<1>(t, P, grid); break;
+    case 64: rc = launch_walk<2>(t, P, grid); break;
+    case 128: rc = launch_walk<4>(t, P, grid); break;
     default: return set_err(t, TREE_ERR_ARG, "group size");
   }
-  BH_LAUNCH_CHECK("walk_force");
+  if (rc) return rc;
   if (t->ev_valid[EV_WALK]) cudaEventRecord(t->ev[EV_WALK], t->stream);
   return 0;
 }
