@@ -46,14 +46,17 @@ static int ensure_particles(tree_ctx *t, long long N) {
   BH_TRY(dev_alloc(t, b.gbox, 6 * ng));
   BH_TRY(dev_alloc(t, b.gcount, ng));
   if (ng >= (1ll << 26)) return set_err(t, TREE_ERR_ARG, "too many groups (needs < 2^26)");
-  t->part_cap = ng / 8 + 1024;
+  t->head_cap = ng / 8 + 1024;
+  t->tail_cap = 4ll * 2 * t->sm_count * 16;  // 4 parts x (2 x resident warps) groups
+  const long long part_cap = t->head_cap + t->tail_cap;
   BH_TRY(dev_alloc(t, b.sched_a, ng));
   BH_TRY(dev_alloc(t, b.sched_b, ng));
   BH_TRY(dev_alloc(t, b.gdone, ng));
   BH_TRY(dev_alloc(t, b.gparts, ng));
-  BH_TRY(dev_alloc(t, b.tasks, ng + t->part_cap));
-  BH_TRY(dev_alloc(t, b.part, t->part_cap * t->group));
-  BH_TRY(dev_alloc(t, b.trace, ng + t->part_cap));
+  BH_TRY(dev_alloc(t, b.gthresh, ng));
+  BH_TRY(dev_alloc(t, b.tasks, ng + part_cap));
+  BH_TRY(dev_alloc(t, b.part, part_cap * t->group));
+  BH_TRY(dev_alloc(t, b.trace, ng + part_cap));
   // scan scratch: 256 digits x sort tiles (4096 per tile) or 23 levels x tree tiles (512 per tile)
   long long s1 = 256 * ((cap + 4095) / 4096), s2 = (long long)NLEVELS * ((cap + 511) / 512);
   t->scan_cap = (s1 > s2 ? s1 : s2) + 4096;
@@ -86,7 +89,7 @@ int ensure_cells(tree_ctx *t, long long nc) {
 static void free_all(tree_ctx *t) {
   Buffers &b = t->b;
   void *ptrs[] = {b.posm, b.vel, b.acc, b.key[0], b.key[1], b.idx[0], b.idx[1], b.scan_tmp, b.scan_blk, b.spos, b.sacc,
-                  b.lv, b.gbox, b.gcount, b.sched_a, b.sched_b, b.gdone, b.gparts, b.tasks, b.part, b.trace, b.c_level, b.c_first, b.c_count, b.c_fcall, b.c_link, b.c_cm, b.c_qa, b.c_qb,
+                  b.lv, b.gbox, b.gcount, b.sched_a, b.sched_b, b.gdone, b.gparts, b.gthresh, b.tasks, b.part, b.trace, b.c_level, b.c_first, b.c_count, b.c_fcall, b.c_link, b.c_cm, b.c_qa, b.c_qb,
                   b.c_test, b.in_pos, b.in_mass, b.out_acc, b.out_pot};
   for (void *p : ptrs) if (p) cudaFree(p);
   b = Buffers();

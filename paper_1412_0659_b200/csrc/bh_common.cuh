@@ -28,7 +28,8 @@ struct DevInfo {
   unsigned long long sched_cost;  // sum of the per-group cost estimates of the counting walk
   unsigned int group_ticket;      // dynamic group fetch counter of the counting walk
   unsigned int task_ticket;       // dynamic task fetch counter of the force walk
-  unsigned int n_tasks, n_tasks_a;  // tasks in the list; of which parts of split groups (listed first)
+  unsigned int n_tasks, n_tasks_a;  // tasks in the list; of which parts of expensive groups (listed first)
+  unsigned int tail_start, pad0;    // first task of the tail region (last groups, split into small tasks)
   unsigned int sched_tot[2];      // totals of the two scheduling scans
   double ekin, epot;
 };
@@ -54,6 +55,7 @@ struct Buffers {
   uint32_t *sched_a = nullptr, *sched_b = nullptr;  // [n_groups] part counts -> offsets (scanned in place)
   uint32_t *gdone = nullptr;   // [n_groups]
   uint8_t *gparts = nullptr;   // [n_groups]
+  uint32_t *gthresh = nullptr; // [n_groups]
   uint32_t *tasks = nullptr;   // [n_groups + part_cap]
   float4 *part = nullptr;      // [part_cap][group]
   uint4 *trace = nullptr;      // [n_groups + part_cap] per-task trace of the last force pass
@@ -79,7 +81,7 @@ struct tree_ctx {
   long long n_cells = 0, cell_cap = 0;
   long long n_groups = 0;
   long long scan_cap = 0;
-  long long part_cap = 0;            // tasks that fit the partial-sum buffer
+  long long head_cap = 0, tail_cap = 0;  // partial-sum slots for expensive-group parts / tail parts
   int sorted = 0;                    // which of key[]/idx[] holds the sorted result
   bool built = false, have_vel = false, have_force = false;
   long long staging_cap = 0;         // capacity of the host-call staging buffers

@@ -1,6 +1,8 @@
 // Force-pass kernels (sm_100a): opening radii, the fused tree-walk + force kernel, un-permute,
 // leapfrog and energy.  The walk+force kernel is bound by the FP32 FMA pipe;
 // it is not a dense contraction, so no tensor cores (north_star).
+#include <algorithm>
+
 #include "bh_common.cuh"
 
 namespace bh {
@@ -45,7 +47,9 @@ __global__ void __launch_bounds__(256) opening_kernel(long long n_cells, const D
 // ------------------------------------------------------------------------------------------
 constexpr int WALK_WARPS = 4;
 constexpr unsigned COUNT_TRUNC = 256;  // the counting walk treats cells this small as opened leaves
-constexpr int STACK_CAP = 32 * (MAX_LEVEL + 1);
+constexpr int PREFIX_MAX = 320;  // breadth-first prefix of a split group: deal when the queue reaches this
+constexpr int DEFER_CAP = 320;   // ... or keep at most this many deferred entries
+constexpr int STACK_CAP = 1024;  // >= 32 per level (depth-first) + the dealt share of a breadth-first prefix
 
 struct __align__(16) WarpSmem {
   float4 pc0[32], pc1[32], pc2[32];  // cx,cy,cz,M | Qxx,Qyy,Qzz,T/2 | Qxy,Qxz,Qyz,-3T/2
@@ -70,6 +74,7 @@ struct WalkParams {
   const uint8_t *gparts;   // parts per group (1 = not split)
   uint32_t *gdone;         // finished parts per split group
   float4 *part;            // partial sums of split groups, [task][group size]
+  const uint32_t *gthresh; // split groups: cells with at most this many particles are dealt out, not expanded, in the prefix
   uint4 *trace;            // per task: start ns (lo 32), duration ns, SM id, task word (tracing aid)
   long long N;
   unsigned n_groups;
@@ -78,6 +83,9 @@ struct WalkParams {
 
 constexpr unsigned TASK_GROUP_BITS = 26;
 constexpr unsigned TASK_GROUP_MASK = (1u << TASK_GROUP_BITS) - 1u;
+constexpr unsigned TASK_NONE = 0xffffffffu;  // hole in the task list
+constexpr unsigned PARTS_MASK = 0x7fu;       // gparts: number of parts | PARTS_HEAD for expensive groups
+constexpr unsigned PARTS_HEAD = 0x80u;
 
 template <int TPL>
 struct Targets {
@@ -244,12 +252,49 @@ __device__ __forceinline__ void stage_pc(WarpSmem &ws, int lane, int cnt, const 
 }
 
 // One kernel, two modes.
-//  COUNT = true : walk only; writes the per-group list lengths (n_pp, n_pc) — the exact cost of
-//                 every group, from which the task list is built (see task kernels below).
-//  COUNT = false: work items are TASKS (group g, part j of s): every part of a group repeats the
-//                 (cheap) walk and evaluates only the source tiles k with k mod s == j, so an
-//                 expensive group is spread over s warps; the parts' partial sums are combined
-//                 in fixed order by the part that finishes last (deterministic).
+//  COUNT = true : truncated walk only; writes a cost estimate per group, from which the task list
+//                 is built (task kernels below).
+//  COUNT = false: work items are TASKS (group g, part j of s). An expensive group is cut into s
+//                 parts: all parts repeat a short breadth-first PREFIX of the walk (tiles met
+//                 there are dealt out by tile number mod s), then the frontier is dealt out
+//                 round-robin (entry i goes to part i mod s) and every part walks and evaluates
+//                 its own share depth-first. The parts' partial sums are combined in part order
+//                 by the part that finishes last, so the result does not depend on timing.
+template <int TPL>
+struct WalkState {
+  int pp_entries, pp_pending, pc_pending;
+  unsigned tile_wait, tile_parts;
+};
+
+// Evaluate what is left in the two queues as partial tiles (tile ownership by the counter rule).
+template <int TPL>
+__device__ __forceinline__ void flush_queues(WarpSmem &ws, int lane, WalkState<TPL> &S, Targets<TPL> &T, Totals<TPL> &R,
+                                             const WalkParams &P, uint32_t g0, uint32_t gsize) {
+  if (S.pc_pending > 0) {
+    const bool mine = S.tile_wait == 0;
+    S.tile_wait = mine ? S.tile_parts - 1 : S.tile_wait - 1;
+    if (mine) {
+      stage_pc(ws, lane, S.pc_pending, P);
+      eval_pc_tile<TPL>(ws, S.pc_pending, T, P.eps2);
+      fold_tile<TPL>(T, R);
+      __syncwarp();
+    }
+    S.pc_pending = 0;
+  }
+  if (S.pp_pending > 0) {
+    const bool mine = S.tile_wait == 0;
+    S.tile_wait = mine ? S.tile_parts - 1 : S.tile_wait - 1;
+    const bool own = stage_pp(ws, lane, S.pp_entries, S.pp_pending, mine, P.spos, g0, gsize);
+    if (mine) {
+      eval_pp_tile<TPL>(ws, S.pp_pending, own, T, P.eps2);
+      fold_tile<TPL>(T, R);
+      __syncwarp();
+    }
+    S.pp_pending = 0;
+    S.pp_entries = 0;
+  }
+}
+
 template <int TPL, bool COUNT>
 __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const WalkParams P) {
   __shared__ WarpSmem smem[WALK_WARPS];
@@ -270,9 +315,10 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const Wa
     if (!COUNT) {
       asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_start));
       const unsigned tk = P.tasks[item];
+      if (tk == TASK_NONE) continue;  // hole in the tail region of the task list
       g = tk & TASK_GROUP_MASK;
       part = tk >> TASK_GROUP_BITS;
-      nparts = P.gparts[g];
+      nparts = P.gparts[g] & PARTS_MASK;
     }
 
     const long long g0 = (long long)g * GS;
@@ -298,26 +344,59 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const Wa
     const float *gb = P.gbox + 6ll * g;
     const float bx0 = gb[0], by0 = gb[1], bz0 = gb[2], bx1 = gb[3], by1 = gb[4], bz1 = gb[5];
 
-    int sp = 1;
+    int sp = 1, sb = 0;               // live stack entries are [sb, sp)
     if (lane == 0) ws.stack[0] = 0u;  // root: cell 0, one cell
     __syncwarp();
-    int pp_entries = 0, pp_pending = 0, pc_pending = 0;
+    WalkState<TPL> S;
+    S.pp_entries = 0; S.pp_pending = 0; S.pc_pending = 0;
+    S.tile_wait = part; S.tile_parts = nparts;
     unsigned n_pp = 0, n_pc = 0;
-    unsigned tile_wait = part;  // tiles to skip before the next one this part evaluates
+    bool prefix = !COUNT && nparts > 1;  // breadth-first until the frontier is dealt out
+    int dp = 0;                          // deferred entries, stored downwards from the end of the stack
+    const unsigned small_cell = prefix ? P.gthresh[g] : 0u;
 
-    while (sp > 0) {
-      // ---- pop exactly min(32, cells on stack) cells
-      const bool have = lane < sp;
-      const unsigned e = have ? ws.stack[sp - 1 - lane] : 0u;
+    for (;;) {
+      // ---- split groups: when the breadth-first prefix has no large cell left to open (or runs out
+      //      of room), deal the frontier out: entry i of (queue, then deferred list) -> part i mod s
+      if (prefix && (sp == sb || sp >= PREFIX_MAX)) {
+        flush_queues<TPL>(ws, lane, S, T, R, P, (uint32_t)g0, gsize);
+        int kept = 0;
+        const int live = sp - sb, all = live + dp;
+        for (int base = 0; base < all; base += 32) {
+          const int i = base + lane;
+          const bool have = i < all;
+          const unsigned e = have ? ws.stack[i < live ? sb + i : STACK_CAP - 1 - (i - live)] : 0u;
+          const bool keep = have && ((unsigned)i % nparts) == part;
+          const unsigned m = __ballot_sync(0xffffffffu, keep);
+          __syncwarp();
+          if (keep) ws.stack[kept + __popc(m & lt)] = e;
+          kept += __popc(m);
+          __syncwarp();
+        }
+        sb = 0; sp = kept; dp = 0;
+        prefix = false;
+        S.tile_parts = 1; S.tile_wait = 0;
+        if (part != 0) { n_pp = 0; n_pc = 0; }  // the prefix is counted by part 0 only
+      }
+      if (sp == sb) break;
+      // ---- pop exactly min(32, cells on stack) cells: from the bottom (shallowest first) while in
+      //      the prefix, from the top (deepest first) afterwards
+      const int live = sp - sb;
+      const bool have = lane < live;
+      const int my = prefix ? sb + lane : sp - 1 - lane;
+      const unsigned e = have ? ws.stack[my] : 0u;
       const unsigned n = have ? (e & 7u) + 1u : 0u;
       const unsigned incl = warp_incl_scan_u(n, lane), excl = incl - n;
       const bool take = have && excl < 32u;
       const bool full = incl <= 32u;
       if (take && !full) {
         unsigned k = 32u - excl;
-        ws.stack[sp - 1 - lane] = (((e >> 3) + k) << 3) | (n - k - 1u);
+        ws.stack[my] = (((e >> 3) + k) << 3) | (n - k - 1u);
       }
-      sp -= __popc(__ballot_sync(0xffffffffu, take && full));
+      {
+        const int nfull = __popc(__ballot_sync(0xffffffffu, take && full));
+        if (prefix) sb += nfull; else sp -= nfull;
+      }
       const unsigned tot_all = __shfl_sync(0xffffffffu, incl, 31);
       const unsigned total = tot_all < 32u ? tot_all : 32u;
       const unsigned head = __reduce_or_sync(0xffffffffu, take ? (1u << excl) : 0u);
@@ -346,56 +425,70 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const Wa
         open_leaf = !accept && leaf;
         open_int = !accept && !leaf;
       }
-      // ---- opened internal cells: push child ranges, deeper levels on top
+      // ---- prefix only: an opened cell with few particles is not expanded here; its child range is
+      //      set aside and dealt out later, so that the parts share the fine-grained work
+      if (prefix) {
+        const bool small = open_int && P.c_count[cell] <= small_cell;
+        const unsigned m = __ballot_sync(0xffffffffu, small);
+        if (dp + __popc(m) <= DEFER_CAP) {
+          if (small) {
+            ws.stack[STACK_CAP - 1 - (dp + __popc(m & lt))] = (lk.x << 3) | ((lk.y & 0xfu) - 1u);
+            open_int = false;
+          }
+          dp += __popc(m);
+        }
+      }
+      // ---- opened internal cells: push child ranges so that the stack stays sorted by level
+      //      (prefix: lane order = shallow to deep; afterwards lane 0 holds the deepest cell)
       {
         const unsigned m = __ballot_sync(0xffffffffu, open_int);
-        if (open_int) ws.stack[sp + __popc(m & gt)] = (lk.x << 3) | ((lk.y & 0xfu) - 1u);
+        if (open_int) ws.stack[sp + __popc(m & (prefix ? lt : gt))] = (lk.x << 3) | ((lk.y & 0xfu) - 1u);
         sp += __popc(m);
       }
       // ---- accepted cells -> p-c queue
       {
         const unsigned m = __ballot_sync(0xffffffffu, accept);
-        if (!COUNT) { if (accept) ws.pcq[pc_pending + __popc(m & lt)] = cell; }
+        if (!COUNT) { if (accept) ws.pcq[S.pc_pending + __popc(m & lt)] = cell; }
         const int c = __popc(m);
-        pc_pending += c;
+        S.pc_pending += c;
         n_pc += c;
       }
       // ---- opened leaves -> p-p range queue
       {
         const unsigned m = __ballot_sync(0xffffffffu, open_leaf);
-        if (!COUNT) { if (open_leaf) ws.ppq[pp_entries + __popc(m & lt)] = lk; }
-        pp_entries += __popc(m);
+        if (!COUNT) { if (open_leaf) ws.ppq[S.pp_entries + __popc(m & lt)] = lk; }
+        S.pp_entries += __popc(m);
         const unsigned c = __reduce_add_sync(0xffffffffu, open_leaf ? lk.y : 0u);
-        pp_pending += (int)c;
+        S.pp_pending += (int)c;
         n_pp += c;
       }
       __syncwarp();
-      if (COUNT) { pc_pending = 0; pp_pending = 0; pp_entries = 0; continue; }
+      if (COUNT) { S.pc_pending = 0; S.pp_pending = 0; S.pp_entries = 0; continue; }
       // ---- evaluate full tiles (only those that belong to this part)
-      if (pc_pending >= 32) {
-        const bool mine = tile_wait == 0;
-        tile_wait = mine ? nparts - 1 : tile_wait - 1;
+      if (S.pc_pending >= 32) {
+        const bool mine = S.tile_wait == 0;
+        S.tile_wait = mine ? S.tile_parts - 1 : S.tile_wait - 1;
         if (mine) {
           stage_pc(ws, lane, 32, P);
           eval_pc_tile<TPL>(ws, 32, T, P.eps2);
           fold_tile<TPL>(T, R);
           __syncwarp();
         }
-        const unsigned mv = (lane + 32 < pc_pending) ? ws.pcq[lane + 32] : 0u;
+        const unsigned mv = (lane + 32 < S.pc_pending) ? ws.pcq[lane + 32] : 0u;
         __syncwarp();
         ws.pcq[lane] = mv;
-        pc_pending -= 32;
+        S.pc_pending -= 32;
         __syncwarp();
       }
-      while (pp_pending >= 32) {
-        const bool mine = tile_wait == 0;
-        tile_wait = mine ? nparts - 1 : tile_wait - 1;
-        const bool own = stage_pp(ws, lane, pp_entries, 32, mine, P.spos, (uint32_t)g0, gsize);
+      while (S.pp_pending >= 32) {
+        const bool mine = S.tile_wait == 0;
+        S.tile_wait = mine ? S.tile_parts - 1 : S.tile_wait - 1;
+        const bool own = stage_pp(ws, lane, S.pp_entries, 32, mine, P.spos, (uint32_t)g0, gsize);
         if (mine) {
           eval_pp_tile<TPL>(ws, 32, own, T, P.eps2);
           fold_tile<TPL>(T, R);
         }
-        pp_pending -= 32;
+        S.pp_pending -= 32;
         __syncwarp();
       }
     }
@@ -407,32 +500,17 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const Wa
       }
       continue;
     }
-    if (part == 0 && lane == 0) {
-      P.gcount[g] = make_uint2(n_pp, n_pc);
+    flush_queues<TPL>(ws, lane, S, T, R, P, (uint32_t)g0, gsize);
+    if (prefix && part != 0) { n_pp = 0; n_pc = 0; }  // walk ended inside the prefix: counted by part 0
+    if (lane == 0) {
+      if (nparts == 1) {
+        P.gcount[g] = make_uint2(n_pp, n_pc);
+      } else {  // gcount of split groups is zeroed by task_class_kernel
+        atomicAdd(&P.gcount[g].x, n_pp);
+        atomicAdd(&P.gcount[g].y, n_pc);
+      }
       atomicAdd(&P.info->n_pp, (unsigned long long)n_pp * gsize);
       atomicAdd(&P.info->n_pc, (unsigned long long)n_pc * gsize);
-    }
-    // ---- flush partial tiles
-    if (pc_pending > 0) {
-      const bool mine = tile_wait == 0;
-      tile_wait = mine ? nparts - 1 : tile_wait - 1;
-      if (mine) {
-        stage_pc(ws, lane, pc_pending, P);
-        eval_pc_tile<TPL>(ws, pc_pending, T, P.eps2);
-        fold_tile<TPL>(T, R);
-        __syncwarp();
-      }
-    }
-    if (pp_pending > 0) {
-      const bool mine = tile_wait == 0;
-      if (mine) {
-        const bool own = stage_pp(ws, lane, pp_entries, pp_pending, true, P.spos, (uint32_t)g0, gsize);
-        eval_pp_tile<TPL>(ws, pp_pending, own, T, P.eps2);
-        fold_tile<TPL>(T, R);
-        __syncwarp();
-      }
-    }
-    if (lane == 0) {
       unsigned long long t_end;
       unsigned smid;
       asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_end));
@@ -452,8 +530,11 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const Wa
         if (j < gsize) P.sacc[g0 + j] = res[t];
       }
     } else {
-      // split group: tasks of one group are consecutive and all lie in the partial-sum buffer
-      float4 *mine = P.part + (size_t)item * GS;
+      // split group: its parts are consecutive tasks, in the head (expensive groups) or the tail
+      // region of the task list; both regions map onto the partial-sum buffer
+      const unsigned na = P.info->n_tasks_a;
+      const size_t slot = item < na ? item : na + (item - P.info->tail_start);
+      float4 *mine = P.part + slot * GS;
 #pragma unroll
       for (int t = 0; t < TPL; ++t) __stcg(&mine[lane + 32u * t], res[t]);
       __threadfence();
@@ -462,7 +543,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const Wa
       prev = __shfl_sync(0xffffffffu, prev, 0);
       if (prev == nparts - 1) {  // last part to finish: combine in fixed order 0..s-1
         __threadfence();
-        const float4 *base = P.part + (size_t)(item - part) * GS;
+        const float4 *base = P.part + (slot - part) * GS;
 #pragma unroll
         for (int t = 0; t < TPL; ++t) {
           float hi[4] = {0.f, 0.f, 0.f, 0.f}, lo[4] = {0.f, 0.f, 0.f, 0.f};
@@ -482,21 +563,28 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const Wa
 }
 
 // ------------------------------------------------------------------------------------------
-// Task list (scheduling only; results do not depend on it beyond the fixed-order partial sums).
-// cost(g) = 13 n_pp + 37 n_pc (FP32 instructions per target of the two evaluators). A group
-// costing more than SPLIT_AT x mean is cut into s = ceil(cost / (mean x SPLIT_TO)) parts, capped
-// at MAX_PARTS and by the room left in the partial-sum buffer. Split groups come first in the
-// task list (longest work first), the rest follows in Peano-Hilbert order (L1/L2 locality).
+// Task list (scheduling only; results depend on it only through the fixed-order partial sums).
+// cost(g) = 13 n_pp + 37 n_pc, estimated by the truncated counting walk. Task list layout:
+//   head : parts of EXPENSIVE groups (cost > 2 x mean: s = ceil(cost / mean) parts), longest first
+//   body : one task per ordinary group, in Peano-Hilbert order (L1/L2 locality between warps)
+//   tail : the last n_tail groups, TAIL_PARTS parts each, so that the kernel ends on small tasks
 // ------------------------------------------------------------------------------------------
 constexpr unsigned MAX_PARTS = 63;
+constexpr unsigned TAIL_PARTS = 4;
 
 __global__ void walk_reset_kernel(DevInfo *info) {
-  if (threadIdx.x == 0) { info->group_ticket = 0; info->task_ticket = 0; info->n_pp = 0; info->n_pc = 0; info->n_tasks = 0; info->sched_cost = 0;
-    unsigned long long now; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(now)); info->t0_ns = now; }
+  if (threadIdx.x == 0) {
+    info->group_ticket = 0; info->task_ticket = 0; info->n_pp = 0; info->n_pc = 0; info->n_tasks = 0;
+    info->sched_cost = 0;
+    unsigned long long now;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(now));
+    info->t0_ns = now;
+  }
 }
 
 __global__ void __launch_bounds__(256) task_cost_kernel(unsigned n_groups, const DevInfo *__restrict__ info,
-                                                        uint32_t *__restrict__ a_cnt, uint32_t *__restrict__ gdone) {
+                                                        uint32_t *__restrict__ a_cnt, uint32_t *__restrict__ gdone,
+                                                        uint32_t *__restrict__ gthresh) {
   unsigned g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= n_groups) return;
   const double mean = (double)info->sched_cost / (double)n_groups;
@@ -509,13 +597,18 @@ __global__ void __launch_bounds__(256) task_cost_kernel(unsigned n_groups, const
   }
   a_cnt[g] = s;
   gdone[g] = 0;
+  // about 16 dealt entries per part: particles opened ~ cost / 13 (an over-estimate)
+  const double per_entry = cost / 13.0 / (16.0 * (s ? s : TAIL_PARTS));
+  gthresh[g] = per_entry < 32.0 ? 32u : (per_entry > 1e9 ? 1000000000u : (unsigned)per_entry);
 }
 
-// after the exclusive scan of a_cnt (in place -> a_off): split groups that do not fit the partial-sum
-// buffer (a suffix of them, offsets are monotone) fall back to one part; writes the class-B counts
-__global__ void __launch_bounds__(256) task_class_kernel(unsigned n_groups, const uint32_t *__restrict__ a_off,
-                                                         const uint32_t *a_total, unsigned part_cap,
-                                                         uint8_t *__restrict__ gparts, uint32_t *__restrict__ b_cnt,
+// after the exclusive scan of a_cnt (in place -> a_off): expensive groups that do not fit the
+// partial-sum buffer (a suffix of them, offsets are monotone) fall back to one part; classifies
+// every group (head / body / tail) and writes the body counts
+__global__ void __launch_bounds__(256) task_class_kernel(unsigned n_groups, unsigned n_tail,
+                                                         const uint32_t *__restrict__ a_off, const uint32_t *a_total,
+                                                         unsigned head_cap, uint8_t *__restrict__ gparts,
+                                                         uint32_t *__restrict__ b_cnt, uint2 *__restrict__ gcount,
                                                          DevInfo *info) {
   unsigned g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= n_groups) return;
@@ -523,30 +616,40 @@ __global__ void __launch_bounds__(256) task_class_kernel(unsigned n_groups, cons
   const unsigned off = a_off[g];
   const unsigned nxt = (g + 1 < n_groups) ? a_off[g + 1] : tot;
   unsigned s = nxt - off;
-  if (s && nxt > part_cap) {
-    if (off <= part_cap) info->n_tasks_a = off;  // the first split group that does not fit
+  if (s && nxt > head_cap) {
+    if (off <= head_cap) info->n_tasks_a = off;  // the first expensive group that does not fit
     s = 0;
   }
-  gparts[g] = (uint8_t)(s ? s : 1);
-  b_cnt[g] = s ? 0u : 1u;
-  if (g == 0 && tot <= part_cap) info->n_tasks_a = tot;
+  const bool tail = g >= n_groups - n_tail;
+  gparts[g] = (uint8_t)(s ? (s | PARTS_HEAD) : (tail ? TAIL_PARTS : 1u));
+  b_cnt[g] = (s || tail) ? 0u : 1u;
+  gcount[g] = make_uint2(0u, 0u);
+  if (g == 0 && tot <= head_cap) info->n_tasks_a = tot;
 }
 
-__global__ void __launch_bounds__(256) task_fill_kernel(unsigned n_groups, const uint32_t *__restrict__ a_off,
+__global__ void __launch_bounds__(256) task_fill_kernel(unsigned n_groups, unsigned n_tail,
+                                                        const uint32_t *__restrict__ a_off,
                                                         const uint32_t *__restrict__ b_off, const uint32_t *b_total,
                                                         const uint8_t *__restrict__ gparts, uint32_t *__restrict__ tasks,
                                                         DevInfo *info) {
   unsigned g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= n_groups) return;
   const unsigned a_end = info->n_tasks_a;
-  const unsigned s = gparts[g];
-  if (s > 1) {
+  const unsigned tail_start = a_end + *b_total;
+  const unsigned gp = gparts[g], s = gp & PARTS_MASK;
+  const bool head = gp & PARTS_HEAD;
+  const bool tail = g >= n_groups - n_tail;
+  if (head) {
     const unsigned off = a_off[g];
     for (unsigned j = 0; j < s; ++j) tasks[off + j] = g | (j << TASK_GROUP_BITS);
-  } else {
+  } else if (!tail) {
     tasks[a_end + b_off[g]] = g;
   }
-  if (g == 0) info->n_tasks = a_end + *b_total;
+  if (tail) {  // fixed slots; an expensive group inside the tail range leaves a hole here
+    const unsigned base = tail_start + (g - (n_groups - n_tail)) * TAIL_PARTS;
+    for (unsigned j = 0; j < TAIL_PARTS; ++j) tasks[base + j] = head ? TASK_NONE : (g | (j << TASK_GROUP_BITS));
+  }
+  if (g == 0) { info->n_tasks = tail_start + n_tail * TAIL_PARTS; info->tail_start = tail_start; }
 }
 
 // a11: results back to caller order
@@ -658,15 +761,18 @@ static int launch_walk(tree_ctx *t, const WalkParams &P, unsigned grid) {
   walk_force_kernel<TPL, true><<<grid, WALK_WARPS * 32, 0, t->stream>>>(P);
   BH_LAUNCH_CHECK("walk_count");
   // 2. task list: split expensive groups, longest work first
-  task_cost_kernel<<<gb, 256, 0, t->stream>>>(ng, info, t->b.sched_a, t->b.gdone);
+  task_cost_kernel<<<gb, 256, 0, t->stream>>>(ng, info, t->b.sched_a, t->b.gdone, t->b.gthresh);
   BH_LAUNCH_CHECK("task_cost");
   int rc = device_excl_scan(t, t->b.sched_a, ng, tot);
   if (rc) return rc;
-  task_class_kernel<<<gb, 256, 0, t->stream>>>(ng, t->b.sched_a, tot, (unsigned)t->part_cap, t->b.gparts, t->b.sched_b, info);
+  const unsigned n_tail = (unsigned)std::min<long long>(ng / 4, t->tail_cap / (long long)TAIL_PARTS);
+  task_class_kernel<<<gb, 256, 0, t->stream>>>(ng, n_tail, t->b.sched_a, tot, (unsigned)t->head_cap, t->b.gparts,
+                                               t->b.sched_b, t->b.gcount, info);
   BH_LAUNCH_CHECK("task_class");
   rc = device_excl_scan(t, t->b.sched_b, ng, tot + 1);
   if (rc) return rc;
-  task_fill_kernel<<<gb, 256, 0, t->stream>>>(ng, t->b.sched_a, t->b.sched_b, tot + 1, t->b.gparts, t->b.tasks, info);
+  task_fill_kernel<<<gb, 256, 0, t->stream>>>(ng, n_tail, t->b.sched_a, t->b.sched_b, tot + 1, t->b.gparts, t->b.tasks,
+                                              info);
   BH_LAUNCH_CHECK("task_fill");
   if (t->ev_valid[EV_SCHED]) cudaEventRecord(t->ev[EV_SCHED], t->stream);
   // 3. the fused walk + force over the task list
@@ -680,7 +786,7 @@ int run_walk(tree_ctx *t, float eps) {
   P.spos = t->b.spos; P.c_test = t->b.c_test; P.c_link = t->b.c_link;
   P.c_cm = t->b.c_cm; P.c_qa = t->b.c_qa; P.c_qb = t->b.c_qb;
   P.gbox = t->b.gbox; P.sacc = t->b.sacc; P.gcount = t->b.gcount; P.info = t->d_info;
-  P.c_count = t->b.c_count; P.trace = t->b.trace; P.tasks = t->b.tasks; P.gparts = t->b.gparts; P.gdone = t->b.gdone; P.part = t->b.part;
+  P.c_count = t->b.c_count; P.trace = t->b.trace; P.gthresh = t->b.gthresh; P.tasks = t->b.tasks; P.gparts = t->b.gparts; P.gdone = t->b.gdone; P.part = t->b.part;
   P.N = t->N; P.n_groups = (unsigned)t->n_groups; P.eps2 = eps * eps;
   walk_reset_kernel<<<1, 32, 0, t->stream>>>(t->d_info);
   BH_LAUNCH_CHECK("walk_reset");
