@@ -47,12 +47,13 @@ __global__ void __launch_bounds__(256) opening_kernel(long long n_cells, const D
 // ------------------------------------------------------------------------------------------
 constexpr int WALK_WARPS = 4;
 constexpr unsigned COUNT_TRUNC = 256;  // the counting walk treats cells this small as opened leaves
+constexpr int FOLD_EVERY = 4;    // tiles (of 32 sources) summed in plain FP32 between compensated folds
 constexpr int PREFIX_MAX = 320;  // breadth-first prefix of a split group: deal when the queue reaches this
 constexpr int DEFER_CAP = 320;   // ... or keep at most this many deferred entries
 constexpr int STACK_CAP = 1024;  // >= 32 per level (depth-first) + the dealt share of a breadth-first prefix
 
 struct __align__(16) WarpSmem {
-  float4 pc0[32], pc1[32], pc2[32];  // cx,cy,cz,M | Qxx,Qyy,Qzz,T/2 | Qxy,Qxz,Qyz,-3T/2
+  float4 pc0[32], pc1[32], pc2[32];  // cx,cy,cz,M | 2.5 Q'xx,Q'yy,Q'zz, 2.5 tr(Q) eps^2 | 2.5 Q'xy,Q'xz,Q'yz (pc_one)
   float4 pp[32];                     // x,y,z,m
   uint32_t ppidx[32];                // slot of each staged p-p source (self-skip by index, S2)
   uint2 ppq[64];                     // pending particle ranges (first, count)
@@ -90,7 +91,8 @@ constexpr unsigned PARTS_HEAD = 0x80u;
 template <int TPL>
 struct Targets {
   float x[TPL], y[TPL], z[TPL];
-  float ax[TPL], ay[TPL], az[TPL], ph[TPL];  // sums over the tile being evaluated
+  float ax[TPL], ay[TPL], az[TPL], ph[TPL];  // sums over the tiles evaluated since the last fold
+  float phq[TPL];                            // quadrupole part of the potential, scaled (see pc_one)
   uint32_t slot[TPL];
 };
 
@@ -116,8 +118,8 @@ __device__ __forceinline__ void fold_tile(Targets<TPL> &T, Totals<TPL> &R) {
     two_sum_fold(R.hi[0][t], R.lo[0][t], T.ax[t]);
     two_sum_fold(R.hi[1][t], R.lo[1][t], T.ay[t]);
     two_sum_fold(R.hi[2][t], R.lo[2][t], T.az[t]);
-    two_sum_fold(R.hi[3][t], R.lo[3][t], T.ph[t]);
-    T.ax[t] = T.ay[t] = T.az[t] = T.ph[t] = 0.0f;
+    two_sum_fold(R.hi[3][t], R.lo[3][t], fmaf(-0.2f, T.phq[t], T.ph[t]));
+    T.ax[t] = T.ay[t] = T.az[t] = T.ph[t] = T.phq[t] = 0.0f;
   }
 }
 
@@ -152,6 +154,11 @@ __device__ __forceinline__ void pp_one(const float4 s, uint32_t sidx, Targets<TP
   }
 }
 
+// Particle-cell interaction, Eqs. (1),(2) with s^2 = |r|^2 + eps^2 in every power (S1),
+// rearranged exactly: with Q' = 3Q - tr(Q) I and w = r^T Q' r - tr(Q) eps^2,
+//   phi = -M rho - 1/2 w rho^5,   a = (M rho^3 + 5/2 w rho^7) r - rho^5 Q' r.
+// Staged per source: a = (cx,cy,cz,M), b = 2.5 (Q'xx,Q'yy,Q'zz, tr(Q) eps^2), c = 2.5 (Q'xy,Q'xz,Q'yz).
+// 33 FP32 instructions + 1 MUFU per target (the paper counts 65 flop for this interaction).
 template <int TPL>
 __device__ __forceinline__ void pc_one(const float4 a, const float4 b, const float4 c, Targets<TPL> &T, float eps2) {
 #pragma unroll
@@ -161,23 +168,18 @@ __device__ __forceinline__ void pc_one(const float4 a, const float4 b, const flo
     r2 = fmaf(dy, dy, r2);
     r2 = fmaf(dz, dz, r2);
     float ri = rsqrt_fast(r2);
-    float ri2 = ri * ri;
-    float vx = fmaf(c.y, dz, fmaf(c.x, dy, b.x * dx));
+    float vx = fmaf(c.y, dz, fmaf(c.x, dy, b.x * dx));   // 2.5 Q' r
     float vy = fmaf(c.z, dz, fmaf(b.y, dy, c.x * dx));
     float vz = fmaf(b.z, dz, fmaf(c.z, dy, c.y * dx));
-    float q = fmaf(dz, vz, fmaf(dy, vy, dx * vx));
+    float w = fmaf(dz, vz, fmaf(dy, vy, fmaf(dx, vx, -b.w)));  // 2.5 w
+    float ri2 = ri * ri;
     float ri3 = ri * ri2;
+    float ri4 = ri2 * ri2;
     float ri5 = ri3 * ri2;
-    float u = q * ri5;
-    float mr = a.w * ri;
-    float p = fmaf(b.w, ri3, -mr);   // -M rho + T/2 rho^3
-    p = fmaf(-1.5f, u, p);           // - 3/2 q rho^5
-    T.ph[t] += p;
-    float g = a.w * ri3;             // M rho^3
-    g = fmaf(c.w, ri5, g);           // - 3/2 T rho^5
-    float w7 = u * ri2;              // q rho^7
-    g = fmaf(7.5f, w7, g);
-    float k = -3.0f * ri5;
+    T.ph[t] = fmaf(-a.w, ri, T.ph[t]);       // -M rho
+    T.phq[t] = fmaf(w, ri5, T.phq[t]);       // 2.5 w rho^5; folded in as -0.2 x
+    float g = fmaf(w, ri4, a.w) * ri3;       // M rho^3 + 2.5 w rho^7
+    float k = -0.4f * ri5;                   // - rho^5 Q' r = k (2.5 Q' r)
     T.ax[t] = fmaf(k, vx, fmaf(g, dx, T.ax[t]));
     T.ay[t] = fmaf(k, vy, fmaf(g, dy, T.ay[t]));
     T.az[t] = fmaf(k, vz, fmaf(g, dz, T.az[t]));
@@ -244,9 +246,11 @@ __device__ __forceinline__ void stage_pc(WarpSmem &ws, int lane, int cnt, const 
   if (lane < cnt) {
     const unsigned c = ws.pcq[lane];
     const float4 a = P.c_cm[c], qa = P.c_qa[c], qb = P.c_qb[c];
+    const float tr = qb.w;
     ws.pc0[lane] = a;
-    ws.pc1[lane] = make_float4(qa.x, qa.y, qa.z, 0.5f * qb.w);
-    ws.pc2[lane] = make_float4(qb.x, qb.y, qb.z, -1.5f * qb.w);
+    ws.pc1[lane] = make_float4(2.5f * fmaf(3.0f, qa.x, -tr), 2.5f * fmaf(3.0f, qa.y, -tr), 2.5f * fmaf(3.0f, qa.z, -tr),
+                               2.5f * tr * P.eps2);
+    ws.pc2[lane] = make_float4(7.5f * qb.x, 7.5f * qb.y, 7.5f * qb.z, 0.0f);
   }
   __syncwarp();
 }
@@ -264,6 +268,7 @@ template <int TPL>
 struct WalkState {
   int pp_entries, pp_pending, pc_pending;
   unsigned tile_wait, tile_parts;
+  int unfolded;  // tiles accumulated in T since the last fold into the running totals
 };
 
 // Evaluate what is left in the two queues as partial tiles (tile ownership by the counter rule).
@@ -276,7 +281,7 @@ __device__ __forceinline__ void flush_queues(WarpSmem &ws, int lane, WalkState<T
     if (mine) {
       stage_pc(ws, lane, S.pc_pending, P);
       eval_pc_tile<TPL>(ws, S.pc_pending, T, P.eps2);
-      fold_tile<TPL>(T, R);
+      if (++S.unfolded >= FOLD_EVERY) { fold_tile<TPL>(T, R); S.unfolded = 0; }
       __syncwarp();
     }
     S.pc_pending = 0;
@@ -287,7 +292,7 @@ __device__ __forceinline__ void flush_queues(WarpSmem &ws, int lane, WalkState<T
     const bool own = stage_pp(ws, lane, S.pp_entries, S.pp_pending, mine, P.spos, g0, gsize);
     if (mine) {
       eval_pp_tile<TPL>(ws, S.pp_pending, own, T, P.eps2);
-      fold_tile<TPL>(T, R);
+      if (++S.unfolded >= FOLD_EVERY) { fold_tile<TPL>(T, R); S.unfolded = 0; }
       __syncwarp();
     }
     S.pp_pending = 0;
@@ -338,7 +343,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const Wa
       float4 p = make_float4(0.f, 0.f, 0.f, 0.f);
       if (!COUNT) p = P.spos[g0 + (j < gsize ? j : gsize - 1)];  // padded lanes copy a real target
       T.x[t] = p.x; T.y[t] = p.y; T.z[t] = p.z;
-      T.ax[t] = T.ay[t] = T.az[t] = T.ph[t] = 0.0f;
+      T.ax[t] = T.ay[t] = T.az[t] = T.ph[t] = T.phq[t] = 0.0f;
       if (j >= gsize) T.slot[t] = 0xffffffffu;
     }
     const float *gb = P.gbox + 6ll * g;
@@ -349,7 +354,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const Wa
     __syncwarp();
     WalkState<TPL> S;
     S.pp_entries = 0; S.pp_pending = 0; S.pc_pending = 0;
-    S.tile_wait = part; S.tile_parts = nparts;
+    S.tile_wait = part; S.tile_parts = nparts; S.unfolded = 0;
     unsigned n_pp = 0, n_pc = 0;
     bool prefix = !COUNT && nparts > 1;  // breadth-first until the frontier is dealt out
     int dp = 0;                          // deferred entries, stored downwards from the end of the stack
@@ -471,7 +476,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const Wa
         if (mine) {
           stage_pc(ws, lane, 32, P);
           eval_pc_tile<TPL>(ws, 32, T, P.eps2);
-          fold_tile<TPL>(T, R);
+          if (++S.unfolded >= FOLD_EVERY) { fold_tile<TPL>(T, R); S.unfolded = 0; }
           __syncwarp();
         }
         const unsigned mv = (lane + 32 < S.pc_pending) ? ws.pcq[lane + 32] : 0u;
@@ -486,7 +491,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const Wa
         const bool own = stage_pp(ws, lane, S.pp_entries, 32, mine, P.spos, (uint32_t)g0, gsize);
         if (mine) {
           eval_pp_tile<TPL>(ws, 32, own, T, P.eps2);
-          fold_tile<TPL>(T, R);
+          if (++S.unfolded >= FOLD_EVERY) { fold_tile<TPL>(T, R); S.unfolded = 0; }
         }
         S.pp_pending -= 32;
         __syncwarp();
@@ -501,6 +506,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const Wa
       continue;
     }
     flush_queues<TPL>(ws, lane, S, T, R, P, (uint32_t)g0, gsize);
+    fold_tile<TPL>(T, R);
     if (prefix && part != 0) { n_pp = 0; n_pc = 0; }  // walk ended inside the prefix: counted by part 0
     if (lane == 0) {
       if (nparts == 1) {
