@@ -45,7 +45,19 @@ __global__ void __launch_bounds__(256) opening_kernel(long long n_cells, const D
 // Evaluate: whenever a queue holds >= 32 sources, 32 of them are staged in shared memory as float4
 // and every lane evaluates them against its TPL targets with broadcast LDS.128 loads.
 // ------------------------------------------------------------------------------------------
+#ifndef BH_WALK_MINB
+#define BH_WALK_MINB 5
+#endif
+#ifndef BH_PP_UNROLL
+#define BH_PP_UNROLL 8
+#endif
+#ifndef BH_PC_UNROLL
+#define BH_PC_UNROLL 8
+#endif
+constexpr int PP_UNROLL = BH_PP_UNROLL, PC_UNROLL = BH_PC_UNROLL;  // sources per unrolled evaluator loop body
 constexpr int WALK_WARPS = 4;
+constexpr int WALK_MINB = BH_WALK_MINB;  // resident blocks per SM the register budget is sized for
+constexpr int COUNT_MINB = 8;            // same for the counting pre-pass (38 registers; shared memory allows 8 blocks)
 constexpr unsigned COUNT_TRUNC = 256;  // the counting walk treats cells this small as opened leaves
 constexpr int FOLD_EVERY = 4;    // tiles (of 32 sources) summed in plain FP32 between compensated folds
 constexpr int PREFIX_MAX = 320;  // breadth-first prefix of a split group: deal when the queue reaches this
@@ -189,7 +201,7 @@ __device__ __forceinline__ void pc_one(const float4 a, const float4 b, const flo
 template <int TPL>
 __device__ __forceinline__ void eval_pp_tile(const WarpSmem &ws, int cnt, bool mask, Targets<TPL> &T, float eps2) {
   if (!mask && cnt == 32) {
-#pragma unroll 8
+#pragma unroll(PP_UNROLL)
     for (int j = 0; j < 32; ++j) pp_one<TPL, false>(ws.pp[j], 0u, T, eps2);
   } else if (!mask) {
     for (int j = 0; j < cnt; ++j) pp_one<TPL, false>(ws.pp[j], 0u, T, eps2);
@@ -202,7 +214,7 @@ __device__ __forceinline__ void eval_pp_tile(const WarpSmem &ws, int cnt, bool m
 template <int TPL>
 __device__ __forceinline__ void eval_pc_tile(const WarpSmem &ws, int cnt, Targets<TPL> &T, float eps2) {
   if (cnt == 32) {
-#pragma unroll 4
+#pragma unroll(PC_UNROLL)
     for (int j = 0; j < 32; ++j) pc_one<TPL>(ws.pc0[j], ws.pc1[j], ws.pc2[j], T, eps2);
   } else {
     for (int j = 0; j < cnt; ++j) pc_one<TPL>(ws.pc0[j], ws.pc1[j], ws.pc2[j], T, eps2);
@@ -301,7 +313,7 @@ __device__ __forceinline__ void flush_queues(WarpSmem &ws, int lane, WalkState<T
 }
 
 template <int TPL, bool COUNT>
-__global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_force_kernel(const WalkParams P) {
+__global__ void __launch_bounds__(WALK_WARPS * 32, COUNT ? COUNT_MINB : WALK_MINB) walk_force_kernel(const WalkParams P) {
   __shared__ WarpSmem smem[WALK_WARPS];
   WarpSmem &ws = smem[threadIdx.x >> 5];
   const int lane = threadIdx.x & 31;
@@ -764,7 +776,8 @@ static int launch_walk(tree_ctx *t, const WalkParams &P, unsigned grid) {
   DevInfo *info = t->d_info;
   uint32_t *tot = info->sched_tot;
   // 1. exact cost of every group: the walk without the evaluation
-  walk_force_kernel<TPL, true><<<grid, WALK_WARPS * 32, 0, t->stream>>>(P);
+  const long long cwant = (ng + WALK_WARPS - 1) / WALK_WARPS, ccap = (long long)t->sm_count * COUNT_MINB;
+  walk_force_kernel<TPL, true><<<(unsigned)(cwant < ccap ? cwant : ccap), WALK_WARPS * 32, 0, t->stream>>>(P);
   BH_LAUNCH_CHECK("walk_count");
   // 2. task list: split expensive groups, longest work first
   task_cost_kernel<<<gb, 256, 0, t->stream>>>(ng, info, t->b.sched_a, t->b.gdone, t->b.gthresh);
@@ -797,7 +810,7 @@ int run_walk(tree_ctx *t, float eps) {
   walk_reset_kernel<<<1, 32, 0, t->stream>>>(t->d_info);
   BH_LAUNCH_CHECK("walk_reset");
   long long want = (t->n_groups + WALK_WARPS - 1) / WALK_WARPS;
-  long long cap = (long long)t->sm_count * 4;
+  long long cap = (long long)t->sm_count * WALK_MINB;
   unsigned grid = (unsigned)(want < cap ? want : cap);
   if (t->ev_valid[EV_OPEN]) cudaEventRecord(t->ev[EV_OPEN], t->stream);
   int rc;
