@@ -99,6 +99,20 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def _ncu_traffic(workload: str):
+    """DRAM bytes per launch of the walk kernel from the committed ncu --set full capture (or None)."""
+    import csv
+    path = os.path.join(ROOT, "profiles", "walk_dram_traffic.csv")
+    try:
+        with open(path) as fh:
+            for row in csv.DictReader(fh):
+                if row["workload"] == workload:
+                    return int(row["dram_bytes_read"]) + int(row["dram_bytes_write"]), row["source"]
+    except (OSError, KeyError, ValueError):
+        pass
+    return None, None
+
+
 def _cpu_oracle_sample(cfg, pos, mass, budget_s: float = 15.0):
     """Time the oracle's tree force (as it stands) on a bounded sample of groups of this workload."""
     import numpy as np
@@ -272,8 +286,10 @@ def run_ours(args):
         peak = _peak_tflops(props.multi_processor_count, 1965.0)
         flops = effective_flops(pp_tot, pc_tot)
         ach = flops / (phase_ms["walk"] * 1e-3) / 1e12
+        traffic, traffic_src = _ncu_traffic(cfg["name"])
         roof = {"bound": "alu", "kernel": "walk_force_kernel", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
-                "frac": ach / peak, "traffic": None,
+                "frac": ach / peak, "traffic": traffic, "traffic_unit": "bytes of DRAM read+write per launch",
+                "traffic_source": traffic_src,
                 "peak_source": f"derived: {props.multi_processor_count} SMs x 128 FP32 lanes x 2 x 1.965 GHz "
                                "(MEASURED_PEAKS.json has no FP32 figure)",
                 "flops_convention": "23 per p-p, 65 per p-c (PAPER.md L190-192)",

@@ -216,7 +216,10 @@ int tree_leapfrog(tree_ctx *t, float dt) {
   rec(t, EV_B0);
   BH_TRY(run_bbox_only(t));
   BH_TRY(build_from_posm(t));
-  BH_TRY(force_impl(t, t->theta, t->eps, nullptr, nullptr));
+  t->reuse_costs = true;  // same particles one step later: last pass's counts predict this pass's costs
+  const int frc = force_impl(t, t->theta, t->eps, nullptr, nullptr);
+  t->reuse_costs = false;
+  if (frc) return frc;
   rec(t, EV_I2);
   BH_TRY(run_kick(t, dt));
   rec(t, EV_I3);

@@ -86,6 +86,7 @@ struct tree_ctx {
   bool built = false, have_vel = false, have_force = false;
   long long staging_cap = 0;         // capacity of the host-call staging buffers
   float theta = 0.f, eps = 0.f;
+  bool reuse_costs = false;          // this force pass may schedule by the previous pass's per-group counts
   int sm_count = 148;
   bh::Buffers b;
   bh::DevInfo *d_info = nullptr;

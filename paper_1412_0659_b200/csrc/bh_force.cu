@@ -60,9 +60,8 @@ constexpr int WALK_MINB = BH_WALK_MINB;  // resident blocks per SM the register 
 constexpr int COUNT_MINB = 8;            // same for the counting pre-pass (38 registers; shared memory allows 8 blocks)
 constexpr unsigned COUNT_TRUNC = 256;  // the counting walk treats cells this small as opened leaves
 constexpr int FOLD_EVERY = 4;    // tiles (of 32 sources) summed in plain FP32 between compensated folds
-constexpr int PREFIX_MAX = 320;  // breadth-first prefix of a split group: deal when the queue reaches this
-constexpr int DEFER_CAP = 320;   // ... or keep at most this many deferred entries
-constexpr int STACK_CAP = 1024;  // >= 32 per level (depth-first) + the dealt share of a breadth-first prefix
+constexpr int DEFER_CAP = 256;   // deferred child ranges one part of a split group may own
+constexpr int STACK_CAP = 1024;  // >= 32 per level (depth-first: 32 x 22) + DEFER_CAP
 
 struct __align__(16) WarpSmem {
   float4 pc0[32], pc1[32], pc2[32];  // cx,cy,cz,M | 2.5 Q'xx,Q'yy,Q'zz, 2.5 tr(Q) eps^2 | 2.5 Q'xy,Q'xz,Q'yz (pc_one)
@@ -312,14 +311,254 @@ __device__ __forceinline__ void flush_queues(WarpSmem &ws, int lane, WalkState<T
   }
 }
 
+// One work item: group g (part `part` of `nparts`).
+template <int TPL, bool COUNT>
+__device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, const int lane, const unsigned item,
+                                          const unsigned g, const unsigned part, const unsigned nparts,
+                                          const unsigned long long t_start) {
+  const unsigned lt = (1u << lane) - 1u;
+  const unsigned gt = ~((lt << 1) | 1u);
+  constexpr unsigned GS = 32u * TPL;
+  const bool SPLIT = !COUNT && nparts > 1;
+  const long long g0 = (long long)g * GS;
+  const long long rem = P.N - g0;
+  const unsigned gsize = rem < (long long)GS ? (unsigned)rem : GS;
+  Targets<TPL> T;
+  Totals<TPL> R;
+#pragma unroll
+  for (int t = 0; t < TPL; ++t) {
+#pragma unroll
+    for (int c = 0; c < 4; ++c) { R.hi[c][t] = 0.0f; R.lo[c][t] = 0.0f; }
+  }
+#pragma unroll
+  for (int t = 0; t < TPL; ++t) {
+    unsigned j = lane + 32u * t;
+    T.slot[t] = (uint32_t)(g0 + j);
+    float4 p = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (!COUNT) p = P.spos[g0 + (j < gsize ? j : gsize - 1)];  // padded lanes copy a real target
+    T.x[t] = p.x; T.y[t] = p.y; T.z[t] = p.z;
+    T.ax[t] = T.ay[t] = T.az[t] = T.ph[t] = T.phq[t] = 0.0f;
+    if (j >= gsize) T.slot[t] = 0xffffffffu;
+  }
+  const float *gb = P.gbox + 6ll * g;
+  const float bx0 = gb[0], by0 = gb[1], bz0 = gb[2], bx1 = gb[3], by1 = gb[4], bz1 = gb[5];
+
+  int sp = 1;                       // live stack entries are [0, sp)
+  if (lane == 0) ws.stack[0] = 0u;  // root: cell 0, one cell
+  __syncwarp();
+  WalkState<TPL> S;
+  S.pp_entries = 0; S.pp_pending = 0; S.pc_pending = 0;
+  S.tile_wait = part; S.tile_parts = nparts; S.unfolded = 0;
+  unsigned n_pp = 0, n_pc = 0;
+  bool prefix = SPLIT;  // all parts walk the large-cell skeleton identically
+  int dp = 0;                          // this part's deferred entries, stored downwards from the end of the stack
+  unsigned dcount = 0;                 // deferred entries seen so far by every part (entry i belongs to part i mod s)
+  const unsigned small_cell = SPLIT ? P.gthresh[g] : 0u;
+
+  for (;;) {
+    // ---- stack empty: evaluate what is left in the queues (the only call site of the partial-tile
+    //      evaluators). A part of a split group has then finished the skeleton all parts walk alike and
+    //      continues with its own share of the deferred child ranges, evaluating every tile itself.
+    if (sp == 0) {
+      if (!COUNT) flush_queues<TPL>(ws, lane, S, T, R, P, (uint32_t)g0, gsize);
+      if (!(SPLIT && prefix)) break;
+      for (int base = 0; base < dp; base += 32) {
+        const int i = base + lane;
+        const unsigned e = i < dp ? ws.stack[STACK_CAP - 1 - i] : 0u;
+        __syncwarp();
+        if (i < dp) ws.stack[i] = e;
+      }
+      __syncwarp();
+      sp = dp; dp = 0;
+      prefix = false;
+      S.tile_parts = 1; S.tile_wait = 0;
+      if (part != 0) { n_pp = 0; n_pc = 0; }  // the prefix is counted by part 0 only
+      if (sp == 0) break;
+    }
+    // ---- pop exactly min(32, cells on stack) cells from the top (deepest first)
+    const int live = sp;
+    const bool have = lane < live;
+    const int my = sp - 1 - lane;
+    const unsigned e = have ? ws.stack[my] : 0u;
+    const unsigned n = have ? (e & 7u) + 1u : 0u;
+    const unsigned incl = warp_incl_scan_u(n, lane), excl = incl - n;
+    const bool take = have && excl < 32u;
+    const bool full = incl <= 32u;
+    if (take && !full) {
+      unsigned k = 32u - excl;
+      ws.stack[my] = (((e >> 3) + k) << 3) | (n - k - 1u);
+    }
+    sp -= __popc(__ballot_sync(0xffffffffu, take && full));
+    const unsigned tot_all = __shfl_sync(0xffffffffu, incl, 31);
+    const unsigned total = tot_all < 32u ? tot_all : 32u;
+    const unsigned head = __reduce_or_sync(0xffffffffu, take ? (1u << excl) : 0u);
+    const int ei = __popc(head & (0xffffffffu >> (31 - lane))) - 1;
+    const unsigned fx = __shfl_sync(0xffffffffu, e >> 3, ei & 31);
+    const unsigned ex = __shfl_sync(0xffffffffu, excl, ei & 31);
+    const bool valid = (unsigned)lane < total;
+    const unsigned cell = fx + ((unsigned)lane - ex);
+
+    // ---- multipole acceptance test (T10), exact op sequence
+    bool accept = false, open_leaf = false, open_int = false;
+    uint2 lk = make_uint2(0u, 0u);
+    if (valid) {
+      const float4 tr = P.c_test[cell];
+      lk = P.c_link[cell];
+      float ux = fmaxf(0.0f, fmaxf(__fsub_rn(bx0, tr.x), __fsub_rn(tr.x, bx1)));
+      float uy = fmaxf(0.0f, fmaxf(__fsub_rn(by0, tr.y), __fsub_rn(tr.y, by1)));
+      float uz = fmaxf(0.0f, fmaxf(__fsub_rn(bz0, tr.z), __fsub_rn(tr.z, bz1)));
+      float d2 = __fmaf_rn(uz, uz, __fmaf_rn(uy, uy, __fmul_rn(ux, ux)));
+      accept = d2 > tr.w;
+      bool leaf = !(lk.y & LEAF_FLAG);
+      if (COUNT && !leaf && !accept) {  // cost estimate: do not descend below small cells
+        const unsigned cc = P.c_count[cell];
+        if (cc <= COUNT_TRUNC) { leaf = true; lk.y = cc; }
+      }
+      open_leaf = !accept && leaf;
+      open_int = !accept && !leaf;
+    }
+    // ---- prefix only: an opened cell with few particles is not expanded here; its child range is
+    //      entry number dcount of the group's deferred list and belongs to part (dcount mod s)
+    if (SPLIT && prefix) {
+      const bool small = open_int && P.c_count[cell] <= small_cell;
+      const unsigned m = __ballot_sync(0xffffffffu, small);
+      if (dcount + __popc(m) <= (unsigned)DEFER_CAP * nparts) {  // the same decision in every part
+        const bool mine = small && ((dcount + __popc(m & lt)) % nparts) == part;
+        const unsigned mm = __ballot_sync(0xffffffffu, mine);
+        if (mine) ws.stack[STACK_CAP - 1 - (dp + __popc(mm & lt))] = (lk.x << 3) | ((lk.y & 0xfu) - 1u);
+        if (small) open_int = false;
+        dp += __popc(mm);
+        dcount += __popc(m);
+      }
+    }
+    // ---- opened internal cells: push child ranges so that the stack stays sorted by level
+    //      (prefix: lane order = shallow to deep; afterwards lane 0 holds the deepest cell)
+    {
+      const unsigned m = __ballot_sync(0xffffffffu, open_int);
+      if (open_int) ws.stack[sp + __popc(m & gt)] = (lk.x << 3) | ((lk.y & 0xfu) - 1u);
+      sp += __popc(m);
+    }
+    // ---- accepted cells -> p-c queue
+    {
+      const unsigned m = __ballot_sync(0xffffffffu, accept);
+      if (!COUNT) { if (accept) ws.pcq[S.pc_pending + __popc(m & lt)] = cell; }
+      const int c = __popc(m);
+      S.pc_pending += c;
+      n_pc += c;
+    }
+    // ---- opened leaves -> p-p range queue
+    {
+      const unsigned m = __ballot_sync(0xffffffffu, open_leaf);
+      if (!COUNT) { if (open_leaf) ws.ppq[S.pp_entries + __popc(m & lt)] = lk; }
+      S.pp_entries += __popc(m);
+      const unsigned c = __reduce_add_sync(0xffffffffu, open_leaf ? lk.y : 0u);
+      S.pp_pending += (int)c;
+      n_pp += c;
+    }
+    __syncwarp();
+    if (COUNT) { S.pc_pending = 0; S.pp_pending = 0; S.pp_entries = 0; continue; }
+    // ---- evaluate full tiles (only those that belong to this part)
+    if (S.pc_pending >= 32) {
+      const bool mine = S.tile_wait == 0;
+      S.tile_wait = mine ? S.tile_parts - 1 : S.tile_wait - 1;
+      if (mine) {
+        stage_pc(ws, lane, 32, P);
+        eval_pc_tile<TPL>(ws, 32, T, P.eps2);
+        if (++S.unfolded >= FOLD_EVERY) { fold_tile<TPL>(T, R); S.unfolded = 0; }
+        __syncwarp();
+      }
+      const unsigned mv = (lane + 32 < S.pc_pending) ? ws.pcq[lane + 32] : 0u;
+      __syncwarp();
+      ws.pcq[lane] = mv;
+      S.pc_pending -= 32;
+      __syncwarp();
+    }
+    while (S.pp_pending >= 32) {
+      const bool mine = S.tile_wait == 0;
+      S.tile_wait = mine ? S.tile_parts - 1 : S.tile_wait - 1;
+      const bool own = stage_pp(ws, lane, S.pp_entries, 32, mine, P.spos, (uint32_t)g0, gsize);
+      if (mine) {
+        eval_pp_tile<TPL>(ws, 32, own, T, P.eps2);
+        if (++S.unfolded >= FOLD_EVERY) { fold_tile<TPL>(T, R); S.unfolded = 0; }
+      }
+      S.pp_pending -= 32;
+      __syncwarp();
+    }
+  }
+  if (COUNT) {
+    if (lane == 0) {
+      const unsigned long long c = 13ull * n_pp + 37ull * n_pc;
+      P.gdone[g] = c > 0xffffffffull ? 0xffffffffu : (unsigned)c;  // read and cleared by task_cost_kernel
+      atomicAdd(&P.info->sched_cost, c);
+    }
+    return;
+  }
+  fold_tile<TPL>(T, R);
+  if (prefix && part != 0) { n_pp = 0; n_pc = 0; }  // walk ended inside the prefix: counted by part 0
+  if (lane == 0) {
+    if (nparts == 1) {
+      P.gcount[g] = make_uint2(n_pp, n_pc);
+    } else {  // gcount of split groups is zeroed by task_class_kernel
+      atomicAdd(&P.gcount[g].x, n_pp);
+      atomicAdd(&P.gcount[g].y, n_pc);
+    }
+    atomicAdd(&P.info->n_pp, (unsigned long long)n_pp * gsize);
+    atomicAdd(&P.info->n_pc, (unsigned long long)n_pc * gsize);
+    unsigned long long t_end;
+    unsigned smid;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_end));
+    asm volatile("mov.u32 %0, %smid;" : "=r"(smid));
+    P.trace[item] = make_uint4((unsigned)(t_start - P.info->t0_ns), (unsigned)(t_end - t_start), smid, P.tasks[item]);
+  }
+  // ---- results
+  float4 res[TPL];
+#pragma unroll
+  for (int t = 0; t < TPL; ++t)
+    res[t] = make_float4(__fadd_rn(R.hi[0][t], R.lo[0][t]), __fadd_rn(R.hi[1][t], R.lo[1][t]),
+                         __fadd_rn(R.hi[2][t], R.lo[2][t]), __fadd_rn(R.hi[3][t], R.lo[3][t]));
+  if (nparts == 1) {
+#pragma unroll
+    for (int t = 0; t < TPL; ++t) {
+      unsigned j = lane + 32u * t;
+      if (j < gsize) P.sacc[g0 + j] = res[t];
+    }
+  } else {
+    // split group: its parts are consecutive tasks, in the head (expensive groups) or the tail
+    // region of the task list; both regions map onto the partial-sum buffer
+    const unsigned na = P.info->n_tasks_a;
+    const size_t slot = item < na ? item : na + (item - P.info->tail_start);
+    float4 *mine = P.part + slot * GS;
+#pragma unroll
+    for (int t = 0; t < TPL; ++t) __stcg(&mine[lane + 32u * t], res[t]);
+    __threadfence();
+    unsigned prev = 0;
+    if (lane == 0) prev = atomicAdd(&P.gdone[g], 1u);
+    prev = __shfl_sync(0xffffffffu, prev, 0);
+    if (prev == nparts - 1) {  // last part to finish: combine in fixed order 0..s-1
+      __threadfence();
+      const float4 *base = P.part + (slot - part) * GS;
+#pragma unroll
+      for (int t = 0; t < TPL; ++t) {
+        float hi[4] = {0.f, 0.f, 0.f, 0.f}, lo[4] = {0.f, 0.f, 0.f, 0.f};
+        for (unsigned q = 0; q < nparts; ++q) {
+          const float4 v = __ldcg(&base[(size_t)q * GS + lane + 32u * t]);
+          two_sum_fold(hi[0], lo[0], v.x); two_sum_fold(hi[1], lo[1], v.y);
+          two_sum_fold(hi[2], lo[2], v.z); two_sum_fold(hi[3], lo[3], v.w);
+        }
+        unsigned j = lane + 32u * t;
+        if (j < gsize)
+          P.sacc[g0 + j] = make_float4(__fadd_rn(hi[0], lo[0]), __fadd_rn(hi[1], lo[1]), __fadd_rn(hi[2], lo[2]),
+                                       __fadd_rn(hi[3], lo[3]));
+      }
+    }
+  }
+}
+
 template <int TPL, bool COUNT>
 __global__ void __launch_bounds__(WALK_WARPS * 32, COUNT ? COUNT_MINB : WALK_MINB) walk_force_kernel(const WalkParams P) {
   __shared__ WarpSmem smem[WALK_WARPS];
   WarpSmem &ws = smem[threadIdx.x >> 5];
   const int lane = threadIdx.x & 31;
-  const unsigned lt = (1u << lane) - 1u;
-  const unsigned gt = ~((lt << 1) | 1u);
-  constexpr unsigned GS = 32u * TPL;
   const unsigned n_items = COUNT ? P.n_groups : P.info->n_tasks;
 
   for (;;) {
@@ -327,256 +566,17 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, COUNT ? COUNT_MINB : WALK_MIN
     if (lane == 0) item = atomicAdd(COUNT ? &P.info->group_ticket : &P.info->task_ticket, 1u);
     item = __shfl_sync(0xffffffffu, item, 0);
     if (item >= n_items) break;
-    unsigned g = item, part = 0, nparts = 1;
-    unsigned long long t_start = 0;
-    if (!COUNT) {
-      asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_start));
-      const unsigned tk = P.tasks[item];
-      if (tk == TASK_NONE) continue;  // hole in the tail region of the task list
-      g = tk & TASK_GROUP_MASK;
-      part = tk >> TASK_GROUP_BITS;
-      nparts = P.gparts[g] & PARTS_MASK;
-    }
-
-    const long long g0 = (long long)g * GS;
-    const long long rem = P.N - g0;
-    const unsigned gsize = rem < (long long)GS ? (unsigned)rem : GS;
-    Targets<TPL> T;
-    Totals<TPL> R;
-#pragma unroll
-    for (int t = 0; t < TPL; ++t) {
-#pragma unroll
-      for (int c = 0; c < 4; ++c) { R.hi[c][t] = 0.0f; R.lo[c][t] = 0.0f; }
-    }
-#pragma unroll
-    for (int t = 0; t < TPL; ++t) {
-      unsigned j = lane + 32u * t;
-      T.slot[t] = (uint32_t)(g0 + j);
-      float4 p = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (!COUNT) p = P.spos[g0 + (j < gsize ? j : gsize - 1)];  // padded lanes copy a real target
-      T.x[t] = p.x; T.y[t] = p.y; T.z[t] = p.z;
-      T.ax[t] = T.ay[t] = T.az[t] = T.ph[t] = T.phq[t] = 0.0f;
-      if (j >= gsize) T.slot[t] = 0xffffffffu;
-    }
-    const float *gb = P.gbox + 6ll * g;
-    const float bx0 = gb[0], by0 = gb[1], bz0 = gb[2], bx1 = gb[3], by1 = gb[4], bz1 = gb[5];
-
-    int sp = 1, sb = 0;               // live stack entries are [sb, sp)
-    if (lane == 0) ws.stack[0] = 0u;  // root: cell 0, one cell
-    __syncwarp();
-    WalkState<TPL> S;
-    S.pp_entries = 0; S.pp_pending = 0; S.pc_pending = 0;
-    S.tile_wait = part; S.tile_parts = nparts; S.unfolded = 0;
-    unsigned n_pp = 0, n_pc = 0;
-    bool prefix = !COUNT && nparts > 1;  // breadth-first until the frontier is dealt out
-    int dp = 0;                          // deferred entries, stored downwards from the end of the stack
-    const unsigned small_cell = prefix ? P.gthresh[g] : 0u;
-
-    for (;;) {
-      // ---- split groups: when the breadth-first prefix has no large cell left to open (or runs out
-      //      of room), deal the frontier out: entry i of (queue, then deferred list) -> part i mod s
-      if (prefix && (sp == sb || sp >= PREFIX_MAX)) {
-        flush_queues<TPL>(ws, lane, S, T, R, P, (uint32_t)g0, gsize);
-        int kept = 0;
-        const int live = sp - sb, all = live + dp;
-        for (int base = 0; base < all; base += 32) {
-          const int i = base + lane;
-          const bool have = i < all;
-          const unsigned e = have ? ws.stack[i < live ? sb + i : STACK_CAP - 1 - (i - live)] : 0u;
-          const bool keep = have && ((unsigned)i % nparts) == part;
-          const unsigned m = __ballot_sync(0xffffffffu, keep);
-          __syncwarp();
-          if (keep) ws.stack[kept + __popc(m & lt)] = e;
-          kept += __popc(m);
-          __syncwarp();
-        }
-        sb = 0; sp = kept; dp = 0;
-        prefix = false;
-        S.tile_parts = 1; S.tile_wait = 0;
-        if (part != 0) { n_pp = 0; n_pc = 0; }  // the prefix is counted by part 0 only
-      }
-      if (sp == sb) break;
-      // ---- pop exactly min(32, cells on stack) cells: from the bottom (shallowest first) while in
-      //      the prefix, from the top (deepest first) afterwards
-      const int live = sp - sb;
-      const bool have = lane < live;
-      const int my = prefix ? sb + lane : sp - 1 - lane;
-      const unsigned e = have ? ws.stack[my] : 0u;
-      const unsigned n = have ? (e & 7u) + 1u : 0u;
-      const unsigned incl = warp_incl_scan_u(n, lane), excl = incl - n;
-      const bool take = have && excl < 32u;
-      const bool full = incl <= 32u;
-      if (take && !full) {
-        unsigned k = 32u - excl;
-        ws.stack[my] = (((e >> 3) + k) << 3) | (n - k - 1u);
-      }
-      {
-        const int nfull = __popc(__ballot_sync(0xffffffffu, take && full));
-        if (prefix) sb += nfull; else sp -= nfull;
-      }
-      const unsigned tot_all = __shfl_sync(0xffffffffu, incl, 31);
-      const unsigned total = tot_all < 32u ? tot_all : 32u;
-      const unsigned head = __reduce_or_sync(0xffffffffu, take ? (1u << excl) : 0u);
-      const int ei = __popc(head & (0xffffffffu >> (31 - lane))) - 1;
-      const unsigned fx = __shfl_sync(0xffffffffu, e >> 3, ei & 31);
-      const unsigned ex = __shfl_sync(0xffffffffu, excl, ei & 31);
-      const bool valid = (unsigned)lane < total;
-      const unsigned cell = fx + ((unsigned)lane - ex);
-
-      // ---- multipole acceptance test (T10), exact op sequence
-      bool accept = false, open_leaf = false, open_int = false;
-      uint2 lk = make_uint2(0u, 0u);
-      if (valid) {
-        const float4 tr = P.c_test[cell];
-        lk = P.c_link[cell];
-        float ux = fmaxf(0.0f, fmaxf(__fsub_rn(bx0, tr.x), __fsub_rn(tr.x, bx1)));
-        float uy = fmaxf(0.0f, fmaxf(__fsub_rn(by0, tr.y), __fsub_rn(tr.y, by1)));
-        float uz = fmaxf(0.0f, fmaxf(__fsub_rn(bz0, tr.z), __fsub_rn(tr.z, bz1)));
-        float d2 = __fmaf_rn(uz, uz, __fmaf_rn(uy, uy, __fmul_rn(ux, ux)));
-        accept = d2 > tr.w;
-        bool leaf = !(lk.y & LEAF_FLAG);
-        if (COUNT && !leaf && !accept) {  // cost estimate: do not descend below small cells
-          const unsigned cc = P.c_count[cell];
-          if (cc <= COUNT_TRUNC) { leaf = true; lk.y = cc; }
-        }
-        open_leaf = !accept && leaf;
-        open_int = !accept && !leaf;
-      }
-      // ---- prefix only: an opened cell with few particles is not expanded here; its child range is
-      //      set aside and dealt out later, so that the parts share the fine-grained work
-      if (prefix) {
-        const bool small = open_int && P.c_count[cell] <= small_cell;
-        const unsigned m = __ballot_sync(0xffffffffu, small);
-        if (dp + __popc(m) <= DEFER_CAP) {
-          if (small) {
-            ws.stack[STACK_CAP - 1 - (dp + __popc(m & lt))] = (lk.x << 3) | ((lk.y & 0xfu) - 1u);
-            open_int = false;
-          }
-          dp += __popc(m);
-        }
-      }
-      // ---- opened internal cells: push child ranges so that the stack stays sorted by level
-      //      (prefix: lane order = shallow to deep; afterwards lane 0 holds the deepest cell)
-      {
-        const unsigned m = __ballot_sync(0xffffffffu, open_int);
-        if (open_int) ws.stack[sp + __popc(m & (prefix ? lt : gt))] = (lk.x << 3) | ((lk.y & 0xfu) - 1u);
-        sp += __popc(m);
-      }
-      // ---- accepted cells -> p-c queue
-      {
-        const unsigned m = __ballot_sync(0xffffffffu, accept);
-        if (!COUNT) { if (accept) ws.pcq[S.pc_pending + __popc(m & lt)] = cell; }
-        const int c = __popc(m);
-        S.pc_pending += c;
-        n_pc += c;
-      }
-      // ---- opened leaves -> p-p range queue
-      {
-        const unsigned m = __ballot_sync(0xffffffffu, open_leaf);
-        if (!COUNT) { if (open_leaf) ws.ppq[S.pp_entries + __popc(m & lt)] = lk; }
-        S.pp_entries += __popc(m);
-        const unsigned c = __reduce_add_sync(0xffffffffu, open_leaf ? lk.y : 0u);
-        S.pp_pending += (int)c;
-        n_pp += c;
-      }
-      __syncwarp();
-      if (COUNT) { S.pc_pending = 0; S.pp_pending = 0; S.pp_entries = 0; continue; }
-      // ---- evaluate full tiles (only those that belong to this part)
-      if (S.pc_pending >= 32) {
-        const bool mine = S.tile_wait == 0;
-        S.tile_wait = mine ? S.tile_parts - 1 : S.tile_wait - 1;
-        if (mine) {
-          stage_pc(ws, lane, 32, P);
-          eval_pc_tile<TPL>(ws, 32, T, P.eps2);
-          if (++S.unfolded >= FOLD_EVERY) { fold_tile<TPL>(T, R); S.unfolded = 0; }
-          __syncwarp();
-        }
-        const unsigned mv = (lane + 32 < S.pc_pending) ? ws.pcq[lane + 32] : 0u;
-        __syncwarp();
-        ws.pcq[lane] = mv;
-        S.pc_pending -= 32;
-        __syncwarp();
-      }
-      while (S.pp_pending >= 32) {
-        const bool mine = S.tile_wait == 0;
-        S.tile_wait = mine ? S.tile_parts - 1 : S.tile_wait - 1;
-        const bool own = stage_pp(ws, lane, S.pp_entries, 32, mine, P.spos, (uint32_t)g0, gsize);
-        if (mine) {
-          eval_pp_tile<TPL>(ws, 32, own, T, P.eps2);
-          if (++S.unfolded >= FOLD_EVERY) { fold_tile<TPL>(T, R); S.unfolded = 0; }
-        }
-        S.pp_pending -= 32;
-        __syncwarp();
-      }
-    }
     if (COUNT) {
-      if (lane == 0) {
-        const unsigned long long c = 13ull * n_pp + 37ull * n_pc;
-        P.gdone[g] = c > 0xffffffffull ? 0xffffffffu : (unsigned)c;  // read and cleared by task_cost_kernel
-        atomicAdd(&P.info->sched_cost, c);
-      }
+      walk_task<TPL, true>(P, ws, lane, item, item, 0u, 1u, 0ull);
       continue;
     }
-    flush_queues<TPL>(ws, lane, S, T, R, P, (uint32_t)g0, gsize);
-    fold_tile<TPL>(T, R);
-    if (prefix && part != 0) { n_pp = 0; n_pc = 0; }  // walk ended inside the prefix: counted by part 0
-    if (lane == 0) {
-      if (nparts == 1) {
-        P.gcount[g] = make_uint2(n_pp, n_pc);
-      } else {  // gcount of split groups is zeroed by task_class_kernel
-        atomicAdd(&P.gcount[g].x, n_pp);
-        atomicAdd(&P.gcount[g].y, n_pc);
-      }
-      atomicAdd(&P.info->n_pp, (unsigned long long)n_pp * gsize);
-      atomicAdd(&P.info->n_pc, (unsigned long long)n_pc * gsize);
-      unsigned long long t_end;
-      unsigned smid;
-      asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_end));
-      asm volatile("mov.u32 %0, %smid;" : "=r"(smid));
-      P.trace[item] = make_uint4((unsigned)(t_start - P.info->t0_ns), (unsigned)(t_end - t_start), smid, P.tasks[item]);
-    }
-    // ---- results
-    float4 res[TPL];
-#pragma unroll
-    for (int t = 0; t < TPL; ++t)
-      res[t] = make_float4(__fadd_rn(R.hi[0][t], R.lo[0][t]), __fadd_rn(R.hi[1][t], R.lo[1][t]),
-                           __fadd_rn(R.hi[2][t], R.lo[2][t]), __fadd_rn(R.hi[3][t], R.lo[3][t]));
-    if (nparts == 1) {
-#pragma unroll
-      for (int t = 0; t < TPL; ++t) {
-        unsigned j = lane + 32u * t;
-        if (j < gsize) P.sacc[g0 + j] = res[t];
-      }
-    } else {
-      // split group: its parts are consecutive tasks, in the head (expensive groups) or the tail
-      // region of the task list; both regions map onto the partial-sum buffer
-      const unsigned na = P.info->n_tasks_a;
-      const size_t slot = item < na ? item : na + (item - P.info->tail_start);
-      float4 *mine = P.part + slot * GS;
-#pragma unroll
-      for (int t = 0; t < TPL; ++t) __stcg(&mine[lane + 32u * t], res[t]);
-      __threadfence();
-      unsigned prev = 0;
-      if (lane == 0) prev = atomicAdd(&P.gdone[g], 1u);
-      prev = __shfl_sync(0xffffffffu, prev, 0);
-      if (prev == nparts - 1) {  // last part to finish: combine in fixed order 0..s-1
-        __threadfence();
-        const float4 *base = P.part + (slot - part) * GS;
-#pragma unroll
-        for (int t = 0; t < TPL; ++t) {
-          float hi[4] = {0.f, 0.f, 0.f, 0.f}, lo[4] = {0.f, 0.f, 0.f, 0.f};
-          for (unsigned q = 0; q < nparts; ++q) {
-            const float4 v = __ldcg(&base[(size_t)q * GS + lane + 32u * t]);
-            two_sum_fold(hi[0], lo[0], v.x); two_sum_fold(hi[1], lo[1], v.y);
-            two_sum_fold(hi[2], lo[2], v.z); two_sum_fold(hi[3], lo[3], v.w);
-          }
-          unsigned j = lane + 32u * t;
-          if (j < gsize)
-            P.sacc[g0 + j] = make_float4(__fadd_rn(hi[0], lo[0]), __fadd_rn(hi[1], lo[1]), __fadd_rn(hi[2], lo[2]),
-                                         __fadd_rn(hi[3], lo[3]));
-        }
-      }
-    }
+    unsigned long long t_start;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_start));
+    const unsigned tk = P.tasks[item];
+    if (tk == TASK_NONE) continue;  // hole in the tail region of the task list
+    const unsigned g = tk & TASK_GROUP_MASK, part = tk >> TASK_GROUP_BITS;
+    const unsigned nparts = P.gparts[g] & PARTS_MASK;
+    walk_task<TPL, false>(P, ws, lane, item, g, part, nparts, t_start);
   }
 }
 
@@ -587,29 +587,56 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, COUNT ? COUNT_MINB : WALK_MIN
 //   body : one task per ordinary group, in Peano-Hilbert order (L1/L2 locality between warps)
 //   tail : the last n_tail groups, TAIL_PARTS parts each, so that the kernel ends on small tasks
 // ------------------------------------------------------------------------------------------
+#ifndef BH_SPLIT_FINE
+#define BH_SPLIT_FINE 1.0
+#endif
+#ifndef BH_SPLIT_AT
+#define BH_SPLIT_AT 2.0
+#endif
+constexpr double SPLIT_FINE = BH_SPLIT_FINE;  // parts per mean-cost unit of an expensive group
+constexpr double SPLIT_AT = BH_SPLIT_AT;      // a group is expensive above this multiple of the mean cost
 constexpr unsigned MAX_PARTS = 63;
+#ifndef BH_TAIL_PER_SM
+#define BH_TAIL_PER_SM 16
+#endif
 constexpr unsigned TAIL_PARTS = 4;
+constexpr long long TAIL_PER_SM = BH_TAIL_PER_SM;  // groups per SM at the end of the list that are cut into TAIL_PARTS
 
-__global__ void walk_reset_kernel(DevInfo *info) {
+__global__ void walk_reset_kernel(DevInfo *info, unsigned reuse_gs) {
   if (threadIdx.x == 0) {
+    // reuse_gs != 0: the per-group costs of the previous force pass stand in for the counting walk
+    // (tree_leapfrog: consecutive steps); their sum follows from the interaction totals
+    const unsigned long long prev = reuse_gs ? (13ull * info->n_pp + 37ull * info->n_pc) / reuse_gs : 0ull;
     info->group_ticket = 0; info->task_ticket = 0; info->n_pp = 0; info->n_pc = 0; info->n_tasks = 0;
-    info->sched_cost = 0;
+    info->sched_cost = prev;
     unsigned long long now;
     asm volatile("mov.u64 %0, %globaltimer;" : "=l"(now));
     info->t0_ns = now;
   }
 }
 
+__device__ __forceinline__ double prev_cost(const uint2 *__restrict__ gcount, unsigned g) {
+  const uint2 c = gcount[g];
+  return 13.0 * (double)c.x + 37.0 * (double)c.y;
+}
+
 __global__ void __launch_bounds__(256) task_cost_kernel(unsigned n_groups, const DevInfo *__restrict__ info,
                                                         uint32_t *__restrict__ a_cnt, uint32_t *__restrict__ gdone,
-                                                        uint32_t *__restrict__ gthresh) {
+                                                        uint32_t *__restrict__ gthresh, const uint2 *__restrict__ prev) {
   unsigned g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= n_groups) return;
   const double mean = (double)info->sched_cost / (double)n_groups;
-  const double cost = (double)gdone[g];
+  double cost;
+  if (prev) {  // exact counts of the previous pass; the neighbours cover a shift of the runs by up to two
+    cost = 0.0;
+    const unsigned a = g >= 2 ? g - 2 : 0u, b = g + 2 < n_groups ? g + 2 : n_groups - 1;
+    for (unsigned q = a; q <= b; ++q) cost = fmax(cost, prev_cost(prev, q));
+  } else {
+    cost = (double)gdone[g];
+  }
   unsigned s = 0;
-  if (cost > 2.0 * mean && mean > 0.0) {
-    double want = ceil(cost / mean);
+  if (cost > SPLIT_AT * mean && mean > 0.0) {
+    double want = ceil(SPLIT_FINE * cost / mean);
     s = want > (double)MAX_PARTS ? MAX_PARTS : (unsigned)want;
     if (s < 2) s = 0;
   }
@@ -775,16 +802,20 @@ static int launch_walk(tree_ctx *t, const WalkParams &P, unsigned grid) {
   const unsigned ng = P.n_groups, gb = (ng + 255) / 256;
   DevInfo *info = t->d_info;
   uint32_t *tot = info->sched_tot;
-  // 1. exact cost of every group: the walk without the evaluation
+  // 1. cost of every group: the walk without the evaluation, or the previous pass's exact counts
+  const bool reuse = t->reuse_costs;
+  if (!reuse) {
   const long long cwant = (ng + WALK_WARPS - 1) / WALK_WARPS, ccap = (long long)t->sm_count * COUNT_MINB;
   walk_force_kernel<TPL, true><<<(unsigned)(cwant < ccap ? cwant : ccap), WALK_WARPS * 32, 0, t->stream>>>(P);
   BH_LAUNCH_CHECK("walk_count");
+  }
   // 2. task list: split expensive groups, longest work first
-  task_cost_kernel<<<gb, 256, 0, t->stream>>>(ng, info, t->b.sched_a, t->b.gdone, t->b.gthresh);
+  task_cost_kernel<<<gb, 256, 0, t->stream>>>(ng, info, t->b.sched_a, t->b.gdone, t->b.gthresh,
+                                              reuse ? t->b.gcount : nullptr);
   BH_LAUNCH_CHECK("task_cost");
   int rc = device_excl_scan(t, t->b.sched_a, ng, tot);
   if (rc) return rc;
-  const unsigned n_tail = (unsigned)std::min<long long>(ng / 4, t->tail_cap / (long long)TAIL_PARTS);
+  const unsigned n_tail = (unsigned)std::min<long long>(std::min<long long>(ng / 4, TAIL_PER_SM * t->sm_count), t->tail_cap / (long long)TAIL_PARTS);
   task_class_kernel<<<gb, 256, 0, t->stream>>>(ng, n_tail, t->b.sched_a, tot, (unsigned)t->head_cap, t->b.gparts,
                                                t->b.sched_b, t->b.gcount, info);
   BH_LAUNCH_CHECK("task_class");
@@ -807,7 +838,7 @@ int run_walk(tree_ctx *t, float eps) {
   P.gbox = t->b.gbox; P.sacc = t->b.sacc; P.gcount = t->b.gcount; P.info = t->d_info;
   P.c_count = t->b.c_count; P.trace = t->b.trace; P.gthresh = t->b.gthresh; P.tasks = t->b.tasks; P.gparts = t->b.gparts; P.gdone = t->b.gdone; P.part = t->b.part;
   P.N = t->N; P.n_groups = (unsigned)t->n_groups; P.eps2 = eps * eps;
-  walk_reset_kernel<<<1, 32, 0, t->stream>>>(t->d_info);
+  walk_reset_kernel<<<1, 32, 0, t->stream>>>(t->d_info, t->reuse_costs ? (unsigned)t->group : 0u);
   BH_LAUNCH_CHECK("walk_reset");
   long long want = (t->n_groups + WALK_WARPS - 1) / WALK_WARPS;
   long long cap = (long long)t->sm_count * WALK_MINB;
