@@ -132,3 +132,29 @@ def test_mw_model_2m_properties_and_sampled_parity():
     assert (np.abs(p - opot[sel]) / np.abs(opot[sel])).max() <= 1e-5
     assert bool(torch.isfinite(acc).all()) and bool(torch.isfinite(pot).all())
     t.close()
+
+
+def test_leapfrog_step_full_parity_with_reused_schedule():
+    # tree_leapfrog schedules the force walk from the previous pass's per-group counts (no counting
+    # pre-pass) and cuts expensive / tail groups into parts: the force of the step's LAST pass must still
+    # be the oracle's force on the step's positions: counts bit-exact, acc/pot <= 1e-5 (north_star).
+    n, theta, eps, dt = 200_000 + 77, 0.4, 0.01, 0.002
+    pos, vel, mass = milky_way(n, 41)
+    t = Tree(device=0)
+    t.build(pos.cuda(), mass.cuda()); t.set_velocity(vel.cuda()); t.force(theta, eps)
+    for _ in range(3):
+        t.leapfrog(dt)
+    p, v, a, ph = _state(t, n)
+    cnt = t.debug("counts")
+    ot = oracle.Tree(p, mass.numpy())  # the positions the last force pass saw
+    assert np.array_equal(t.debug("order"), ot.keys()[1])
+    assert np.array_equal(t.debug("cells"), ot.cells())
+    oacc, opot, onpp, onpc = ot.force(theta, eps)
+    assert np.array_equal(cnt[:, 0], onpp) and np.array_equal(cnt[:, 1], onpc)
+    rel = np.linalg.norm(a.astype(np.float64) - oacc, axis=1) / np.linalg.norm(oacc, axis=1)
+    prel = np.abs(ph - opot) / np.abs(opot)
+    assert rel.max() <= 1e-5 and prel.max() <= 1e-5, (rel.max(), prel.max())
+    trace = t.debug("task_trace")
+    parts = trace[:, 3] >> 26
+    assert parts.max() >= 1  # the schedule did contain split groups
+    t.close()
