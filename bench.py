@@ -219,6 +219,7 @@ def run_ours(args):
 
     # ---- device-resident steps: tree_leapfrog
     t.build(d_pos, d_mass); t.set_velocity(d_vel); t.force(cfg["theta"], cfg["eps"])
+    ke0, pe0 = t.energy()  # synchronised velocities: E(0) of the KDK run (T12)
     for _ in range(args.warmup):
         t.leapfrog(dt)
     barrier()
@@ -241,6 +242,9 @@ def run_ours(args):
     barrier()
     wall = time.perf_counter() - wall0
     launches = t.launch_count() - l0
+    ke1, pe1 = t.energy()
+    energy = {"steps": args.warmup + args.steps, "dt": dt, "e0": ke0 + pe0, "e1": ke1 + pe1,
+              "rel_drift": abs((ke1 + pe1) - (ke0 + pe0)) / abs(ke0 + pe0)}
     clocks = sampler.stop()
     step_ms = sum(a.elapsed_time(b) for a, b in ev)
     tt = torch.tensor([step_ms, float(pp_tot), float(pc_tot), phase_ms["walk"]], dtype=torch.float64, device=dev)
@@ -299,6 +303,14 @@ def run_ours(args):
         cpu = None
         if world == 1 and not args.no_cpu:
             cpu = _cpu_oracle_sample(cfg, pos.cpu().numpy(), mass.cpu().numpy(), budget_s=15.0)
+            if "steps" in cfg:  # config 5: energy drift of the oracle on its 262,144-particle version
+                import oracle
+                op, ov, om = gen(262144, 1006)
+                t0 = time.perf_counter()
+                *_, en = oracle.leapfrog(op.numpy(), ov.numpy(), om.numpy(), dt, args.warmup + args.steps,
+                                         cfg["theta"], cfg["eps"])
+                energy["oracle_262144"] = {"steps": args.warmup + args.steps, "seconds": time.perf_counter() - t0,
+                                           "rel_drift": abs(en[-1].sum() - en[0].sum()) / abs(en[0].sum())}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": step_ms_max / args.steps, "higher_is_better": True,
@@ -311,6 +323,7 @@ def run_ours(args):
             "pp_per_particle": pp_tot / args.steps / n, "pc_per_particle": pc_tot / args.steps / n,
             "phase_ms": {k: v / args.steps for k, v in phase_ms.items()},
             "roofline": roof,
+            "energy": energy,
             "cpu_baseline": cpu,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 16 * n,
                     "ms_per_step": 1e3 * e2e_s / args.steps, "phase_ms": e_phase,
