@@ -90,6 +90,16 @@ int tree_force_host(tree_ctx *t, float theta, float eps, float *acc, float *pot)
  * sums, written to HOST doubles (either may be NULL).  Synchronises. */
 int tree_energy(tree_ctx *t, double *kinetic, double *potential);
 
+/* Exact softened sum over ALL N particles of the current state for a list of targets (PAPER.md L29
+ * "each of the N objects exerts N-1 interactions"; L184-190 with Q = 0): for target i = idx[k],
+ * over all j != i (by index): phi = -sum m_j / s, a = sum m_j r / s^3, r = x_j - x_i,
+ * s^2 = |r|^2 + eps^2, evaluated and accumulated in FP64 from the FP32 state.  This is the
+ * "direct summation" the tree force is measured against (theta -> 0 limit, L31); it is O(n N).
+ * idx: DEV int64[n], caller-order particle indices in [0, N); acc: DEV double[n][3];
+ * pot: DEV double[n]; both are overwritten.  Needs tree_build (any later tree_leapfrog state is
+ * the one summed).  Asynchronous on the context's stream. */
+int tree_direct(tree_ctx *t, const long long *idx, long long n, float eps, double *acc, double *pot);
+
 /* Internal arrays for the parity tests, copied to HOST memory `dst`.  *count receives the number
  * of records; with dst == NULL only *count is written.  Synchronises.  `what`: */
 #define TREE_DBG_KEYS 0        /* uint64[N]     PH key per particle, caller order                  */

@@ -33,6 +33,7 @@ _SIGS = {
     "tree_get_state": (C.c_int, [C.c_void_p] * 5),
     "tree_build_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_longlong]),
     "tree_force_host": (C.c_int, [C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.c_void_p]),
+    "tree_direct": (C.c_int, [C.c_void_p, C.c_void_p, C.c_longlong, C.c_float, C.c_void_p, C.c_void_p]),
     "tree_energy": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     "tree_get_debug": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.POINTER(C.c_longlong)]),
     "tree_get_stats": (C.c_int, [C.c_void_p, C.c_void_p, C.POINTER(C.c_ulonglong), C.POINTER(C.c_ulonglong)]),
@@ -178,6 +179,10 @@ class Tree:
 
     def force_host(self, theta: float, eps: float, acc=None, pot=None):
         _check(self.h, load_library().tree_force_host(self.h, float(theta), float(eps), _ptr(acc), _ptr(pot)))
+
+    def direct(self, idx, eps, acc, pot):
+        """tree_direct: idx int64 device tensor [n]; acc float64 [n,3], pot float64 [n] device tensors."""
+        _check(self.h, load_library().tree_direct(self.h, _ptr(idx), int(idx.numel()), float(eps), _ptr(acc), _ptr(pot)))
 
     def energy(self):
         ke, pe = C.c_double(0), C.c_double(0)

@@ -245,6 +245,15 @@ int tree_get_state(tree_ctx *t, float *pos, float *vel, float *acc, float *pot) 
   return run_get_state(t, pos, vel, acc, pot);
 }
 
+int tree_direct(tree_ctx *t, const long long *idx, long long n, float eps, double *acc, double *pot) {
+  if (!t) return TREE_ERR_ARG;
+  if (!idx || !acc || !pot || n <= 0 || !(eps >= 0.0f) || !isfinite(eps))
+    return set_err(t, TREE_ERR_ARG, "tree_direct: bad argument");
+  if (t->N <= 0 || !t->b.posm) return set_err(t, TREE_ERR_ORDER, "tree_direct before tree_build");
+  BH_CUDA(cudaSetDevice(t->device));
+  return run_direct(t, idx, n, eps, acc, pot);
+}
+
 int tree_build_host(tree_ctx *t, const float *pos, const float *mass, long long N) {
   if (!t) return TREE_ERR_ARG;
   if (!pos || !mass || N <= 0 || N > 2147483647LL) return set_err(t, TREE_ERR_ARG, "tree_build_host: bad argument");

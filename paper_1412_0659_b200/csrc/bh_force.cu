@@ -786,6 +786,48 @@ __global__ void __launch_bounds__(256) get_state_kernel(const float4 *__restrict
 }
 
 // ------------------------------------------------------------------------------------------
+// Direct summation (the definition the tree force approximates), FP64.
+// One thread per target, sources staged through shared memory; the source range is cut over
+// blockIdx.y and the partial sums are added with FP64 atomics (acc / pot zeroed before).
+// ------------------------------------------------------------------------------------------
+constexpr int DIRECT_THREADS = 128;
+
+__global__ void __launch_bounds__(DIRECT_THREADS) direct_kernel(const float4 *__restrict__ posm, long long N,
+                                                                const long long *__restrict__ idx, long long n,
+                                                                double eps2, double *__restrict__ acc,
+                                                                double *__restrict__ pot) {
+  __shared__ float4 tile[DIRECT_THREADS];
+  const long long k = blockIdx.x * (long long)DIRECT_THREADS + threadIdx.x;
+  const long long i = k < n ? idx[k] : -1;
+  const float4 pi = i >= 0 ? posm[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+  const double xi = pi.x, yi = pi.y, zi = pi.z;
+  const long long chunk = (N + gridDim.y - 1) / gridDim.y;
+  const long long j0 = blockIdx.y * chunk, j1 = j0 + chunk < N ? j0 + chunk : N;
+  double ax = 0.0, ay = 0.0, az = 0.0, ph = 0.0;
+  for (long long base = j0; base < j1; base += DIRECT_THREADS) {
+    const long long j = base + threadIdx.x;
+    tile[threadIdx.x] = j < j1 ? posm[j] : make_float4(0.f, 0.f, 0.f, 0.f);
+    __syncthreads();
+    const int cnt = (int)(j1 - base < DIRECT_THREADS ? j1 - base : DIRECT_THREADS);
+#pragma unroll 4
+    for (int q = 0; q < cnt; ++q) {
+      const float4 s = tile[q];
+      const double dx = (double)s.x - xi, dy = (double)s.y - yi, dz = (double)s.z - zi;
+      const double r2 = dx * dx + dy * dy + dz * dz + eps2;
+      const double m = (base + q == i) ? 0.0 : (double)s.w;  // self term skipped by index (S2)
+      const double ri = (base + q == i) ? 0.0 : rsqrt(r2);
+      const double mr = m * ri, mr3 = mr * ri * ri;
+      ax += mr3 * dx; ay += mr3 * dy; az += mr3 * dz; ph -= mr;
+    }
+    __syncthreads();
+  }
+  if (i >= 0) {
+    atomicAdd(&acc[3 * k], ax); atomicAdd(&acc[3 * k + 1], ay); atomicAdd(&acc[3 * k + 2], az);
+    atomicAdd(&pot[k], ph);
+  }
+}
+
+// ------------------------------------------------------------------------------------------
 // host launchers
 // ------------------------------------------------------------------------------------------
 static inline unsigned blocks_for(long long n, int threads) { return (unsigned)((n + threads - 1) / threads); }
@@ -887,6 +929,22 @@ int run_energy(tree_ctx *t) {
 int run_set_velocity(tree_ctx *t, const float *vel) {
   set_vel_kernel<<<blocks_for(t->N, 256), 256, 0, t->stream>>>(vel, t->b.vel, t->N);
   BH_LAUNCH_CHECK("set_velocity");
+  return 0;
+}
+
+int run_direct(tree_ctx *t, const long long *idx, long long n, float eps, double *acc, double *pot) {
+  cudaError_t e = cudaMemsetAsync(acc, 0, (size_t)n * 3 * sizeof(double), t->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(pot, 0, (size_t)n * sizeof(double), t->stream);
+  if (e != cudaSuccess) return set_err(t, TREE_ERR_CUDA, "tree_direct: memset", e);
+  const unsigned gx = blocks_for(n, DIRECT_THREADS);
+  long long gy = ((long long)t->sm_count * 16 + gx - 1) / gx;  // about 16 blocks per SM in total
+  const long long gy_max = (t->N + 4 * DIRECT_THREADS - 1) / (4 * DIRECT_THREADS);
+  if (gy > gy_max) gy = gy_max;
+  if (gy < 1) gy = 1;
+  if (gy > 65535) gy = 65535;
+  direct_kernel<<<dim3(gx, (unsigned)gy), DIRECT_THREADS, 0, t->stream>>>(t->b.posm, t->N, idx, n,
+                                                                          (double)eps * (double)eps, acc, pot);
+  BH_LAUNCH_CHECK("direct");
   return 0;
 }
 

@@ -158,3 +158,31 @@ def test_leapfrog_step_full_parity_with_reused_schedule():
     parts = trace[:, 3] >> 26
     assert parts.max() >= 1  # the schedule did contain split groups
     t.close()
+
+
+def test_full_size_sampled_parity_config3():
+    # BASELINE config 3: Milky-Way-shaped, N = 8,388,608, eps = 0.01, theta = 0.4.  Integer stages and
+    # moments on the full arrays (bit-exact); counts and forces against the oracle on every 509th group.
+    cfg, pos, vel, mass = config(2, with_vel=False)
+    n = cfg["n"]
+    t = Tree(device=0)
+    acc = torch.empty((n, 3), device="cuda"); pot = torch.empty(n, device="cuda")
+    t.build(pos.cuda(), mass.cuda()); t.force(cfg["theta"], cfg["eps"], acc, pot)
+    torch.cuda.synchronize()
+    ot = oracle.Tree(pos.numpy(), mass.numpy())
+    key, order, skey = ot.keys()
+    assert np.array_equal(t.debug("keys"), key)
+    assert np.array_equal(t.debug("order"), order)
+    assert np.array_equal(t.debug("cells"), ot.cells())
+    assert np.array_equal(t.debug("moments"), ot.moments())
+    stride = 509
+    oacc, opot, onpp, onpc = ot.force(cfg["theta"], cfg["eps"], g0=3, stride=stride)
+    gsel = np.arange(3, ot.n_groups, stride)
+    cnt = t.debug("counts")
+    assert np.array_equal(cnt[gsel, 0], onpp[gsel]) and np.array_equal(cnt[gsel, 1], onpc[gsel])
+    sel = np.concatenate([order[64 * g: 64 * g + 64] for g in gsel])
+    a = acc.cpu().numpy().astype(np.float64)[sel]; p = pot.cpu().numpy().astype(np.float64)[sel]
+    rel = np.linalg.norm(a - oacc[sel], axis=1) / np.linalg.norm(oacc[sel], axis=1)
+    assert rel.max() <= 1e-5, rel.max()
+    assert (np.abs(p - opot[sel]) / np.abs(opot[sel])).max() <= 1e-5
+    t.close()
