@@ -182,6 +182,7 @@ def run_ours(args):
 
     from nbody_inputs import config
     from paper_1412_0659_b200 import Tree, effective_flops
+    from paper_1412_0659_b200.replicas import replica_seed, reduce_max_sum, whole_job_rate
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -197,7 +198,7 @@ def run_ours(args):
     cfg = dict(CONFIGS[args.config])
     if args.n:
         cfg["n"] = args.n
-    cfg["seed"] = cfg["seed"] + 7919 * rank  # every rank its own replica of the workload
+    cfg["seed"] = replica_seed(cfg["seed"], rank)  # every rank its own replica of the workload
     from nbody_inputs import plummer, milky_way
     gen = plummer if cfg["model"] == "plummer" else milky_way
     gen_dev = dev if cfg["n"] > (1 << 22) else "cpu"
@@ -247,14 +248,9 @@ def run_ours(args):
               "rel_drift": abs((ke1 + pe1) - (ke0 + pe0)) / abs(ke0 + pe0)}
     clocks = sampler.stop()
     step_ms = sum(a.elapsed_time(b) for a, b in ev)
-    tt = torch.tensor([step_ms, float(pp_tot), float(pc_tot), phase_ms["walk"]], dtype=torch.float64, device=dev)
-    if world > 1:
-        mx = tt.clone(); dist.all_reduce(mx, op=dist.ReduceOp.MAX)
-        sm = tt.clone(); dist.all_reduce(sm, op=dist.ReduceOp.SUM)
-        step_ms_max, walk_ms_max = float(mx[0]), float(mx[3])
-        pp_all, pc_all = float(sm[1]), float(sm[2])
-    else:
-        step_ms_max, walk_ms_max, pp_all, pc_all = step_ms, phase_ms["walk"], float(pp_tot), float(pc_tot)
+    mx, sm = reduce_max_sum([step_ms, float(pp_tot), float(pc_tot), phase_ms["walk"]], dev)
+    step_ms_max, walk_ms_max = mx[0], mx[3]
+    pp_all, pc_all = sm[1], sm[2]
     value = (pp_all + pc_all) / (step_ms_max * 1e-3)
 
     # ---- end to end through the C ABI with host buffers (build + force, copies timed)
@@ -276,13 +272,7 @@ def run_ours(args):
         for key, v in ems.items():
             e_phase[key] = e_phase.get(key, 0.0) + v / args.steps
         e_pp += pp; e_pc += pc
-    te = torch.tensor([e2e_s, float(e_pp + e_pc)], dtype=torch.float64, device=dev)
-    if world > 1:
-        mx = te.clone(); dist.all_reduce(mx, op=dist.ReduceOp.MAX)
-        sm = te.clone(); dist.all_reduce(sm, op=dist.ReduceOp.SUM)
-        e2e_val = float(sm[1]) / float(mx[0])
-    else:
-        e2e_val = (e_pp + e_pc) / e2e_s
+    e2e_val = whole_job_rate(e2e_s, float(e_pp + e_pc), dev)
     t2.close()
 
     if rank == 0:
