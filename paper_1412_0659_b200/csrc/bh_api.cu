@@ -278,7 +278,9 @@ int tree_force_host(tree_ctx *t, float theta, float eps, float *acc, float *pot)
   if (rc) return rc;
   if (acc) BH_CUDA(cudaMemcpyAsync(acc, t->b.out_acc, (size_t)t->N * 12, cudaMemcpyDeviceToHost, t->stream));
   if (pot) BH_CUDA(cudaMemcpyAsync(pot, t->b.out_pot, (size_t)t->N * 4, cudaMemcpyDeviceToHost, t->stream));
+  BH_CUDA(cudaMemcpyAsync(&t->h_info->walk_overflow, &t->d_info->walk_overflow, sizeof(unsigned), cudaMemcpyDeviceToHost, t->stream));
   BH_CUDA(cudaStreamSynchronize(t->stream));
+  if (t->h_info->walk_overflow) return set_err(t, TREE_ERR_CUDA, "force walk: stack overflow, results invalid");
   return TREE_OK;
 }
 
@@ -427,6 +429,7 @@ int tree_get_stats(tree_ctx *t, double *ms, unsigned long long *n_pp, unsigned l
     BH_CUDA(cudaMemcpy(t->h_info, t->d_info, sizeof(DevInfo), cudaMemcpyDeviceToHost));
     if (n_pp) *n_pp = t->h_info->n_pp;
     if (n_pc) *n_pc = t->h_info->n_pc;
+    if (t->have_force && t->h_info->walk_overflow) return set_err(t, TREE_ERR_CUDA, "force walk: stack overflow, results invalid");
   }
   return TREE_OK;
 }

@@ -29,7 +29,8 @@ struct DevInfo {
   unsigned int group_ticket;      // dynamic group fetch counter of the counting walk
   unsigned int task_ticket;       // dynamic task fetch counter of the force walk
   unsigned int n_tasks, n_tasks_a;  // tasks in the list; of which parts of expensive groups (listed first)
-  unsigned int tail_start, pad0;    // first task of the tail region (last groups, split into small tasks)
+  unsigned int tail_start;          // first task of the tail region (last groups, split into small tasks)
+  unsigned int walk_overflow;       // set if a warp's walk stack would have overflowed (results invalid)
   unsigned int sched_tot[2];      // totals of the two scheduling scans
   double ekin, epot;
 };

@@ -58,7 +58,10 @@ constexpr int PP_UNROLL = BH_PP_UNROLL, PC_UNROLL = BH_PC_UNROLL;  // sources pe
 constexpr int WALK_WARPS = 4;
 constexpr int WALK_MINB = BH_WALK_MINB;  // resident blocks per SM the register budget is sized for
 constexpr int COUNT_MINB = 8;            // same for the counting pre-pass (38 registers; shared memory allows 8 blocks)
-constexpr unsigned COUNT_TRUNC = 256;  // the counting walk treats cells this small as opened leaves
+#ifndef BH_COUNT_TRUNC
+#define BH_COUNT_TRUNC 256
+#endif
+constexpr unsigned COUNT_TRUNC = BH_COUNT_TRUNC;  // the counting walk treats cells this small as opened leaves
 constexpr int FOLD_EVERY = 4;    // tiles (of 32 sources) summed in plain FP32 between compensated folds
 constexpr int DEFER_CAP = 256;   // deferred child ranges one part of a split group may own
 constexpr int STACK_CAP = 1024;  // >= 32 per level (depth-first: 32 x 22) + DEFER_CAP
@@ -437,6 +440,10 @@ __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, con
       const unsigned m = __ballot_sync(0xffffffffu, open_int);
       if (open_int) ws.stack[sp + __popc(m & gt)] = (lk.x << 3) | ((lk.y & 0xfu) - 1u);
       sp += __popc(m);
+      if (sp + dp + 32 > STACK_CAP) {  // cannot happen within the bounds of DESIGN.md §Walk; never write past the stack
+        if (lane == 0) P.info->walk_overflow = 1u;
+        sp = 0; dp = 0;
+      }
     }
     // ---- accepted cells -> p-c queue
     {
@@ -609,6 +616,7 @@ __global__ void walk_reset_kernel(DevInfo *info, unsigned reuse_gs) {
     const unsigned long long prev = reuse_gs ? (13ull * info->n_pp + 37ull * info->n_pc) / reuse_gs : 0ull;
     info->group_ticket = 0; info->task_ticket = 0; info->n_pp = 0; info->n_pc = 0; info->n_tasks = 0;
     info->sched_cost = prev;
+    info->walk_overflow = 0;
     unsigned long long now;
     asm volatile("mov.u64 %0, %globaltimer;" : "=l"(now));
     info->t0_ns = now;
