@@ -24,3 +24,14 @@ def pytest_collection_modifyitems(config, items):
     for it in items:
         if "gpu" in it.keywords:
             it.add_marker(skip)
+
+
+@pytest.fixture(scope="session", autouse=True)
+def _built_libraries():
+    """Build (if stale or missing) the CUDA library and the C++ oracle once per session: nvcc
+    cross-compiles without a GPU, so this also runs in the CPU-only suite."""
+    from paper_1412_0659_b200 import build as cuda_build
+    cuda_build.build(force=False)
+    import oracle
+    oracle.build()
+    yield
