@@ -10,6 +10,7 @@ from .generators import (  # noqa: F401
     uniform01,
     plummer,
     milky_way,
+    milky_way_clumpy,
     subsample_indices,
     config,
     CONFIGS,

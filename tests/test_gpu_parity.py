@@ -188,3 +188,29 @@ def test_host_buffer_calls_match_device_calls():
     t2.build_host(hp, hm); t2.force_host(0.4, 0.01, ha, hph)
     assert np.array_equal(ha.numpy().astype(np.float64), acc) and np.array_equal(hph.numpy().astype(np.float64), pot)
     t.close(); t2.close()
+
+
+def test_clumpy_disk_full_parity():
+    # SURVEY.md §8(f) NEXT-4 (structured disks cost more): compact clumps in the disk give a
+    # deep tree and very uneven group costs; every stage must still equal the oracle's.
+    from nbody_inputs import milky_way_clumpy
+    n, theta, eps = 150_000 + 5, 0.4, 0.01
+    pos, mass = milky_way_clumpy(n, 1007, n_clumps=24, clump_fraction=0.3, clump_scale=0.01)
+    t = Tree(device=0)
+    acc = torch.empty((n, 3), device="cuda"); pot = torch.empty(n, device="cuda")
+    t.build(pos.cuda(), mass.cuda()); t.force(theta, eps, acc, pot)
+    torch.cuda.synchronize()
+    ot = oracle.Tree(pos.numpy(), mass.numpy())
+    assert np.array_equal(t.debug("order"), ot.keys()[1])
+    assert np.array_equal(t.debug("cells"), ot.cells())
+    assert np.array_equal(t.debug("moments"), ot.moments())
+    oacc, opot, onpp, onpc = ot.force(theta, eps)
+    cnt = t.debug("counts")
+    assert np.array_equal(cnt[:, 0], onpp) and np.array_equal(cnt[:, 1], onpc)
+    a = acc.cpu().numpy().astype(np.float64); p = pot.cpu().numpy().astype(np.float64)
+    rel = np.linalg.norm(a - oacc, axis=1) / np.linalg.norm(oacc, axis=1)
+    assert rel.max() <= 1e-5, rel.max()
+    assert (np.abs(p - opot) / np.abs(opot)).max() <= 1e-5
+    assert ot.cells()[:, 0].max() >= 12  # the clumps do deepen the tree
+    ms, pp, pc = t.stats()  # raises if the walk stack guard fired
+    t.close()

@@ -57,3 +57,21 @@ def test_subsample_and_configs():
     assert [CONFIGS[k]["n"] for k in range(5)] == [16384, 1048576, 8388608, 134217728, 33554432]
     cfg, pos, vel, m = config(0)
     assert cfg["eps"] == 0.01 and cfg["theta"] == 0.4 and pos.shape == (16384, 3)
+
+
+def test_clumpy_disk_moves_only_disk_particles_and_is_seeded():
+    import torch
+    from nbody_inputs import milky_way, milky_way_clumpy
+    from nbody_inputs.generators import mw_counts
+    n = 48000
+    p1, m1 = milky_way_clumpy(n, 9)
+    p2, m2 = milky_way_clumpy(n, 9)
+    q, _, mq = milky_way(n, 9, with_vel=False)
+    assert torch.equal(p1, p2) and torch.equal(m1, m2) and torch.equal(m1, mq)
+    nd, nb, nh = mw_counts(n)
+    moved = (p1 != q).any(dim=1)
+    assert int(moved.sum()) == int(nd * 0.2) and not bool(moved[int(nd * 0.2):].any())
+    assert bool(torch.isfinite(p1).all()) and torch.unique(p1, dim=0).shape[0] == n
+    # the clumps are compact: moved particles sit within a few scale radii of an unmoved disk particle
+    d = torch.cdist(p1[moved][:200].double(), q[int(nd * 0.2):nd].double()).min(dim=1).values
+    assert float(d.median()) < 0.1
