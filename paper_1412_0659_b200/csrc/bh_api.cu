@@ -62,6 +62,11 @@ static int ensure_particles(tree_ctx *t, long long N) {
   t->scan_cap = (s1 > s2 ? s1 : s2) + 4096;
   BH_TRY(dev_alloc(t, b.scan_tmp, t->scan_cap));
   BH_TRY(dev_alloc(t, b.scan_blk, t->scan_cap / 4096 + 16));
+  BH_TRY(dev_alloc(t, b.sort_hist, 8 * 256 + 8));
+  t->sort_status_cap = 256 * ((cap + 2047) / 2048);
+  BH_TRY(dev_alloc(t, b.sort_status, t->sort_status_cap));
+  BH_CUDA(cudaMemsetAsync(b.sort_status, 0, (size_t)t->sort_status_cap * sizeof(unsigned long long), t->stream));
+  t->sort_epoch = 0;
   t->cap = cap;
   t->have_vel = false;
   t->have_force = false;
@@ -88,7 +93,7 @@ int ensure_cells(tree_ctx *t, long long nc) {
 
 static void free_all(tree_ctx *t) {
   Buffers &b = t->b;
-  void *ptrs[] = {b.posm, b.vel, b.acc, b.key[0], b.key[1], b.idx[0], b.idx[1], b.scan_tmp, b.scan_blk, b.spos, b.sacc,
+  void *ptrs[] = {b.posm, b.vel, b.acc, b.key[0], b.key[1], b.idx[0], b.idx[1], b.scan_tmp, b.scan_blk, b.sort_hist, b.sort_status, b.spos, b.sacc,
                   b.lv, b.gbox, b.gcount, b.sched_a, b.sched_b, b.gdone, b.gparts, b.gthresh, b.tasks, b.part, b.trace, b.c_level, b.c_first, b.c_count, b.c_fcall, b.c_link, b.c_cm, b.c_qa, b.c_qb,
                   b.c_test, b.in_pos, b.in_mass, b.out_acc, b.out_pot};
   for (void *p : ptrs) if (p) cudaFree(p);

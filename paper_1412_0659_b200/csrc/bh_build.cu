@@ -222,69 +222,112 @@ int device_excl_scan(tree_ctx *t, uint32_t *a, long long n, uint32_t *total_out)
 }
 
 // ------------------------------------------------------------------------------------------
-// a3: stable LSD radix sort of (key 64-bit, index 32-bit), 8 bits per pass.
-// Per pass: tile histograms -> device-wide scan (digit-major) -> stable tile scatter.
+// a3: stable LSD radix sort of (key 64-bit, index 32-bit), 8 bits per pass, 8 passes.
 // ------------------------------------------------------------------------------------------
-constexpr int SORT_THREADS = 512;
-constexpr int SORT_IPT = 8;
-constexpr int SORT_TILE = SORT_THREADS * SORT_IPT;  // 4096
-constexpr int SORT_WARPS = SORT_THREADS / 32;
 constexpr int RADIX = 256;
 
-__global__ void __launch_bounds__(SORT_THREADS) sort_hist_kernel(const uint64_t *__restrict__ kin, long long N,
-                                                                  int shift, int ntiles, uint32_t *__restrict__ hist) {
-  __shared__ unsigned h[RADIX];
-  if (threadIdx.x < RADIX) h[threadIdx.x] = 0;
+// ------------------------------------------------------------------------------------------
+// One-sweep form: one pass over the keys builds the 8 digit histograms; each of the 8 passes
+// is then ONE kernel that ranks a tile, obtains the tile's global digit offsets by decoupled
+// look-back over the preceding tiles' status words, and scatters. Per pass 12 B read + 12 B
+// written per particle (+ 2 KB of status per 2048-key tile); 10 launches instead of 40.
+// Tiles take their index from an atomic ticket, so a tile only ever waits for tiles that are
+// already running or finished. Status word: flag (2 bits) | epoch (30 bits) | value (32 bits);
+// the epoch changes every pass, so the array is never cleared.
+// ------------------------------------------------------------------------------------------
+constexpr int OS_THREADS = 256;
+constexpr int OS_IPT = 8;
+constexpr int OS_TILE = OS_THREADS * OS_IPT;  // 2048
+constexpr int OS_WARPS = OS_THREADS / 32;
+#ifndef BH_OS_MINB
+#define BH_OS_MINB 5
+#endif
+constexpr int OS_MINB = BH_OS_MINB;  // resident blocks per SM (shared memory allows 6)
+constexpr unsigned long long OS_LOCAL = 1ull << 62, OS_INCL = 2ull << 62;
+
+__global__ void __launch_bounds__(256) sort_hist8_kernel(const uint64_t *__restrict__ key, long long N,
+                                                         uint32_t *__restrict__ ghist /*[8][256]*/) {
+  __shared__ unsigned h[8 * RADIX];
+  for (int i = threadIdx.x; i < 8 * RADIX; i += blockDim.x) h[i] = 0;
   __syncthreads();
-  long long base = (long long)blockIdx.x * SORT_TILE;
+  for (long long p = blockIdx.x * (long long)blockDim.x + threadIdx.x; p < N; p += (long long)gridDim.x * blockDim.x) {
+    const uint64_t k = key[p];
 #pragma unroll
-  for (int k = 0; k < SORT_IPT; ++k) {
-    long long p = base + k * SORT_THREADS + threadIdx.x;
-    if (p < N) atomicAdd(&h[(unsigned)(kin[p] >> shift) & 255u], 1u);
+    for (int d = 0; d < 8; ++d) atomicAdd(&h[d * RADIX + ((unsigned)(k >> (8 * d)) & 255u)], 1u);
   }
   __syncthreads();
-  if (threadIdx.x < RADIX) hist[(long long)threadIdx.x * ntiles + blockIdx.x] = h[threadIdx.x];
+  for (int i = threadIdx.x; i < 8 * RADIX; i += blockDim.x) {
+    const unsigned v = h[i];
+    if (v) atomicAdd(&ghist[i], v);
+  }
 }
 
-struct SortSmem {
-  uint64_t key[SORT_TILE];
-  uint32_t val[SORT_TILE];
-  unsigned wc[SORT_WARPS][RADIX];
+// exclusive scan of each of the 8 histograms (block p handles pass p); also clears the tile tickets
+__global__ void __launch_bounds__(RADIX) sort_scan8_kernel(uint32_t *__restrict__ ghist, uint32_t *__restrict__ ticket) {
+  __shared__ unsigned s_w[9];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const unsigned v = ghist[blockIdx.x * RADIX + threadIdx.x];
+  const unsigned inc = warp_incl_scan(v, lane);
+  if (lane == 31) s_w[w] = inc;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    unsigned run = 0;
+    for (int k = 0; k < RADIX / 32; ++k) { unsigned c = s_w[k]; s_w[k] = run; run += c; }
+    ticket[blockIdx.x] = 0;
+  }
+  __syncthreads();
+  ghist[blockIdx.x * RADIX + threadIdx.x] = inc - v + s_w[w];
+}
+
+__device__ __forceinline__ unsigned long long ld_status(const unsigned long long *p) {
+  unsigned long long v;
+  asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_status(unsigned long long *p, unsigned long long v) {
+  asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+
+struct OsSmem {
+  uint64_t key[OS_TILE];
+  uint32_t val[OS_TILE];
+  unsigned wc[OS_WARPS][RADIX];
   unsigned dstart[RADIX];
   unsigned gbase[RADIX];
+  unsigned tile;
 };
 
-__global__ void __launch_bounds__(SORT_THREADS) sort_scatter_kernel(const uint64_t *__restrict__ kin,
-                                                                     const uint32_t *__restrict__ vin,
-                                                                     uint64_t *__restrict__ kout,
-                                                                     uint32_t *__restrict__ vout,
-                                                                     const uint32_t *__restrict__ scanned, int shift,
-                                                                     long long N, int ntiles) {
+__global__ void __launch_bounds__(OS_THREADS, OS_MINB) sort_onesweep_kernel(const uint64_t *__restrict__ kin,
+                                                                   const uint32_t *__restrict__ vin,
+                                                                   uint64_t *__restrict__ kout, uint32_t *__restrict__ vout,
+                                                                   const uint32_t *__restrict__ gscan /*[256] of this pass*/,
+                                                                   uint32_t *__restrict__ ticket,
+                                                                   unsigned long long *__restrict__ status /*[tiles][256]*/,
+                                                                   unsigned long long epoch, int shift, long long N) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  SortSmem &sm = *reinterpret_cast<SortSmem *>(smem_raw);
+  OsSmem &sm = *reinterpret_cast<OsSmem *>(smem_raw);
   const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const unsigned lt = (1u << lane) - 1u;
-  const long long base = (long long)blockIdx.x * SORT_TILE;
+  if (threadIdx.x == 0) sm.tile = atomicAdd(ticket, 1u);
   for (int i = lane; i < RADIX; i += 32) sm.wc[w][i] = 0;
-  if (threadIdx.x < RADIX) sm.gbase[threadIdx.x] = scanned[(long long)threadIdx.x * ntiles + blockIdx.x];
-  __syncwarp();
-  uint64_t key[SORT_IPT];
-  uint32_t val[SORT_IPT];
-  unsigned rank[SORT_IPT];
+  __syncthreads();
+  const unsigned tile = sm.tile;
+  const long long base = (long long)tile * OS_TILE;
+  uint64_t key[OS_IPT];
+  unsigned rank[OS_IPT];
   // warp-striped: warp w owns items [w*256, w*256+256) of the tile, item k of lane l at k*32+l
 #pragma unroll
-  for (int k = 0; k < SORT_IPT; ++k) {
-    long long p = base + w * (32 * SORT_IPT) + k * 32 + lane;
-    bool valid = p < N;
+  for (int k = 0; k < OS_IPT; ++k) {
+    const long long p = base + w * (32 * OS_IPT) + k * 32 + lane;
+    const bool valid = p < N;
     key[k] = valid ? kin[p] : 0;
-    val[k] = valid ? (vin ? vin[p] : (uint32_t)p) : 0;
   }
 #pragma unroll
-  for (int k = 0; k < SORT_IPT; ++k) {
-    long long p = base + w * (32 * SORT_IPT) + k * 32 + lane;
-    bool valid = p < N;
-    unsigned d = (unsigned)(key[k] >> shift) & 255u;
-    unsigned act = __ballot_sync(0xffffffffu, valid);
+  for (int k = 0; k < OS_IPT; ++k) {
+    const long long p = base + w * (32 * OS_IPT) + k * 32 + lane;
+    const bool valid = p < N;
+    const unsigned d = (unsigned)(key[k] >> shift) & 255u;
+    const unsigned act = __ballot_sync(0xffffffffu, valid);
     unsigned peers = 0, c0 = 0;
     if (valid) {
       peers = __match_any_sync(act, d);
@@ -296,19 +339,35 @@ __global__ void __launch_bounds__(SORT_THREADS) sort_scatter_kernel(const uint64
     rank[k] = c0 + __popc(peers & lt);
   }
   __syncthreads();
-  // per digit: exclusive prefix over warps, tile total
-  if (threadIdx.x < RADIX) {
+  // thread d: digit d's exclusive prefix over the warps, the tile's count, then the look-back
+  {
+    const unsigned d = threadIdx.x;
     unsigned run = 0;
 #pragma unroll
-    for (int ww = 0; ww < SORT_WARPS; ++ww) {
-      unsigned c = sm.wc[ww][threadIdx.x];
-      sm.wc[ww][threadIdx.x] = run;
+    for (int ww = 0; ww < OS_WARPS; ++ww) {
+      const unsigned c = sm.wc[ww][d];
+      sm.wc[ww][d] = run;
       run += c;
     }
-    sm.dstart[threadIdx.x] = run;
+    sm.dstart[d] = run;  // tile count of digit d (scanned below)
+    unsigned long long *mine = status + (size_t)tile * RADIX + d;
+    const unsigned long long tag = epoch << 32;
+    unsigned excl = 0;
+    if (tile > 0) {
+      st_status(mine, OS_LOCAL | tag | run);
+      for (long long q = (long long)tile - 1; q >= 0; --q) {
+        const unsigned long long *pq = status + (size_t)q * RADIX + d;
+        unsigned long long v;
+        do { v = ld_status(pq); } while ((v & 0x3fffffff00000000ull) != tag || (v >> 62) == 0ull);
+        excl += (unsigned)v;
+        if ((v >> 62) == 2ull) break;
+      }
+    }
+    st_status(mine, OS_INCL | tag | (unsigned long long)(excl + run));
+    sm.gbase[d] = gscan[d] + excl;
   }
   __syncthreads();
-  if (w == 0) {  // exclusive scan of the 256 digit totals
+  if (w == 0) {  // exclusive scan of the 256 tile counts
     unsigned v[8], s = 0;
 #pragma unroll
     for (int j = 0; j < 8; ++j) { v[j] = sm.dstart[lane * 8 + j]; s += v[j]; }
@@ -318,22 +377,22 @@ __global__ void __launch_bounds__(SORT_THREADS) sort_scatter_kernel(const uint64
   }
   __syncthreads();
 #pragma unroll
-  for (int k = 0; k < SORT_IPT; ++k) {
-    long long p = base + w * (32 * SORT_IPT) + k * 32 + lane;
+  for (int k = 0; k < OS_IPT; ++k) {
+    const long long p = base + w * (32 * OS_IPT) + k * 32 + lane;
     if (p < N) {
-      unsigned d = (unsigned)(key[k] >> shift) & 255u;
-      unsigned q = sm.dstart[d] + sm.wc[w][d] + rank[k];
+      const unsigned d = (unsigned)(key[k] >> shift) & 255u;
+      const unsigned q = sm.dstart[d] + sm.wc[w][d] + rank[k];
       sm.key[q] = key[k];
-      sm.val[q] = val[k];
+      sm.val[q] = vin ? vin[p] : (uint32_t)p;  // payload read late: 8 registers fewer while ranking
     }
   }
   __syncthreads();
-  long long rem = N - base;
-  int cnt = rem < SORT_TILE ? (int)rem : SORT_TILE;
-  for (int j = threadIdx.x; j < cnt; j += SORT_THREADS) {
-    uint64_t kk = sm.key[j];
-    unsigned d = (unsigned)(kk >> shift) & 255u;
-    long long dst = (long long)sm.gbase[d] + (j - sm.dstart[d]);
+  const long long rem = N - base;
+  const int cnt = rem < OS_TILE ? (int)rem : OS_TILE;
+  for (int j = threadIdx.x; j < cnt; j += OS_THREADS) {
+    const uint64_t kk = sm.key[j];
+    const unsigned d = (unsigned)(kk >> shift) & 255u;
+    const long long dst = (long long)sm.gbase[d] + (j - (int)sm.dstart[d]);
     kout[dst] = kk;
     vout[dst] = sm.val[j];
   }
@@ -626,21 +685,29 @@ int run_keys(tree_ctx *t) {
 int run_sort(tree_ctx *t) {
   static bool attr_set = false;
   if (!attr_set) {
-    BH_CUDA(cudaFuncSetAttribute(sort_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem)));
+    BH_CUDA(cudaFuncSetAttribute(sort_onesweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(OsSmem)));
+    BH_CUDA(cudaFuncSetAttribute(sort_onesweep_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
     attr_set = true;
   }
-  const int ntiles = (int)((t->N + SORT_TILE - 1) / SORT_TILE);
+  const unsigned ntiles = (unsigned)((t->N + OS_TILE - 1) / OS_TILE);
+  uint32_t *ghist = t->b.sort_hist, *ticket = t->b.sort_hist + 8 * RADIX;
+  BH_CUDA(cudaMemsetAsync(ghist, 0, 8 * RADIX * sizeof(uint32_t), t->stream));
+  const long long hwant = (t->N + 256 * 16 - 1) / (256 * 16), hcap = (long long)t->sm_count * 8;
+  sort_hist8_kernel<<<(unsigned)(hwant < hcap ? hwant : hcap), 256, 0, t->stream>>>(t->b.key[0], t->N, ghist);
+  BH_LAUNCH_CHECK("sort_hist8");
+  sort_scan8_kernel<<<8, RADIX, 0, t->stream>>>(ghist, ticket);
+  BH_LAUNCH_CHECK("sort_scan8");
   int cur = 0;
   for (int pass = 0; pass < 8; ++pass) {
-    const int shift = 8 * pass;
-    sort_hist_kernel<<<ntiles, SORT_THREADS, 0, t->stream>>>(t->b.key[cur], t->N, shift, ntiles, t->b.scan_tmp);
-    BH_LAUNCH_CHECK("sort_hist");
-    int rc = device_excl_scan(t, t->b.scan_tmp, (long long)RADIX * ntiles, nullptr);
-    if (rc) return rc;
-    sort_scatter_kernel<<<ntiles, SORT_THREADS, sizeof(SortSmem), t->stream>>>(
-        t->b.key[cur], pass == 0 ? nullptr : t->b.idx[cur], t->b.key[cur ^ 1], t->b.idx[cur ^ 1], t->b.scan_tmp, shift,
-        t->N, ntiles);
-    BH_LAUNCH_CHECK("sort_scatter");
+    const unsigned long long epoch = (++t->sort_epoch) & 0x3fffffffull;
+    if (epoch == 0) {  // wrapped: old words could alias the new epoch
+      BH_CUDA(cudaMemsetAsync(t->b.sort_status, 0, (size_t)t->sort_status_cap * sizeof(unsigned long long), t->stream));
+      ++t->sort_epoch;
+    }
+    sort_onesweep_kernel<<<ntiles, OS_THREADS, sizeof(OsSmem), t->stream>>>(
+        t->b.key[cur], pass == 0 ? nullptr : t->b.idx[cur], t->b.key[cur ^ 1], t->b.idx[cur ^ 1], ghist + pass * RADIX,
+        ticket + pass, t->b.sort_status, t->sort_epoch & 0x3fffffffull, 8 * pass, t->N);
+    BH_LAUNCH_CHECK("sort_onesweep");
     cur ^= 1;
   }
   t->sorted = cur;

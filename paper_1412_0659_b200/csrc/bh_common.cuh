@@ -43,7 +43,9 @@ struct Buffers {
   // sort
   uint64_t *key[2] = {nullptr, nullptr};
   uint32_t *idx[2] = {nullptr, nullptr};
-  uint32_t *scan_tmp = nullptr;  // tile histograms / tile level counts (scanned in place)
+  uint32_t *scan_tmp = nullptr;  // tile level counts of the tree build / scheduling scans (scanned in place)
+  uint32_t *sort_hist = nullptr;              // [8][256] digit histograms -> global digit offsets, then 8 tile tickets
+  unsigned long long *sort_status = nullptr;  // [sort tiles][256] decoupled look-back words of the one-sweep sort
   uint32_t *scan_blk = nullptr;  // block sums for the device-wide scan
   // slot (sorted) order
   float4 *spos = nullptr;
@@ -82,6 +84,8 @@ struct tree_ctx {
   long long n_cells = 0, cell_cap = 0;
   long long n_groups = 0;
   long long scan_cap = 0;
+  long long sort_status_cap = 0;     // words in b.sort_status
+  unsigned long long sort_epoch = 0; // look-back epoch: one per sort pass, never reused before a clear
   long long head_cap = 0, tail_cap = 0;  // partial-sum slots for expensive-group parts / tail parts
   int sorted = 0;                    // which of key[]/idx[] holds the sorted result
   bool built = false, have_vel = false, have_force = false;

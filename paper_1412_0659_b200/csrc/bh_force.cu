@@ -365,18 +365,20 @@ __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, con
     if (sp == 0) {
       if (!COUNT) flush_queues<TPL>(ws, lane, S, T, R, P, (uint32_t)g0, gsize);
       if (!(SPLIT && prefix)) break;
-      for (int base = 0; base < dp; base += 32) {
-        const int i = base + lane;
-        const unsigned e = i < dp ? ws.stack[STACK_CAP - 1 - i] : 0u;
+      if constexpr (!COUNT) {
+        for (int base = 0; base < dp; base += 32) {
+          const int i = base + lane;
+          const unsigned e = i < dp ? ws.stack[STACK_CAP - 1 - i] : 0u;
+          __syncwarp();
+          if (i < dp) ws.stack[i] = e;
+        }
         __syncwarp();
-        if (i < dp) ws.stack[i] = e;
+        sp = dp; dp = 0;
+        prefix = false;
+        S.tile_parts = 1; S.tile_wait = 0;
+        if (part != 0) { n_pp = 0; n_pc = 0; }  // the prefix is counted by part 0 only
+        if (sp == 0) break;
       }
-      __syncwarp();
-      sp = dp; dp = 0;
-      prefix = false;
-      S.tile_parts = 1; S.tile_wait = 0;
-      if (part != 0) { n_pp = 0; n_pc = 0; }  // the prefix is counted by part 0 only
-      if (sp == 0) break;
     }
     // ---- pop exactly min(32, cells on stack) cells from the top (deepest first)
     const int live = sp;
