@@ -244,6 +244,10 @@ constexpr int OS_WARPS = OS_THREADS / 32;
 #endif
 constexpr int OS_MINB = BH_OS_MINB;  // resident blocks per SM (shared memory allows 6)
 constexpr unsigned long long OS_LOCAL = 1ull << 62, OS_INCL = 2ull << 62;
+#ifndef BH_OS_LOOK
+#define BH_OS_LOOK 4
+#endif
+constexpr int OS_LOOK = BH_OS_LOOK;  // status words one thread keeps in flight during the look-back
 
 __global__ void __launch_bounds__(256) sort_hist8_kernel(const uint64_t *__restrict__ key, long long N,
                                                          uint32_t *__restrict__ ghist /*[8][256]*/) {
@@ -355,12 +359,21 @@ __global__ void __launch_bounds__(OS_THREADS, OS_MINB) sort_onesweep_kernel(cons
     unsigned excl = 0;
     if (tile > 0) {
       st_status(mine, OS_LOCAL | tag | run);
-      for (long long q = (long long)tile - 1; q >= 0; --q) {
-        const unsigned long long *pq = status + (size_t)q * RADIX + d;
-        unsigned long long v;
-        do { v = ld_status(pq); } while ((v & 0x3fffffff00000000ull) != tag || (v >> 62) == 0ull);
-        excl += (unsigned)v;
-        if ((v >> 62) == 2ull) break;
+      // look back over the preceding tiles, OS_LOOK status words in flight at a time
+      bool done = false;
+      for (long long q = (long long)tile - 1; q >= 0 && !done; q -= OS_LOOK) {
+        unsigned long long v[OS_LOOK];
+#pragma unroll
+        for (int j = 0; j < OS_LOOK; ++j)
+          v[j] = (q - j >= 0) ? ld_status(status + (size_t)(q - j) * RADIX + d) : (OS_INCL | tag);
+#pragma unroll
+        for (int j = 0; j < OS_LOOK; ++j) {
+          if (done) break;
+          unsigned long long x = v[j];
+          while ((x & 0x3fffffff00000000ull) != tag || (x >> 62) == 0ull) x = ld_status(status + (size_t)(q - j) * RADIX + d);
+          excl += (unsigned)x;
+          done = (x >> 62) == 2ull;
+        }
       }
     }
     st_status(mine, OS_INCL | tag | (unsigned long long)(excl + run));
