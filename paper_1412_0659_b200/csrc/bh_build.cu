@@ -582,15 +582,15 @@ __global__ void __launch_bounds__(256) groups_kernel(const float4 *__restrict__ 
 // which are one level deeper and already done).  FP64 accumulation in slot order, one rounding to
 // FP32 per stored value (S13).  Q = sum m d d^T about the FP32-rounded centre of mass (S4).
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) moments_level_kernel(int c0, int c1, int level, const DevInfo *__restrict__ info,
-                                                            const float4 *__restrict__ spos,
-                                                            const uint2 *__restrict__ c_link,
-                                                            const uint32_t *__restrict__ c_first,
-                                                            uint32_t *__restrict__ c_count, float4 *__restrict__ c_cm,
-                                                            float4 *__restrict__ c_qa, float4 *__restrict__ c_qb) {
-  int c = c0 + blockIdx.x * blockDim.x + threadIdx.x;
-  if (c >= c1) return;
+// One cell. `leaves` selects which kind of cell this call handles: leaves depend on the particles only and
+// are all done by one launch; internal cells follow level by level, deepest first.
+__device__ __forceinline__ void moments_cell(int c, int level, bool leaves, const DevInfo *__restrict__ info,
+                                             const float4 *__restrict__ spos, const uint2 *__restrict__ c_link,
+                                             const uint32_t *__restrict__ c_first, uint32_t *__restrict__ c_count,
+                                             float4 *__restrict__ c_cm, float4 *__restrict__ c_qa,
+                                             float4 *__restrict__ c_qb) {
   const uint2 lk = c_link[c];
+  if (leaves != !(lk.y & LEAF_FLAG)) return;
   double M = 0, s0 = 0, s1 = 0, s2 = 0;
   double Q0 = 0, Q1 = 0, Q2 = 0, Q3 = 0, Q4 = 0, Q5 = 0;
   float cx, cy, cz;
@@ -661,9 +661,50 @@ __global__ void __launch_bounds__(128) moments_level_kernel(int c0, int c1, int 
   c_qb[c] = make_float4((float)Q3, (float)Q4, (float)Q5, __fadd_rn(__fadd_rn(q0, q1), q2));
 }
 
+// all leaves, any level (the level of a cell comes from c_level)
+__global__ void __launch_bounds__(128) moments_leaf_kernel(int n_cells, const DevInfo *__restrict__ info,
+                                                           const float4 *__restrict__ spos, const uint2 *__restrict__ c_link,
+                                                           const uint8_t *__restrict__ c_level,
+                                                           const uint32_t *__restrict__ c_first,
+                                                           uint32_t *__restrict__ c_count, float4 *__restrict__ c_cm,
+                                                           float4 *__restrict__ c_qa, float4 *__restrict__ c_qb) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= n_cells) return;
+  moments_cell(c, (int)c_level[c], true, info, spos, c_link, c_first, c_count, c_cm, c_qa, c_qb);
+}
+
+// internal cells of one level [c0, c1)
+__global__ void __launch_bounds__(128) moments_level_kernel(int c0, int c1, int level, const DevInfo *__restrict__ info,
+                                                            const float4 *__restrict__ spos,
+                                                            const uint2 *__restrict__ c_link,
+                                                            const uint32_t *__restrict__ c_first,
+                                                            uint32_t *__restrict__ c_count, float4 *__restrict__ c_cm,
+                                                            float4 *__restrict__ c_qa, float4 *__restrict__ c_qb) {
+  const int c = c0 + blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= c1) return;
+  moments_cell(c, level, false, info, spos, c_link, c_first, c_count, c_cm, c_qa, c_qb);
+}
+
+// internal cells of the top levels ltop .. 0 (few cells): one block, a block barrier between levels
+__global__ void __launch_bounds__(256) moments_top_kernel(int ltop, const DevInfo *__restrict__ info,
+                                                          const float4 *__restrict__ spos, const uint2 *__restrict__ c_link,
+                                                          const uint32_t *__restrict__ c_first,
+                                                          uint32_t *__restrict__ c_count, float4 *__restrict__ c_cm,
+                                                          float4 *__restrict__ c_qa, float4 *__restrict__ c_qb) {
+  for (int l = ltop; l >= 0; --l) {
+    const int c0 = info->level_off[l], c1 = info->level_off[l + 1];
+    for (int c = c0 + threadIdx.x; c < c1; c += blockDim.x)
+      moments_cell(c, l, false, info, spos, c_link, c_first, c_count, c_cm, c_qa, c_qb);
+    __threadfence();
+    __syncthreads();
+  }
+}
+
 // ------------------------------------------------------------------------------------------
 // host launchers
 // ------------------------------------------------------------------------------------------
+constexpr int MOMENTS_TOP_CELLS = 2048;
+
 static inline int grid_for(tree_ctx *t, long long n, int threads, int per_sm) {
   long long need = (n + threads - 1) / threads;
   long long cap = (long long)t->sm_count * per_sm;
@@ -765,13 +806,24 @@ int run_groups_moments(tree_ctx *t) {
   groups_kernel<<<(unsigned)((thr + 255) / 256), 256, 0, t->stream>>>(t->b.spos, t->N, t->group, t->n_groups, t->b.gbox);
   BH_LAUNCH_CHECK("groups");
   const int *off = t->h_info->level_off;
-  for (int l = MAX_LEVEL; l >= 0; --l) {
+  const int nc = (int)t->n_cells;
+  moments_leaf_kernel<<<(nc + 127) / 128, 128, 0, t->stream>>>(nc, t->d_info, t->b.spos, t->b.c_link, t->b.c_level,
+                                                               t->b.c_first, t->b.c_count, t->b.c_cm, t->b.c_qa, t->b.c_qb);
+  BH_LAUNCH_CHECK("moments_leaf");
+  int ltop = -1;  // levels 0..ltop together hold at most MOMENTS_TOP_CELLS cells: one block does them
+  while (ltop + 1 <= MAX_LEVEL && off[ltop + 2] <= MOMENTS_TOP_CELLS) ++ltop;
+  for (int l = MAX_LEVEL; l > ltop; --l) {
     int c0 = off[l], c1 = off[l + 1];
     if (c1 <= c0) continue;
     moments_level_kernel<<<(c1 - c0 + 127) / 128, 128, 0, t->stream>>>(c0, c1, l, t->d_info, t->b.spos, t->b.c_link,
                                                                        t->b.c_first, t->b.c_count, t->b.c_cm, t->b.c_qa,
                                                                        t->b.c_qb);
     BH_LAUNCH_CHECK("moments_level");
+  }
+  if (ltop >= 0) {
+    moments_top_kernel<<<1, 256, 0, t->stream>>>(ltop, t->d_info, t->b.spos, t->b.c_link, t->b.c_first, t->b.c_count,
+                                                 t->b.c_cm, t->b.c_qa, t->b.c_qb);
+    BH_LAUNCH_CHECK("moments_top");
   }
   return 0;
 }
