@@ -135,6 +135,57 @@ int tree_get_debug(tree_ctx *t, int what, void *dst, long long *count);
 #define TREE_NPHASE 11
 int tree_get_stats(tree_ctx *t, double *ms, unsigned long long *n_pp, unsigned long long *n_pc);
 
+/* ---- sharded force pass over several GPUs of one NVLink / NVSwitch node ------------------------
+ * PAPER.md section III-B (L81-125) cuts the Peano-Hilbert curve into one piece per GPU (L93-97),
+ * balances the pieces by the flops of the tree-walk (L107) and exchanges pruned trees over MPI
+ * (L111-119) because node memory and network were the limits of 2014.  Here every
+ * context of a node holds ALL N particles and builds the same tree (the build is ~3 % of a step on
+ * this hardware); what is cut is the force pass: `world` contexts (one per GPU, one process each, or
+ * several in one process) share one pass, context `rank` walking one contiguous range of groups of
+ * the PH-sorted order with ~1/world of the estimated walk cost, and the walk kernel stores each
+ * group's accelerations, potentials and interaction counts straight into the result buffers of
+ * every attached context over NVLink (peer stores): there is no separate collective.  The one
+ * exchange step is a barrier between the two halves of the pass, which the CALLER provides
+ * (e.g. one NCCL all-reduce on the contexts' streams; the binding's ShardedTree does that):
+ *     tree_force_begin on every context  ->  barrier  ->  tree_force_end on every context.
+ * Results are those of the same pass on one context up to the order of a few partial sums (the task
+ * list differs); interaction counts per group are identical.
+ *
+ * Set-up, once, in this order: tree_reserve (buffers for the largest N) -> tree_shard_config ->
+ * tree_shard_export / exchange the blobs / tree_shard_attach for every other rank (or
+ * tree_shard_attach_local for contexts of the same process).  With world > 1, tree_force and
+ * tree_leapfrog return TREE_ERR_ORDER (they cannot contain the barrier) and a tree_build beyond the
+ * reserved capacity returns TREE_ERR_ORDER (it would invalidate the exported buffers). */
+#define TREE_SHARD_MAX_WORLD 16
+#define TREE_SHARD_HANDLE_BYTES 128
+
+/* Allocate the particle-sized buffers for up to N particles now (they are otherwise grown by
+ * tree_build). */
+int tree_reserve(tree_ctx *t, long long N);
+/* This context is `rank` of `world` (1 <= world <= TREE_SHARD_MAX_WORLD); world = 1 undoes it. */
+int tree_shard_config(tree_ctx *t, int rank, int world);
+/* Write this context's result-buffer handle (a CUDA IPC handle and the reserved sizes) to
+ * HOST memory handle[TREE_SHARD_HANDLE_BYTES].  Needs tree_reserve. */
+int tree_shard_export(tree_ctx *t, void *handle);
+/* Map the result buffers of context `peer_rank` living in ANOTHER process from its exported
+ * HOST blob (cudaIpcOpenMemHandle; the GPUs must be peer-capable).  The peer must have reserved
+ * the same N with the same group size. */
+int tree_shard_attach(tree_ctx *t, int peer_rank, const void *handle);
+/* Same for a context of THIS process (any device; peer access is enabled if needed). */
+int tree_shard_attach_local(tree_ctx *t, int peer_rank, tree_ctx *peer);
+/* First half of tree_force: opening radii, cost estimate, partition, task list, fused walk+force
+ * over this context's range, results stored into every attached context.  Asynchronous. */
+int tree_force_begin(tree_ctx *t, float theta, float eps);
+/* Second half, after the caller's barrier: results to caller order (acc, pot as in tree_force). */
+int tree_force_end(tree_ctx *t, float *acc, float *pot);
+/* tree_leapfrog in two halves around the same barrier: kick, drift, rebuild, tree_force_begin |
+ * tree_force_end, kick. */
+int tree_leapfrog_begin(tree_ctx *t, float dt);
+int tree_leapfrog_end(tree_ctx *t);
+/* The range of groups [*g_lo, *g_hi) and of slots [*s_lo, *s_hi) this context walked in the last
+ * pass, to HOST memory (any pointer may be NULL).  Synchronises. */
+int tree_shard_range(tree_ctx *t, long long *g_lo, long long *g_hi, long long *s_lo, long long *s_hi);
+
 /* Number of kernels this library launched on the context since tree_create (for accounting). */
 long long tree_launch_count(const tree_ctx *t);
 

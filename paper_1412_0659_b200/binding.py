@@ -17,6 +17,8 @@ _lib = None
 # Flop convention of PAPER.md L190-192: 23 per particle-particle, 65 per particle-cell interaction.
 FLOP_PP = 23
 FLOP_PC = 65
+SHARD_MAX_WORLD = 16
+SHARD_HANDLE_BYTES = 128
 
 PHASES = ("keys", "sort", "permute", "build", "moments", "opening", "walk", "unpermute", "integrate", "sched", "total")
 
@@ -37,6 +39,16 @@ _SIGS = {
     "tree_energy": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     "tree_get_debug": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.POINTER(C.c_longlong)]),
     "tree_get_stats": (C.c_int, [C.c_void_p, C.c_void_p, C.POINTER(C.c_ulonglong), C.POINTER(C.c_ulonglong)]),
+    "tree_reserve": (C.c_int, [C.c_void_p, C.c_longlong]),
+    "tree_shard_config": (C.c_int, [C.c_void_p, C.c_int, C.c_int]),
+    "tree_shard_export": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "tree_shard_attach": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
+    "tree_shard_attach_local": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p]),
+    "tree_force_begin": (C.c_int, [C.c_void_p, C.c_float, C.c_float]),
+    "tree_force_end": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "tree_leapfrog_begin": (C.c_int, [C.c_void_p, C.c_float]),
+    "tree_leapfrog_end": (C.c_int, [C.c_void_p]),
+    "tree_shard_range": (C.c_int, [C.c_void_p] + [C.POINTER(C.c_longlong)] * 4),
     "tree_launch_count": (C.c_longlong, [C.c_void_p]),
     "tree_last_error": (C.c_char_p, [C.c_void_p]),
 }
@@ -163,6 +175,44 @@ class Tree:
 
     def leapfrog(self, dt: float):
         tree_leapfrog(self.h, dt)
+
+    # -- sharded force pass (include/tree.h "sharded force pass"); ShardedTree in sharded.py drives these
+    def reserve(self, n: int):
+        _check(self.h, load_library().tree_reserve(self.h, int(n)))
+
+    def shard_config(self, rank: int, world: int):
+        _check(self.h, load_library().tree_shard_config(self.h, int(rank), int(world)))
+
+    def shard_export(self) -> bytes:
+        buf = C.create_string_buffer(SHARD_HANDLE_BYTES)
+        _check(self.h, load_library().tree_shard_export(self.h, buf))
+        return buf.raw
+
+    def shard_attach(self, peer_rank: int, handle: bytes):
+        assert len(handle) == SHARD_HANDLE_BYTES
+        buf = C.create_string_buffer(handle, SHARD_HANDLE_BYTES)
+        _check(self.h, load_library().tree_shard_attach(self.h, int(peer_rank), buf))
+
+    def shard_attach_local(self, peer_rank: int, peer: "Tree"):
+        _check(self.h, load_library().tree_shard_attach_local(self.h, int(peer_rank), peer.h))
+
+    def force_begin(self, theta: float, eps: float):
+        _check(self.h, load_library().tree_force_begin(self.h, float(theta), float(eps)))
+
+    def force_end(self, acc=None, pot=None):
+        _check(self.h, load_library().tree_force_end(self.h, _ptr(acc), _ptr(pot)))
+
+    def leapfrog_begin(self, dt: float):
+        _check(self.h, load_library().tree_leapfrog_begin(self.h, float(dt)))
+
+    def leapfrog_end(self):
+        _check(self.h, load_library().tree_leapfrog_end(self.h))
+
+    def shard_range(self):
+        """(g_lo, g_hi, slot_lo, slot_hi) of the last pass on this context."""
+        v = [C.c_longlong(0) for _ in range(4)]
+        _check(self.h, load_library().tree_shard_range(self.h, *[C.byref(x) for x in v]))
+        return tuple(int(x.value) for x in v)
 
     def set_velocity(self, vel):
         assert vel.is_cuda and vel.numel() == 3 * self.n

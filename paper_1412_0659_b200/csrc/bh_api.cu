@@ -31,20 +31,47 @@ static int dev_alloc(tree_ctx *t, T *&p, long long n) {
 
 #define BH_TRY(x) do { int _rc = (x); if (_rc) return _rc; } while (0)
 
+static size_t slab_bytes(long long cap, long long ng) { return 2 * (size_t)cap * sizeof(float4) + 2 * (size_t)ng * sizeof(uint2); }
+
+// result buffers inside a slab of `t`'s reserved sizes (the local one or a mapped peer's)
+void shard_views(const tree_ctx *t, void *base, int parity, float4 **sacc, uint2 **gcount) {
+  const long long ng = (t->cap + t->group - 1) / t->group;
+  char *p = (char *)base;
+  *sacc = (float4 *)(p + (size_t)parity * (size_t)t->cap * sizeof(float4));
+  *gcount = (uint2 *)(p + 2 * (size_t)t->cap * sizeof(float4) + (size_t)parity * (size_t)ng * sizeof(uint2));
+}
+
+static void detach_peers(tree_ctx *t) {
+  for (int r = 0; r < TREE_SHARD_MAX_WORLD; ++r) {
+    if (t->peer_base[r] && t->peer_ipc[r]) cudaIpcCloseMemHandle(t->peer_base[r]);
+    t->peer_base[r] = nullptr;
+    t->peer_ipc[r] = false;
+  }
+  cudaGetLastError();
+}
+
 static int ensure_particles(tree_ctx *t, long long N) {
   if (N <= t->cap) return 0;
+  if (t->shard_world > 1 && t->cap > 0)
+    return set_err(t, TREE_ERR_ORDER, "sharded context: N exceeds the capacity given to tree_reserve");
   long long cap = N;
   Buffers &b = t->b;
+  t->cap = 0;
   BH_TRY(dev_alloc(t, b.posm, cap));
   BH_TRY(dev_alloc(t, b.vel, cap));
   BH_TRY(dev_alloc(t, b.acc, cap));
   for (int k = 0; k < 2; ++k) { BH_TRY(dev_alloc(t, b.key[k], cap)); BH_TRY(dev_alloc(t, b.idx[k], cap)); }
   BH_TRY(dev_alloc(t, b.spos, cap));
-  BH_TRY(dev_alloc(t, b.sacc, cap));
   BH_TRY(dev_alloc(t, b.lv, cap));
   long long ng = (cap + t->group - 1) / t->group;
   BH_TRY(dev_alloc(t, b.gbox, 6 * ng));
-  BH_TRY(dev_alloc(t, b.gcount, ng));
+  {
+    char *slab = (char *)b.shard_slab;
+    BH_TRY(dev_alloc(t, slab, (long long)slab_bytes(cap, ng)));
+    b.shard_slab = slab;
+    BH_CUDA(cudaMemsetAsync(slab, 0, slab_bytes(cap, ng), t->stream));
+  }
+  BH_TRY(dev_alloc(t, b.gcost, ng));
   if (ng >= (1ll << 26)) return set_err(t, TREE_ERR_ARG, "too many groups (needs < 2^26)");
   t->head_cap = ng / 8 + 1024;
   t->tail_cap = 4ll * 2 * t->sm_count * 16;  // 4 parts x (2 x resident warps) groups
@@ -68,6 +95,9 @@ static int ensure_particles(tree_ctx *t, long long N) {
   BH_CUDA(cudaMemsetAsync(b.sort_status, 0, (size_t)t->sort_status_cap * sizeof(unsigned long long), t->stream));
   t->sort_epoch = 0;
   t->cap = cap;
+  for (int k = 0; k < 2; ++k) shard_views(t, b.shard_slab, k, &b.sacc2[k], &b.gcount2[k]);
+  b.sacc = b.sacc2[t->pass & 1];
+  b.gcount = b.gcount2[t->pass & 1];
   t->have_vel = false;
   t->have_force = false;
   t->built = false;
@@ -92,9 +122,10 @@ int ensure_cells(tree_ctx *t, long long nc) {
 }
 
 static void free_all(tree_ctx *t) {
+  detach_peers(t);
   Buffers &b = t->b;
-  void *ptrs[] = {b.posm, b.vel, b.acc, b.key[0], b.key[1], b.idx[0], b.idx[1], b.scan_tmp, b.scan_blk, b.sort_hist, b.sort_status, b.spos, b.sacc,
-                  b.lv, b.gbox, b.gcount, b.sched_a, b.sched_b, b.gdone, b.gparts, b.gthresh, b.tasks, b.part, b.trace, b.c_level, b.c_first, b.c_count, b.c_fcall, b.c_link, b.c_cm, b.c_qa, b.c_qb,
+  void *ptrs[] = {b.posm, b.vel, b.acc, b.key[0], b.key[1], b.idx[0], b.idx[1], b.scan_tmp, b.scan_blk, b.sort_hist, b.sort_status, b.spos, b.shard_slab, b.gcost,
+                  b.lv, b.gbox, b.sched_a, b.sched_b, b.gdone, b.gparts, b.gthresh, b.tasks, b.part, b.trace, b.c_level, b.c_first, b.c_count, b.c_fcall, b.c_link, b.c_cm, b.c_qa, b.c_qb,
                   b.c_test, b.in_pos, b.in_mass, b.out_acc, b.out_pot};
   for (void *p : ptrs) if (p) cudaFree(p);
   b = Buffers();
@@ -117,14 +148,63 @@ static int build_from_posm(tree_ctx *t) {
   return 0;
 }
 
-static int force_impl(tree_ctx *t, float theta, float eps, float *acc, float *pot) {
+// First half of a force pass: everything up to and including the fused walk + force kernel.  The pass
+// writes into the result buffers of parity (pass & 1); the other parity still holds the previous pass
+// (its per-group counts schedule this one, and a sharded peer may still be reading it).
+static int force_begin_impl(tree_ctx *t, float theta, float eps) {
+  if (t->shard_world > 1)
+    for (int r = 0; r < t->shard_world; ++r)
+      if (r != t->shard_rank && !t->peer_base[r]) return set_err(t, TREE_ERR_ORDER, "sharded context: a peer is not attached");
+  t->pass++;
+  t->b.sacc = t->b.sacc2[t->pass & 1];
+  t->b.gcount = t->b.gcount2[t->pass & 1];
   rec(t, EV_F0);
   BH_TRY(run_opening(t, theta));
   BH_TRY(run_walk(t, eps));  // records EV_OPEN before and EV_WALK after the walk kernel
+  t->theta = theta; t->eps = eps;
+  t->have_force = false;
+  t->force_open = true;
+  return 0;
+}
+
+// Second half: results to caller order (in a sharded pass, after the caller's barrier).
+static int force_end_impl(tree_ctx *t, float *acc, float *pot) {
   BH_TRY(run_unpermute(t, acc, pot));
   rec(t, EV_UNPERM);
-  t->theta = theta; t->eps = eps;
+  t->force_open = false;
   t->have_force = true;
+  return 0;
+}
+
+static int force_impl(tree_ctx *t, float theta, float eps, float *acc, float *pot) {
+  BH_TRY(force_begin_impl(t, theta, eps));
+  return force_end_impl(t, acc, pot);
+}
+
+static int leapfrog_begin_impl(tree_ctx *t, float dt) {
+  rec(t, EV_I0);
+  BH_TRY(run_kick_drift(t, dt));
+  rec(t, EV_I1);
+  t->built = false;
+  t->have_force = false;
+  rec(t, EV_B0);
+  BH_TRY(run_bbox_only(t));
+  BH_TRY(build_from_posm(t));
+  t->reuse_costs = true;  // same particles one step later: last pass's counts predict this pass's costs
+  const int frc = force_begin_impl(t, t->theta, t->eps);
+  t->reuse_costs = false;
+  if (frc) return frc;
+  t->step_open = true;
+  t->step_dt = dt;
+  return 0;
+}
+
+static int leapfrog_end_impl(tree_ctx *t) {
+  BH_TRY(force_end_impl(t, nullptr, nullptr));
+  rec(t, EV_I2);
+  BH_TRY(run_kick(t, t->step_dt));
+  rec(t, EV_I3);
+  t->step_open = false;
   return 0;
 }
 
@@ -187,6 +267,7 @@ int tree_build(tree_ctx *t, const float *pos, const float *mass, long long N) {
   if (!t) return TREE_ERR_ARG;
   if (!pos || !mass || N <= 0 || N > 2147483647LL) return set_err(t, TREE_ERR_ARG, "tree_build: bad argument");
   BH_CUDA(cudaSetDevice(t->device));
+  if (t->force_open || t->step_open) return set_err(t, TREE_ERR_ORDER, "tree_build inside an open force pass");
   t->built = false;
   t->have_force = false;
   if (N != t->N) t->have_vel = false;
@@ -203,31 +284,162 @@ int tree_force(tree_ctx *t, float theta, float eps, float *acc, float *pot) {
   if (!(theta >= 0.0f) || !(eps >= 0.0f) || !isfinite(theta) || !isfinite(eps))
     return set_err(t, TREE_ERR_ARG, "tree_force: theta and eps must be finite and >= 0");
   if (!t->built) return set_err(t, TREE_ERR_ORDER, "tree_force before tree_build");
+  if (t->force_open || t->step_open) return set_err(t, TREE_ERR_ORDER, "tree_force inside an open force pass");
+  if (t->shard_world > 1) return set_err(t, TREE_ERR_ORDER, "sharded context: use tree_force_begin / barrier / tree_force_end");
   BH_CUDA(cudaSetDevice(t->device));
   return force_impl(t, theta, eps, acc, pot);
 }
 
-int tree_leapfrog(tree_ctx *t, float dt) {
-  if (!t) return TREE_ERR_ARG;
+static int leapfrog_check(tree_ctx *t, float dt) {
   if (!isfinite(dt)) return set_err(t, TREE_ERR_ARG, "tree_leapfrog: dt not finite");
+  if (t->force_open || t->step_open) return set_err(t, TREE_ERR_ORDER, "tree_leapfrog inside an open force pass");
   if (!t->built || !t->have_force) return set_err(t, TREE_ERR_ORDER, "tree_leapfrog before tree_build + tree_force");
   if (!t->have_vel) return set_err(t, TREE_ERR_ORDER, "tree_leapfrog before tree_set_velocity");
+  return 0;
+}
+
+int tree_leapfrog(tree_ctx *t, float dt) {
+  if (!t) return TREE_ERR_ARG;
+  BH_TRY(leapfrog_check(t, dt));
+  if (t->shard_world > 1) return set_err(t, TREE_ERR_ORDER, "sharded context: use tree_leapfrog_begin / barrier / tree_leapfrog_end");
   BH_CUDA(cudaSetDevice(t->device));
-  rec(t, EV_I0);
-  BH_TRY(run_kick_drift(t, dt));
-  rec(t, EV_I1);
-  t->built = false;
-  t->have_force = false;
-  rec(t, EV_B0);
-  BH_TRY(run_bbox_only(t));
-  BH_TRY(build_from_posm(t));
-  t->reuse_costs = true;  // same particles one step later: last pass's counts predict this pass's costs
-  const int frc = force_impl(t, t->theta, t->eps, nullptr, nullptr);
-  t->reuse_costs = false;
-  if (frc) return frc;
-  rec(t, EV_I2);
-  BH_TRY(run_kick(t, dt));
-  rec(t, EV_I3);
+  BH_TRY(leapfrog_begin_impl(t, dt));
+  return leapfrog_end_impl(t);
+}
+
+int tree_leapfrog_begin(tree_ctx *t, float dt) {
+  if (!t) return TREE_ERR_ARG;
+  BH_TRY(leapfrog_check(t, dt));
+  BH_CUDA(cudaSetDevice(t->device));
+  return leapfrog_begin_impl(t, dt);
+}
+
+int tree_leapfrog_end(tree_ctx *t) {
+  if (!t) return TREE_ERR_ARG;
+  if (!t->step_open) return set_err(t, TREE_ERR_ORDER, "tree_leapfrog_end without tree_leapfrog_begin");
+  BH_CUDA(cudaSetDevice(t->device));
+  return leapfrog_end_impl(t);
+}
+
+static int force_check(tree_ctx *t, float theta, float eps) {
+  if (!(theta >= 0.0f) || !(eps >= 0.0f) || !isfinite(theta) || !isfinite(eps))
+    return set_err(t, TREE_ERR_ARG, "tree_force: theta and eps must be finite and >= 0");
+  if (!t->built) return set_err(t, TREE_ERR_ORDER, "tree_force before tree_build");
+  if (t->force_open || t->step_open) return set_err(t, TREE_ERR_ORDER, "tree_force inside an open force pass");
+  return 0;
+}
+
+int tree_force_begin(tree_ctx *t, float theta, float eps) {
+  if (!t) return TREE_ERR_ARG;
+  BH_TRY(force_check(t, theta, eps));
+  BH_CUDA(cudaSetDevice(t->device));
+  return force_begin_impl(t, theta, eps);
+}
+
+int tree_force_end(tree_ctx *t, float *acc, float *pot) {
+  if (!t) return TREE_ERR_ARG;
+  if (!t->force_open || t->step_open) return set_err(t, TREE_ERR_ORDER, "tree_force_end without tree_force_begin");
+  BH_CUDA(cudaSetDevice(t->device));
+  return force_end_impl(t, acc, pot);
+}
+
+int tree_reserve(tree_ctx *t, long long N) {
+  if (!t) return TREE_ERR_ARG;
+  if (N <= 0 || N > 2147483647LL) return set_err(t, TREE_ERR_ARG, "tree_reserve: bad N");
+  BH_CUDA(cudaSetDevice(t->device));
+  return ensure_particles(t, N);
+}
+
+int tree_shard_config(tree_ctx *t, int rank, int world) {
+  if (!t) return TREE_ERR_ARG;
+  if (world < 1 || world > TREE_SHARD_MAX_WORLD || rank < 0 || rank >= world)
+    return set_err(t, TREE_ERR_ARG, "tree_shard_config: need 0 <= rank < world <= TREE_SHARD_MAX_WORLD");
+  if (t->force_open || t->step_open) return set_err(t, TREE_ERR_ORDER, "tree_shard_config inside an open force pass");
+  if (world > 1 && t->cap <= 0) return set_err(t, TREE_ERR_ORDER, "tree_shard_config before tree_reserve");
+  BH_CUDA(cudaSetDevice(t->device));
+  BH_CUDA(cudaStreamSynchronize(t->stream));
+  if (world != t->shard_world || rank != t->shard_rank) detach_peers(t);
+  t->shard_rank = rank;
+  t->shard_world = world;
+  return TREE_OK;
+}
+
+namespace {
+struct ShardBlob {  // TREE_SHARD_HANDLE_BYTES
+  cudaIpcMemHandle_t ipc;
+  long long cap;
+  int group, device;
+  char pad[TREE_SHARD_HANDLE_BYTES - sizeof(cudaIpcMemHandle_t) - sizeof(long long) - 2 * sizeof(int)];
+};
+static_assert(sizeof(ShardBlob) == TREE_SHARD_HANDLE_BYTES, "blob size");
+}  // namespace
+
+int tree_shard_export(tree_ctx *t, void *handle) {
+  if (!t) return TREE_ERR_ARG;
+  if (!handle) return set_err(t, TREE_ERR_ARG, "tree_shard_export: NULL");
+  if (t->cap <= 0 || !t->b.shard_slab) return set_err(t, TREE_ERR_ORDER, "tree_shard_export before tree_reserve");
+  BH_CUDA(cudaSetDevice(t->device));
+  ShardBlob blob;
+  memset(&blob, 0, sizeof(blob));
+  BH_CUDA(cudaIpcGetMemHandle(&blob.ipc, t->b.shard_slab));
+  blob.cap = t->cap; blob.group = t->group; blob.device = t->device;
+  memcpy(handle, &blob, sizeof(blob));
+  return TREE_OK;
+}
+
+static int attach_check(tree_ctx *t, int peer_rank, long long cap, int group) {
+  if (t->shard_world <= 1) return set_err(t, TREE_ERR_ORDER, "tree_shard_attach before tree_shard_config");
+  if (peer_rank < 0 || peer_rank >= t->shard_world || peer_rank == t->shard_rank)
+    return set_err(t, TREE_ERR_ARG, "tree_shard_attach: bad peer rank");
+  if (cap != t->cap || group != t->group)
+    return set_err(t, TREE_ERR_ARG, "tree_shard_attach: the peer reserved a different N or group size");
+  if (t->peer_base[peer_rank]) return set_err(t, TREE_ERR_ORDER, "tree_shard_attach: peer already attached");
+  return 0;
+}
+
+int tree_shard_attach(tree_ctx *t, int peer_rank, const void *handle) {
+  if (!t) return TREE_ERR_ARG;
+  if (!handle) return set_err(t, TREE_ERR_ARG, "tree_shard_attach: NULL");
+  ShardBlob blob;
+  memcpy(&blob, handle, sizeof(blob));
+  BH_TRY(attach_check(t, peer_rank, blob.cap, blob.group));
+  BH_CUDA(cudaSetDevice(t->device));
+  void *base = nullptr;
+  BH_CUDA(cudaIpcOpenMemHandle(&base, blob.ipc, cudaIpcMemLazyEnablePeerAccess));
+  t->peer_base[peer_rank] = base;
+  t->peer_ipc[peer_rank] = true;
+  return TREE_OK;
+}
+
+int tree_shard_attach_local(tree_ctx *t, int peer_rank, tree_ctx *peer) {
+  if (!t) return TREE_ERR_ARG;
+  if (!peer || peer == t || !peer->b.shard_slab) return set_err(t, TREE_ERR_ARG, "tree_shard_attach_local: bad peer");
+  BH_TRY(attach_check(t, peer_rank, peer->cap, peer->group));
+  BH_CUDA(cudaSetDevice(t->device));
+  if (peer->device != t->device) {
+    int can = 0;
+    BH_CUDA(cudaDeviceCanAccessPeer(&can, t->device, peer->device));
+    if (!can) return set_err(t, TREE_ERR_CUDA, "tree_shard_attach_local: devices are not peer-capable");
+    cudaError_t e = cudaDeviceEnablePeerAccess(peer->device, 0);
+    if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled) return set_err(t, TREE_ERR_CUDA, "cudaDeviceEnablePeerAccess", e);
+    cudaGetLastError();
+  }
+  t->peer_base[peer_rank] = peer->b.shard_slab;
+  t->peer_ipc[peer_rank] = false;
+  return TREE_OK;
+}
+
+int tree_shard_range(tree_ctx *t, long long *g_lo, long long *g_hi, long long *s_lo, long long *s_hi) {
+  if (!t) return TREE_ERR_ARG;
+  if (!t->have_force && !t->force_open) return set_err(t, TREE_ERR_ORDER, "tree_shard_range before a force pass");
+  BH_CUDA(cudaSetDevice(t->device));
+  BH_CUDA(cudaMemcpyAsync(t->h_info, t->d_info, sizeof(DevInfo), cudaMemcpyDeviceToHost, t->stream));
+  BH_CUDA(cudaStreamSynchronize(t->stream));
+  const long long lo = t->h_info->g_lo, hi = t->h_info->g_hi;
+  if (g_lo) *g_lo = lo;
+  if (g_hi) *g_hi = hi;
+  if (s_lo) *s_lo = lo * t->group < t->N ? lo * t->group : t->N;
+  if (s_hi) *s_hi = hi * t->group < t->N ? hi * t->group : t->N;
   return TREE_OK;
 }
 

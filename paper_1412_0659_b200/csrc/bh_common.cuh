@@ -32,6 +32,7 @@ struct DevInfo {
   unsigned int tail_start;          // first task of the tail region (last groups, split into small tasks)
   unsigned int walk_overflow;       // set if a warp's walk stack would have overflowed (results invalid)
   unsigned int sched_tot[2];      // totals of the two scheduling scans
+  unsigned int g_lo, g_hi;        // groups this context walks in the current force pass (all of them unless sharded)
   double ekin, epot;
 };
 
@@ -49,11 +50,15 @@ struct Buffers {
   uint32_t *scan_blk = nullptr;  // block sums for the device-wide scan
   // slot (sorted) order
   float4 *spos = nullptr;
-  float4 *sacc = nullptr;
+  void *shard_slab = nullptr;  // one allocation (one IPC handle): sacc2[0] | sacc2[1] | gcount2[0] | gcount2[1]
+  float4 *sacc2[2] = {nullptr, nullptr};  // results in slot order, double-buffered by force pass
+  float4 *sacc = nullptr;                 // = sacc2[pass & 1], the buffer of the current / last force pass
   uint16_t *lv = nullptr;   // per slot: L0 | Lleaf << 5
   // groups
   float *gbox = nullptr;    // [n_groups][6]
-  uint2 *gcount = nullptr;  // [n_groups] n_pp, n_pc
+  uint2 *gcount2[2] = {nullptr, nullptr};  // [n_groups] n_pp, n_pc, double-buffered like sacc2
+  uint2 *gcount = nullptr;                 // = gcount2[pass & 1]
+  double *gcost = nullptr;  // [n_groups] cost estimate of the current pass (task list and shard partition)
   // scheduling of the force walk
   uint32_t *sched_a = nullptr, *sched_b = nullptr;  // [n_groups] part counts -> offsets (scanned in place)
   uint32_t *gdone = nullptr;   // [n_groups]
@@ -92,6 +97,16 @@ struct tree_ctx {
   long long staging_cap = 0;         // capacity of the host-call staging buffers
   float theta = 0.f, eps = 0.f;
   bool reuse_costs = false;          // this force pass may schedule by the previous pass's per-group counts
+  // sharded force pass: this context walks one contiguous cost-balanced range of groups and
+  // stores the results into every attached context's result buffers
+  int shard_rank = 0, shard_world = 1;
+  unsigned pass = 0;                 // force passes begun; parity selects the result buffers
+  bool force_open = false;           // between tree_force_begin and tree_force_end
+  bool step_open = false;            // between tree_leapfrog_begin and tree_leapfrog_end
+  float step_dt = 0.f;
+  float *open_acc = nullptr, *open_pot = nullptr;
+  void *peer_base[TREE_SHARD_MAX_WORLD] = {};   // mapped result slab of each attached peer (nullptr: not attached)
+  bool peer_ipc[TREE_SHARD_MAX_WORLD] = {};     // mapping came from cudaIpcOpenMemHandle (to be closed)
   int sm_count = 148;
   bh::Buffers b;
   bh::DevInfo *d_info = nullptr;
@@ -135,6 +150,7 @@ int run_tree(tree_ctx *t);      // octree construction; synchronises once (cell 
 int run_groups_moments(tree_ctx *t);
 int run_opening(tree_ctx *t, float theta);
 int run_walk(tree_ctx *t, float eps);
+void shard_views(const tree_ctx *t, void *base, int parity, float4 **sacc, uint2 **gcount);
 int run_unpermute(tree_ctx *t, float *acc, float *pot);
 int run_kick_drift(tree_ctx *t, float dt);
 int run_kick(tree_ctx *t, float dt);

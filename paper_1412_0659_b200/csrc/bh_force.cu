@@ -81,8 +81,11 @@ struct WalkParams {
   const uint2 *c_link;
   const float4 *c_cm, *c_qa, *c_qb;
   const float *gbox;
-  float4 *sacc;
-  uint2 *gcount;
+  float4 *sacc;            // this context's result buffer of the current pass
+  uint2 *gcount;           // this context's per-group counts of the current pass
+  float4 *peer_sacc[TREE_SHARD_MAX_WORLD];   // sharded pass: the same two buffers of every attached context
+  uint2 *peer_gcount[TREE_SHARD_MAX_WORLD];  // (peer stores over NVLink); n_peers = 0 otherwise
+  int n_peers;
   DevInfo *info;
   const uint32_t *c_count; // particles per cell (counting walk only)
   const uint32_t *tasks;   // task = group | part << TASK_GROUP_BITS
@@ -507,6 +510,7 @@ __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, con
   if (lane == 0) {
     if (nparts == 1) {
       P.gcount[g] = make_uint2(n_pp, n_pc);
+      for (int q = 0; q < P.n_peers; ++q) P.peer_gcount[q][g] = make_uint2(n_pp, n_pc);
     } else {  // gcount of split groups is zeroed by task_class_kernel
       atomicAdd(&P.gcount[g].x, n_pp);
       atomicAdd(&P.gcount[g].y, n_pc);
@@ -529,7 +533,10 @@ __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, con
 #pragma unroll
     for (int t = 0; t < TPL; ++t) {
       unsigned j = lane + 32u * t;
-      if (j < gsize) P.sacc[g0 + j] = res[t];
+      if (j < gsize) {
+        P.sacc[g0 + j] = res[t];
+        for (int q = 0; q < P.n_peers; ++q) P.peer_sacc[q][g0 + j] = res[t];
+      }
     }
   } else {
     // split group: its parts are consecutive tasks, in the head (expensive groups) or the tail
@@ -555,9 +562,16 @@ __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, con
           two_sum_fold(hi[2], lo[2], v.z); two_sum_fold(hi[3], lo[3], v.w);
         }
         unsigned j = lane + 32u * t;
-        if (j < gsize)
-          P.sacc[g0 + j] = make_float4(__fadd_rn(hi[0], lo[0]), __fadd_rn(hi[1], lo[1]), __fadd_rn(hi[2], lo[2]),
-                                       __fadd_rn(hi[3], lo[3]));
+        if (j < gsize) {
+          const float4 sum = make_float4(__fadd_rn(hi[0], lo[0]), __fadd_rn(hi[1], lo[1]), __fadd_rn(hi[2], lo[2]),
+                                         __fadd_rn(hi[3], lo[3]));
+          P.sacc[g0 + j] = sum;
+          for (int q = 0; q < P.n_peers; ++q) P.peer_sacc[q][g0 + j] = sum;
+        }
+      }
+      if (P.n_peers > 0 && lane == 0) {  // every part's counts were added before it signalled gdone
+        const uint2 c = __ldcg(&P.gcount[g]);
+        for (int q = 0; q < P.n_peers; ++q) P.peer_gcount[q][g] = c;
       }
     }
   }
@@ -611,14 +625,12 @@ constexpr unsigned MAX_PARTS = 63;
 constexpr unsigned TAIL_PARTS = 4;
 constexpr long long TAIL_PER_SM = BH_TAIL_PER_SM;  // groups per SM at the end of the list that are cut into TAIL_PARTS
 
-__global__ void walk_reset_kernel(DevInfo *info, unsigned reuse_gs) {
+__global__ void walk_reset_kernel(DevInfo *info, unsigned n_groups) {
   if (threadIdx.x == 0) {
-    // reuse_gs != 0: the per-group costs of the previous force pass stand in for the counting walk
-    // (tree_leapfrog: consecutive steps); their sum follows from the interaction totals
-    const unsigned long long prev = reuse_gs ? (13ull * info->n_pp + 37ull * info->n_pc) / reuse_gs : 0ull;
     info->group_ticket = 0; info->task_ticket = 0; info->n_pp = 0; info->n_pc = 0; info->n_tasks = 0;
-    info->sched_cost = prev;
+    info->sched_cost = 0;  // summed by the counting walk, or by group_cost_kernel from the previous pass's counts
     info->walk_overflow = 0;
+    info->g_lo = 0; info->g_hi = n_groups;  // narrowed by shard_partition_kernel in a sharded pass
     unsigned long long now;
     asm volatile("mov.u64 %0, %globaltimer;" : "=l"(now));
     info->t0_ns = now;
@@ -630,22 +642,90 @@ __device__ __forceinline__ double prev_cost(const uint2 *__restrict__ gcount, un
   return 13.0 * (double)c.x + 37.0 * (double)c.y;
 }
 
+// Cost estimate of every group for this pass: the counting walk's (left in gdone), or -- tree_leapfrog,
+// the same particles one step later -- the exact counts of the previous pass (the neighbours cover a
+// shift of the runs by up to two); in that case their sum is formed here.
+__global__ void __launch_bounds__(256) group_cost_kernel(unsigned n_groups, DevInfo *info, const uint32_t *__restrict__ gdone,
+                                                         const uint2 *__restrict__ prev, double *__restrict__ gcost) {
+  const unsigned g = blockIdx.x * blockDim.x + threadIdx.x;
+  double own = 0.0;
+  if (g < n_groups) {
+    double cost;
+    if (prev) {
+      own = prev_cost(prev, g);
+      cost = own;
+      const unsigned a = g >= 2 ? g - 2 : 0u, b = g + 2 < n_groups ? g + 2 : n_groups - 1;
+      for (unsigned q = a; q <= b; ++q) cost = fmax(cost, prev_cost(prev, q));
+    } else {
+      cost = (double)gdone[g];
+    }
+    gcost[g] = cost;
+  }
+  if (prev) {  // block-uniform
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) own += __shfl_xor_sync(0xffffffffu, own, o);
+    __shared__ double s_own[8];
+    if ((threadIdx.x & 31) == 0) s_own[threadIdx.x >> 5] = own;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      double a = 0.0;
+      for (int k = 0; k < 8; ++k) a += s_own[k];
+      atomicAdd(&info->sched_cost, (unsigned long long)a);  // integers below 2^53: exact, order-independent
+    }
+  }
+}
+
+// Sharded pass: rank r of `world` walks the groups [B(r), B(r+1)), B(r) = number of groups whose exclusive
+// cost prefix is below r/world of the total (contiguous pieces of the PH curve; L107:
+// balanced on the flops of the tree-walk).  Every context evaluates this on identical costs in the same
+// order, so all agree.  One block; thread i owns one contiguous chunk.
+constexpr int PARTITION_THREADS = 1024;
+__global__ void __launch_bounds__(PARTITION_THREADS) shard_partition_kernel(unsigned n_groups, const double *__restrict__ gcost,
+                                                                            unsigned rank, unsigned world, DevInfo *info) {
+  __shared__ double s_sum[PARTITION_THREADS];
+  __shared__ unsigned s_cnt[2];
+  const unsigned chunk = (n_groups + PARTITION_THREADS - 1) / PARTITION_THREADS;
+  const unsigned c0 = min(threadIdx.x * chunk, n_groups), c1 = min(c0 + chunk, n_groups);
+  double sum = 0.0;
+  for (unsigned g = c0; g < c1; ++g) sum += gcost[g];
+  s_sum[threadIdx.x] = sum;
+  if (threadIdx.x < 2) s_cnt[threadIdx.x] = 0u;
+  __syncthreads();
+  __shared__ double s_total;
+  if (threadIdx.x == 0) {  // serial exclusive scan of 1024 chunk sums: the order is part of the contract
+    double run = 0.0;
+    for (int i = 0; i < PARTITION_THREADS; ++i) { const double v = s_sum[i]; s_sum[i] = run; run += v; }
+    s_total = run;
+  }
+  __syncthreads();
+  const double total = s_total;
+  const double t_lo = total * (double)rank / (double)world, t_hi = total * (double)(rank + 1u) / (double)world;
+  double run = s_sum[threadIdx.x];
+  unsigned n_lo = 0, n_hi = 0;
+  for (unsigned g = c0; g < c1; ++g) {
+    n_lo += run < t_lo;
+    n_hi += run < t_hi;
+    run += gcost[g];
+  }
+  if (n_lo) atomicAdd(&s_cnt[0], n_lo);
+  if (n_hi) atomicAdd(&s_cnt[1], n_hi);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    info->g_lo = rank == 0 ? 0u : s_cnt[0];
+    info->g_hi = rank + 1 == world ? n_groups : s_cnt[1];
+  }
+}
+
 __global__ void __launch_bounds__(256) task_cost_kernel(unsigned n_groups, const DevInfo *__restrict__ info,
                                                         uint32_t *__restrict__ a_cnt, uint32_t *__restrict__ gdone,
-                                                        uint32_t *__restrict__ gthresh, const uint2 *__restrict__ prev) {
+                                                        uint32_t *__restrict__ gthresh, const double *__restrict__ gcost) {
   unsigned g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= n_groups) return;
-  const double mean = (double)info->sched_cost / (double)n_groups;
-  double cost;
-  if (prev) {  // exact counts of the previous pass; the neighbours cover a shift of the runs by up to two
-    cost = 0.0;
-    const unsigned a = g >= 2 ? g - 2 : 0u, b = g + 2 < n_groups ? g + 2 : n_groups - 1;
-    for (unsigned q = a; q <= b; ++q) cost = fmax(cost, prev_cost(prev, q));
-  } else {
-    cost = (double)gdone[g];
-  }
+  const double mean = (double)info->sched_cost / (double)n_groups;  // over ALL groups, also in a sharded pass
+  const double cost = gcost[g];
+  const bool mine = g >= info->g_lo && g < info->g_hi;
   unsigned s = 0;
-  if (cost > SPLIT_AT * mean && mean > 0.0) {
+  if (mine && cost > SPLIT_AT * mean && mean > 0.0) {
     double want = ceil(SPLIT_FINE * cost / mean);
     s = want > (double)MAX_PARTS ? MAX_PARTS : (unsigned)want;
     if (s < 2) s = 0;
@@ -657,10 +737,16 @@ __global__ void __launch_bounds__(256) task_cost_kernel(unsigned n_groups, const
   gthresh[g] = per_entry < 32.0 ? 32u : (per_entry > 1e9 ? 1000000000u : (unsigned)per_entry);
 }
 
+// the last groups of this context's range are cut into TAIL_PARTS so that the kernel ends on small tasks
+__device__ __forceinline__ unsigned tail_groups(const DevInfo *info, unsigned n_tail) {
+  const unsigned mine = info->g_hi - info->g_lo;
+  return min(n_tail, mine / 4u);
+}
+
 // after the exclusive scan of a_cnt (in place -> a_off): expensive groups that do not fit the
 // partial-sum buffer (a suffix of them, offsets are monotone) fall back to one part; classifies
-// every group (head / body / tail) and writes the body counts
-__global__ void __launch_bounds__(256) task_class_kernel(unsigned n_groups, unsigned n_tail,
+// every group of this context's range (head / body / tail) and writes the body counts
+__global__ void __launch_bounds__(256) task_class_kernel(unsigned n_groups, unsigned n_tail_max,
                                                          const uint32_t *__restrict__ a_off, const uint32_t *a_total,
                                                          unsigned head_cap, uint8_t *__restrict__ gparts,
                                                          uint32_t *__restrict__ b_cnt, uint2 *__restrict__ gcount,
@@ -668,6 +754,10 @@ __global__ void __launch_bounds__(256) task_class_kernel(unsigned n_groups, unsi
   unsigned g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= n_groups) return;
   const unsigned tot = *a_total;
+  if (g == 0 && tot <= head_cap) info->n_tasks_a = tot;
+  const unsigned lo = info->g_lo, hi = info->g_hi;
+  if (g < lo || g >= hi) { gparts[g] = 1; b_cnt[g] = 0u; return; }  // another context's group: its counts arrive by peer store
+  const unsigned n_tail = tail_groups(info, n_tail_max);
   const unsigned off = a_off[g];
   const unsigned nxt = (g + 1 < n_groups) ? a_off[g + 1] : tot;
   unsigned s = nxt - off;
@@ -675,25 +765,28 @@ __global__ void __launch_bounds__(256) task_class_kernel(unsigned n_groups, unsi
     if (off <= head_cap) info->n_tasks_a = off;  // the first expensive group that does not fit
     s = 0;
   }
-  const bool tail = g >= n_groups - n_tail;
+  const bool tail = g >= hi - n_tail;
   gparts[g] = (uint8_t)(s ? (s | PARTS_HEAD) : (tail ? TAIL_PARTS : 1u));
   b_cnt[g] = (s || tail) ? 0u : 1u;
   gcount[g] = make_uint2(0u, 0u);
-  if (g == 0 && tot <= head_cap) info->n_tasks_a = tot;
 }
 
-__global__ void __launch_bounds__(256) task_fill_kernel(unsigned n_groups, unsigned n_tail,
+__global__ void __launch_bounds__(256) task_fill_kernel(unsigned n_groups, unsigned n_tail_max,
                                                         const uint32_t *__restrict__ a_off,
                                                         const uint32_t *__restrict__ b_off, const uint32_t *b_total,
                                                         const uint8_t *__restrict__ gparts, uint32_t *__restrict__ tasks,
                                                         DevInfo *info) {
   unsigned g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= n_groups) return;
+  const unsigned lo = info->g_lo, hi = info->g_hi;
+  const unsigned n_tail = tail_groups(info, n_tail_max);
   const unsigned a_end = info->n_tasks_a;
   const unsigned tail_start = a_end + *b_total;
+  if (g == 0) { info->n_tasks = tail_start + n_tail * TAIL_PARTS; info->tail_start = tail_start; }
+  if (g < lo || g >= hi) return;
   const unsigned gp = gparts[g], s = gp & PARTS_MASK;
   const bool head = gp & PARTS_HEAD;
-  const bool tail = g >= n_groups - n_tail;
+  const bool tail = g >= hi - n_tail;
   if (head) {
     const unsigned off = a_off[g];
     for (unsigned j = 0; j < s; ++j) tasks[off + j] = g | (j << TASK_GROUP_BITS);
@@ -701,10 +794,9 @@ __global__ void __launch_bounds__(256) task_fill_kernel(unsigned n_groups, unsig
     tasks[a_end + b_off[g]] = g;
   }
   if (tail) {  // fixed slots; an expensive group inside the tail range leaves a hole here
-    const unsigned base = tail_start + (g - (n_groups - n_tail)) * TAIL_PARTS;
+    const unsigned base = tail_start + (g - (hi - n_tail)) * TAIL_PARTS;
     for (unsigned j = 0; j < TAIL_PARTS; ++j) tasks[base + j] = head ? TASK_NONE : (g | (j << TASK_GROUP_BITS));
   }
-  if (g == 0) { info->n_tasks = tail_start + n_tail * TAIL_PARTS; info->tail_start = tail_start; }
 }
 
 // a11: results back to caller order
@@ -857,17 +949,24 @@ static int launch_walk(tree_ctx *t, const WalkParams &P, unsigned grid) {
   // 1. cost of every group: the walk without the evaluation, or the previous pass's exact counts
   const bool reuse = t->reuse_costs;
   if (!reuse) {
-  const long long cwant = (ng + WALK_WARPS - 1) / WALK_WARPS, ccap = (long long)t->sm_count * COUNT_MINB;
-  walk_force_kernel<TPL, true><<<(unsigned)(cwant < ccap ? cwant : ccap), WALK_WARPS * 32, 0, t->stream>>>(P);
-  BH_LAUNCH_CHECK("walk_count");
+    const long long cwant = (ng + WALK_WARPS - 1) / WALK_WARPS, ccap = (long long)t->sm_count * COUNT_MINB;
+    walk_force_kernel<TPL, true><<<(unsigned)(cwant < ccap ? cwant : ccap), WALK_WARPS * 32, 0, t->stream>>>(P);
+    BH_LAUNCH_CHECK("walk_count");
   }
-  // 2. task list: split expensive groups, longest work first
-  task_cost_kernel<<<gb, 256, 0, t->stream>>>(ng, info, t->b.sched_a, t->b.gdone, t->b.gthresh,
-                                              reuse ? t->b.gcount : nullptr);
+  group_cost_kernel<<<gb, 256, 0, t->stream>>>(ng, info, t->b.gdone, reuse ? t->b.gcount2[(t->pass + 1) & 1] : nullptr,
+                                               t->b.gcost);
+  BH_LAUNCH_CHECK("group_cost");
+  if (t->shard_world > 1) {
+    shard_partition_kernel<<<1, PARTITION_THREADS, 0, t->stream>>>(ng, t->b.gcost, (unsigned)t->shard_rank,
+                                                                   (unsigned)t->shard_world, info);
+    BH_LAUNCH_CHECK("shard_partition");
+  }
+  // 2. task list of this context's range: split expensive groups, longest work first
+  task_cost_kernel<<<gb, 256, 0, t->stream>>>(ng, info, t->b.sched_a, t->b.gdone, t->b.gthresh, t->b.gcost);
   BH_LAUNCH_CHECK("task_cost");
   int rc = device_excl_scan(t, t->b.sched_a, ng, tot);
   if (rc) return rc;
-  const unsigned n_tail = (unsigned)std::min<long long>(std::min<long long>(ng / 4, TAIL_PER_SM * t->sm_count), t->tail_cap / (long long)TAIL_PARTS);
+  const unsigned n_tail = (unsigned)std::min<long long>(TAIL_PER_SM * t->sm_count, t->tail_cap / (long long)TAIL_PARTS);
   task_class_kernel<<<gb, 256, 0, t->stream>>>(ng, n_tail, t->b.sched_a, tot, (unsigned)t->head_cap, t->b.gparts,
                                                t->b.sched_b, t->b.gcount, info);
   BH_LAUNCH_CHECK("task_class");
@@ -888,9 +987,17 @@ int run_walk(tree_ctx *t, float eps) {
   P.spos = t->b.spos; P.c_test = t->b.c_test; P.c_link = t->b.c_link;
   P.c_cm = t->b.c_cm; P.c_qa = t->b.c_qa; P.c_qb = t->b.c_qb;
   P.gbox = t->b.gbox; P.sacc = t->b.sacc; P.gcount = t->b.gcount; P.info = t->d_info;
+  P.n_peers = 0;
+  for (int r = 0; r < TREE_SHARD_MAX_WORLD; ++r) { P.peer_sacc[r] = nullptr; P.peer_gcount[r] = nullptr; }
+  if (t->shard_world > 1)
+    for (int r = 0; r < t->shard_world; ++r)
+      if (r != t->shard_rank) {
+        shard_views(t, t->peer_base[r], (int)(t->pass & 1), &P.peer_sacc[P.n_peers], &P.peer_gcount[P.n_peers]);
+        ++P.n_peers;
+      }
   P.c_count = t->b.c_count; P.trace = t->b.trace; P.gthresh = t->b.gthresh; P.tasks = t->b.tasks; P.gparts = t->b.gparts; P.gdone = t->b.gdone; P.part = t->b.part;
   P.N = t->N; P.n_groups = (unsigned)t->n_groups; P.eps2 = eps * eps;
-  walk_reset_kernel<<<1, 32, 0, t->stream>>>(t->d_info, t->reuse_costs ? (unsigned)t->group : 0u);
+  walk_reset_kernel<<<1, 32, 0, t->stream>>>(t->d_info, (unsigned)t->n_groups);
   BH_LAUNCH_CHECK("walk_reset");
   long long want = (t->n_groups + WALK_WARPS - 1) / WALK_WARPS;
   long long cap = (long long)t->sm_count * WALK_MINB;

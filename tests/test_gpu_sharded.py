@@ -1,0 +1,154 @@
+"""GPU parity of the sharded force pass (include/tree.h "sharded force pass"): `world`
+contexts share one pass, each walking one contiguous cost-balanced range of the PH-sorted groups
+ and storing its results into every context's buffers.  One GPU is enough to
+check the path: the contexts live in one process on cuda:0 and their kernels run one after the other
+(none waits for another); across GPUs the same stores go over NVLink.  Every context must end up with
+the complete result, equal to the oracle's within 1e-5 and with bit-exact interaction counts."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from nbody_inputs import plummer, milky_way
+from paper_1412_0659_b200 import Tree, TreeError
+from paper_1412_0659_b200.sharded import connect_local, force_local, leapfrog_local
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-5
+
+
+def _make(world, n, leaf=16, group=64):
+    trees = [Tree(device=0, leaf_size=leaf, group_size=group) for _ in range(world)]
+    for t in trees:
+        t.reserve(n)
+    connect_local(trees)
+    return trees
+
+
+def _close(trees):
+    torch.cuda.synchronize()
+    for t in trees:
+        t.close()
+
+
+@pytest.mark.parametrize("model,n,seed,world", [
+    ("plummer", 20011, 11, 2),   # ragged last group
+    ("plummer", 16384, 1001, 3), # BASELINE config 1, three ranks
+    ("mw", 100000, 3, 4),        # deep, uneven tree: cost balance differs strongly from count balance
+    ("plummer", 300, 4, 8),      # fewer groups than ranks x 4: some ranks own no or one group
+])
+def test_sharded_pass_equals_oracle_on_every_rank(model, n, seed, world):
+    theta, eps = 0.4, 0.01
+    pos, _, mass = (plummer if model == "plummer" else milky_way)(n, seed, with_vel=False)
+    dpos, dmass = pos.cuda(), mass.cuda()
+    trees = _make(world, n)
+    outs = [(torch.zeros((n, 3), device="cuda"), torch.zeros(n, device="cuda")) for _ in range(world)]
+    for t in trees:
+        t.build(dpos, dmass)
+    force_local(trees, theta, eps, outs)
+    torch.cuda.synchronize()
+    ot = oracle.Tree(pos.numpy(), mass.numpy())
+    oacc, opot, onpp, onpc = ot.force(theta, eps)
+    # the ranges tile the groups in rank order
+    ranges = [t.shard_range() for t in trees]
+    assert ranges[0][0] == 0 and ranges[-1][1] == ot.n_groups
+    for a, b in zip(ranges[:-1], ranges[1:]):
+        assert a[1] == b[0] and a[3] == b[2]
+    assert all(r[0] <= r[1] for r in ranges)
+    # cost balance: no rank above twice its fair share when it owns more than a few groups
+    cost = 13.0 * onpp + 37.0 * onpc
+    if ot.n_groups >= 32 * world:
+        shares = [cost[r[0]:r[1]].sum() / cost.sum() for r in ranges]
+        assert max(shares) < 2.0 / world, shares
+    tot_pp = tot_pc = 0
+    for t, (acc, pot) in zip(trees, outs):
+        cnt = t.debug("counts")  # peers stored their groups' counts here
+        assert np.array_equal(cnt[:, 0], onpp) and np.array_equal(cnt[:, 1], onpc)
+        a = acc.cpu().numpy().astype(np.float64); p = pot.cpu().numpy().astype(np.float64)
+        rel = np.linalg.norm(a - oacc, axis=1) / np.linalg.norm(oacc, axis=1)
+        prel = np.abs(p - opot) / np.abs(opot)
+        assert rel.max() <= TOL and prel.max() <= TOL, (rel.max(), prel.max())
+        _, pp, pc = t.stats()
+        tot_pp += pp; tot_pc += pc
+    gs = np.minimum(ot.group_size, ot.n - ot.group_size * np.arange(ot.n_groups))
+    assert tot_pp == int((onpp.astype(np.int64) * gs).sum()) and tot_pc == int((onpc.astype(np.int64) * gs).sum())
+    # every rank holds the same bits
+    for acc, pot in outs[1:]:
+        assert torch.equal(acc, outs[0][0]) and torch.equal(pot, outs[0][1])
+    _close(trees)
+
+
+def test_sharded_leapfrog_matches_single_context_and_ranks_agree_bitwise():
+    n, theta, eps, dt, steps, world = 30011, 0.4, 0.01, 1e-3, 4, 3
+    pos, vel, mass = plummer(n, 21)
+    dpos, dvel, dmass = pos.cuda(), vel.cuda(), mass.cuda()
+    single = Tree(device=0)
+    single.build(dpos, dmass); single.set_velocity(dvel); single.force(theta, eps)
+    trees = _make(world, n)
+    for t in trees:
+        t.build(dpos, dmass); t.set_velocity(dvel)
+    force_local(trees, theta, eps)
+    for _ in range(steps):
+        single.leapfrog(dt)
+        leapfrog_local(trees, dt)  # steps after the first schedule and partition by the previous pass's counts
+    torch.cuda.synchronize()
+
+    def state(t):
+        p = torch.empty((n, 3), device="cuda"); v = torch.empty((n, 3), device="cuda")
+        a = torch.empty((n, 3), device="cuda"); ph = torch.empty(n, device="cuda")
+        t.get_state(p, v, a, ph)
+        return p, v, a, ph
+
+    ref = state(single)
+    sts = [state(t) for t in trees]
+    for st in sts[1:]:
+        for x, y in zip(st, sts[0]):
+            assert torch.equal(x, y)  # identical inputs, identical tree, the same stored results
+    for x, y in zip(sts[0], ref):
+        d = (x.double() - y.double()).abs().max().item()
+        assert d <= 2e-6 * y.double().abs().max().item(), d  # a few partial sums are ordered differently
+    # the partition follows the previous pass's costs: ranges still tile the groups
+    ranges = [t.shard_range() for t in trees]
+    assert ranges[0][0] == 0 and ranges[-1][1] == (n + 63) // 64
+    assert all(a[1] == b[0] for a, b in zip(ranges[:-1], ranges[1:]))
+    single.close(); _close(trees)
+
+
+def test_sharded_call_order_errors():
+    n = 4096
+    pos, _, mass = plummer(n, 5, with_vel=False)
+    t = Tree(device=0)
+    with pytest.raises(TreeError) as e:
+        t.shard_config(0, 2)          # needs tree_reserve first
+    assert e.value.code == -4
+    t.reserve(n)
+    with pytest.raises(TreeError):
+        t.shard_config(2, 2)          # rank out of range
+    t.shard_config(0, 2)
+    t.build(pos.cuda(), mass.cuda())
+    with pytest.raises(TreeError) as e:
+        t.force(0.4, 0.01)            # cannot contain the barrier
+    assert e.value.code == -4
+    with pytest.raises(TreeError) as e:
+        t.force_begin(0.4, 0.01)      # peer 1 not attached
+    assert e.value.code == -4
+    big = plummer(2 * n, 5, with_vel=False)
+    with pytest.raises(TreeError) as e:
+        t.build(big[0].cuda(), big[2].cuda())  # beyond the reserved capacity: would invalidate exported buffers
+    assert e.value.code == -4
+    h = t.shard_export()
+    assert len(h) == 128 and any(h)
+    with pytest.raises(TreeError):
+        t.force_end()                 # no pass open
+    t.shard_config(0, 1)              # back to one context
+    t.build(pos.cuda(), mass.cuda())
+    t.force(0.4, 0.01)
+    # begin / end on one context is tree_force in two halves
+    acc = torch.empty((n, 3), device="cuda"); acc2 = torch.empty((n, 3), device="cuda")
+    t.force(0.4, 0.01, acc)
+    t.force_begin(0.4, 0.01)
+    with pytest.raises(TreeError):
+        t.force_begin(0.4, 0.01)      # already open
+    t.force_end(acc2)
+    assert torch.equal(acc, acc2)
+    t.close()
