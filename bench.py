@@ -17,6 +17,8 @@ e2e     : the same metric through the C ABI with HOST buffers (tree_build_host +
 roofline: the fused walk+force kernel against the FP32 FMA peak (bound "alu")
 N > 1   : the path is partitioned by independent problems: every rank runs its own replica of the
           workload (seed + rank), no data-path collective; scaling "weak".
+          ``--sharded``: ONE problem over the N GPUs instead (every rank builds the same tree,
+          walks a cost-balanced range of groups and peer-stores its results into all ranks); scaling "strong".
 ``--impl reference`` times the CPU oracle (oracle/) on the host cores on a bounded sample.
 """
 from __future__ import annotations
@@ -198,7 +200,9 @@ def run_ours(args):
     cfg = dict(CONFIGS[args.config])
     if args.n:
         cfg["n"] = args.n
-    cfg["seed"] = replica_seed(cfg["seed"], rank)  # every rank its own replica of the workload
+    sharded = bool(args.sharded)
+    if not sharded:
+        cfg["seed"] = replica_seed(cfg["seed"], rank)  # every rank its own replica of the workload
     from nbody_inputs import plummer, milky_way
     gen = plummer if cfg["model"] == "plummer" else milky_way
     gen_dev = dev if cfg["n"] > (1 << 22) else "cpu"
@@ -211,6 +215,12 @@ def run_ours(args):
 
     stream = torch.cuda.current_stream(dev)
     t = Tree(device=local, stream=stream.cuda_stream)
+    if sharded:  # one problem over all ranks: same particles everywhere, the force pass is cut
+        from paper_1412_0659_b200.sharded import ShardedTree
+        drv = ShardedTree(t, device=dev)
+        drv.connect(n)
+    else:
+        drv = t
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
 
     def barrier():
@@ -219,10 +229,10 @@ def run_ours(args):
         torch.cuda.synchronize(dev)
 
     # ---- device-resident steps: tree_leapfrog
-    t.build(d_pos, d_mass); t.set_velocity(d_vel); t.force(cfg["theta"], cfg["eps"])
+    drv.build(d_pos, d_mass); drv.set_velocity(d_vel); drv.force(cfg["theta"], cfg["eps"])
     ke0, pe0 = t.energy()  # synchronised velocities: E(0) of the KDK run (T12)
     for _ in range(args.warmup):
-        t.leapfrog(dt)
+        drv.leapfrog(dt)
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
@@ -234,9 +244,9 @@ def run_ours(args):
     for k in range(args.steps):
         flush.fill_(k & 0xff)  # L2 flush, outside the event pair
         ev[k][0].record(stream)
-        t.leapfrog(dt)
+        drv.leapfrog(dt)
         ev[k][1].record(stream)
-        ms, pp, pc = t.stats()  # synchronises; reads the library's own per-phase CUDA events
+        ms, pp, pc = t.stats()  # synchronises; reads the library's own per-phase CUDA events (this rank's share)
         for key, v in ms.items():
             phase_ms[key] = phase_ms.get(key, 0.0) + v
         pp_tot += pp; pc_tot += pc
@@ -254,7 +264,28 @@ def run_ours(args):
     value = (pp_all + pc_all) / (step_ms_max * 1e-3)
 
     # ---- end to end through the C ABI with host buffers (build + force, copies timed)
-    t2 = Tree(device=local, stream=stream.cuda_stream)
+    if sharded:
+        # the sharded pass has no *_host call: the same copies through torch, then build + sharded force
+        d_acc = torch.empty((n, 3), device=dev); d_pot = torch.empty(n, device=dev)
+
+        class _HostCalls:
+            def build_host(self, hp, hm):
+                d_pos.copy_(hp, non_blocking=True); d_mass.copy_(hm, non_blocking=True)
+                drv.build(d_pos, d_mass)
+
+            def force_host(self, theta, eps, ha, hp):
+                drv.force(theta, eps, d_acc, d_pot)
+                ha.copy_(d_acc, non_blocking=True); hp.copy_(d_pot, non_blocking=True)
+                torch.cuda.synchronize(dev)
+
+            def stats(self):
+                return t.stats()
+
+            def close(self):
+                pass
+        t2 = _HostCalls()
+    else:
+        t2 = Tree(device=local, stream=stream.cuda_stream)
     for _ in range(min(args.warmup, 3)):
         t2.build_host(h_pos, h_mass); t2.force_host(cfg["theta"], cfg["eps"], h_acc, h_pot)
     barrier()
@@ -272,7 +303,7 @@ def run_ours(args):
         for key, v in ems.items():
             e_phase[key] = e_phase.get(key, 0.0) + v / args.steps
         e_pp += pp; e_pc += pc
-    e2e_val = whole_job_rate(e2e_s, float(e_pp + e_pc), dev)
+    e2e_val = whole_job_rate(e2e_s, float(e_pp + e_pc), dev)  # each rank counts the interactions it evaluated
     t2.close()
 
     if rank == 0:
@@ -304,13 +335,15 @@ def run_ours(args):
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": step_ms_max / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": cfg["name"], "n_per_gpu": n, "model": cfg["model"], "theta": cfg["theta"],
+            "scaling": "strong" if sharded else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": cfg["name"], ("n_total" if sharded else "n_per_gpu"): n, "model": cfg["model"], "theta": cfg["theta"],
                        "eps": cfg["eps"], "dt": dt, "leaf_size": 16, "group_size": 64,
                        "step": "tree_leapfrog = kick/drift + keys + sort + build + moments + walk+force + kick",
-                       "l2": "flushed between steps (256 MB write)", "parallelism": f"replicas x{world}"},
+                       "l2": "flushed between steps (256 MB write)", "parallelism": (f"sharded force pass x{world} (replicated tree, peer stores)" if sharded
+                                       else f"replicas x{world}")},
             "effective_tflops_step": effective_flops(pp_all, pc_all) / (step_ms_max * 1e-3) / 1e12,
-            "pp_per_particle": pp_tot / args.steps / n, "pc_per_particle": pc_tot / args.steps / n,
+            "pp_per_particle": (pp_all if sharded else pp_tot) / args.steps / n,
+            "pc_per_particle": (pc_all if sharded else pc_tot) / args.steps / n,
             "phase_ms": {k: v / args.steps for k, v in phase_ms.items()},
             "roofline": roof,
             "energy": energy,
@@ -321,7 +354,7 @@ def run_ours(args):
             "gpu_launches": launches, "clocks": clocks, "wall_s_timed_region": wall,
         }
         print(json.dumps(line))
-    t.close()
+    drv.close()
     if world > 1:
         dist.destroy_process_group()
     return 0
@@ -336,6 +369,8 @@ def main():
     ap.add_argument("--n", type=int, default=0, help="override N (debugging only)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--sharded", action="store_true",
+                    help="N > 1: one problem over all GPUs (sharded force pass, strong scaling) instead of replicas")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

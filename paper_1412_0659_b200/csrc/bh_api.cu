@@ -77,7 +77,7 @@ static int ensure_particles(tree_ctx *t, long long N) {
   t->tail_cap = 4ll * 2 * t->sm_count * 16;  // 4 parts x (2 x resident warps) groups
   const long long part_cap = t->head_cap + t->tail_cap;
   BH_TRY(dev_alloc(t, b.sched_a, ng));
-  BH_TRY(dev_alloc(t, b.sched_b, ng));
+  BH_TRY(dev_alloc(t, b.sched_b, ng + 2));  // also holds the 64-bit partial cost sums of the shard partition
   BH_TRY(dev_alloc(t, b.gdone, ng));
   BH_TRY(dev_alloc(t, b.gparts, ng));
   BH_TRY(dev_alloc(t, b.gthresh, ng));

@@ -676,51 +676,128 @@ __global__ void __launch_bounds__(256) group_cost_kernel(unsigned n_groups, DevI
 }
 
 // Sharded pass: rank r of `world` walks the groups [B(r), B(r+1)), B(r) = number of groups whose exclusive
-// cost prefix is below r/world of the total (contiguous pieces of the PH curve; L107:
-// balanced on the flops of the tree-walk).  Every context evaluates this on identical costs in the same
-// order, so all agree.  One block; thread i owns one contiguous chunk.
-constexpr int PARTITION_THREADS = 1024;
-__global__ void __launch_bounds__(PARTITION_THREADS) shard_partition_kernel(unsigned n_groups, const double *__restrict__ gcost,
-                                                                            unsigned rank, unsigned world, DevInfo *info) {
-  __shared__ double s_sum[PARTITION_THREADS];
-  __shared__ unsigned s_cnt[2];
-  const unsigned chunk = (n_groups + PARTITION_THREADS - 1) / PARTITION_THREADS;
-  const unsigned c0 = min(threadIdx.x * chunk, n_groups), c1 = min(c0 + chunk, n_groups);
-  double sum = 0.0;
-  for (unsigned g = c0; g < c1; ++g) sum += gcost[g];
-  s_sum[threadIdx.x] = sum;
-  if (threadIdx.x < 2) s_cnt[threadIdx.x] = 0u;
-  __syncthreads();
-  __shared__ double s_total;
-  if (threadIdx.x == 0) {  // serial exclusive scan of 1024 chunk sums: the order is part of the contract
-    double run = 0.0;
-    for (int i = 0; i < PARTITION_THREADS; ++i) { const double v = s_sum[i]; s_sum[i] = run; run += v; }
-    s_total = run;
+// cost prefix is below floor(total r / world) (contiguous pieces of the PH curve; L107:
+// balanced on the flops of the tree-walk).  Costs are integers (13 n_pp + 37 n_pc), so the prefix sums do
+// not depend on the order of addition and every context arrives at the same bounds.
+constexpr int PART_BLOCK = 1024;  // groups per partial sum
+__global__ void __launch_bounds__(256) shard_blocksum_kernel(unsigned n_groups, const double *__restrict__ gcost,
+                                                             unsigned long long *__restrict__ bsum) {
+  unsigned long long v = 0;
+  const unsigned base = blockIdx.x * PART_BLOCK;
+#pragma unroll
+  for (int k = 0; k < PART_BLOCK / 256; ++k) {
+    const unsigned g = base + k * 256 + threadIdx.x;
+    if (g < n_groups) v += (unsigned long long)gcost[g];
   }
-  __syncthreads();
-  const double total = s_total;
-  const double t_lo = total * (double)rank / (double)world, t_hi = total * (double)(rank + 1u) / (double)world;
-  double run = s_sum[threadIdx.x];
-  unsigned n_lo = 0, n_hi = 0;
-  for (unsigned g = c0; g < c1; ++g) {
-    n_lo += run < t_lo;
-    n_hi += run < t_hi;
-    run += gcost[g];
-  }
-  if (n_lo) atomicAdd(&s_cnt[0], n_lo);
-  if (n_hi) atomicAdd(&s_cnt[1], n_hi);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  __shared__ unsigned long long s[8];
+  if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = v;
   __syncthreads();
   if (threadIdx.x == 0) {
-    info->g_lo = rank == 0 ? 0u : s_cnt[0];
-    info->g_hi = rank + 1 == world ? n_groups : s_cnt[1];
+    unsigned long long a = 0;
+    for (int k = 0; k < 8; ++k) a += s[k];
+    bsum[blockIdx.x] = a;
   }
+}
+
+// exclusive scan over the 1024 threads of a block (warp shuffles + one shared-memory step); also the total
+__device__ __forceinline__ unsigned long long block_excl_scan_u64(unsigned long long v, unsigned long long *s_warp,
+                                                                  unsigned long long &total) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  unsigned long long incl = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const unsigned long long n = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += n;
+  }
+  __syncthreads();  // s_warp may still be read from a previous call
+  if (lane == 31) s_warp[w] = incl;
+  __syncthreads();
+  if (w == 0) {
+    unsigned long long x = s_warp[lane], xi = x;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const unsigned long long n = __shfl_up_sync(0xffffffffu, xi, o);
+      if (lane >= o) xi += n;
+    }
+    s_warp[lane] = xi - x;
+    if (lane == 31) s_warp[32] = xi;
+  }
+  __syncthreads();
+  total = s_warp[32];
+  return s_warp[w] + incl - v;
+}
+
+__global__ void __launch_bounds__(PART_BLOCK) shard_bounds_kernel(unsigned n_groups, unsigned n_blocks,
+                                                                  const double *__restrict__ gcost,
+                                                                  const unsigned long long *__restrict__ bsum,
+                                                                  unsigned rank, unsigned world, DevInfo *info) {
+  __shared__ unsigned long long s_warp[33];
+  __shared__ unsigned s_cnt;
+  // 1. exclusive prefix of the partial sums at the start of this thread's chunk of them
+  const unsigned chunk = (n_blocks + PART_BLOCK - 1) / PART_BLOCK;
+  const unsigned b0 = min(threadIdx.x * chunk, n_blocks), b1 = min(b0 + chunk, n_blocks);
+  unsigned long long mine = 0;
+  for (unsigned b = b0; b < b1; ++b) mine += bsum[b];
+  unsigned long long total;
+  const unsigned long long start = block_excl_scan_u64(mine, s_warp, total);
+  unsigned bound[2];
+  for (int k = 0; k < 2; ++k) {
+    const unsigned r = rank + k;
+    const unsigned long long T = (total / world) * r + ((total % world) * r) / world;  // floor(total r / world)
+    // 2. the last partial-sum block whose first group lies below T, and its exclusive prefix
+    if (threadIdx.x == 0) s_cnt = 0u;
+    __syncthreads();
+    unsigned long long run = start;
+    unsigned below = 0;
+    for (unsigned b = b0; b < b1; ++b) { below += run < T; run += bsum[b]; }
+    if (below) atomicAdd(&s_cnt, below);
+    __syncthreads();
+    const unsigned n_below = s_cnt;
+    if (n_below == 0) { bound[k] = 0u; __syncthreads(); continue; }  // T = 0
+    const unsigned bstar = n_below - 1;
+    // exclusive prefix of block bstar = start of the thread that owns it + the blocks before it in that chunk
+    __shared__ unsigned long long s_pre;
+    if (bstar >= b0 && bstar < b1) {
+      unsigned long long pre = start;
+      for (unsigned b = b0; b < bstar; ++b) pre += bsum[b];
+      s_pre = pre;
+    }
+    __syncthreads();
+    // 3. inside that block: groups whose exclusive prefix is below T
+    const unsigned g = bstar * PART_BLOCK + threadIdx.x;
+    const unsigned long long c = g < n_groups ? (unsigned long long)gcost[g] : 0ull;
+    unsigned long long dummy;
+    const unsigned long long ex = s_pre + block_excl_scan_u64(c, s_warp, dummy);
+    const int inside = __syncthreads_count(g < n_groups && ex < T);
+    bound[k] = bstar * PART_BLOCK + (unsigned)inside;
+  }
+  if (threadIdx.x == 0) {
+    info->g_lo = rank == 0 ? 0u : bound[0];
+    info->g_hi = rank + 1 == world ? n_groups : bound[1];
+  }
+}
+
+// The last groups of this context's range are cut into TAIL_PARTS parts so that the kernel ends on small
+// tasks; a range shorter than that tail (small N, or many ranks sharing the pass) is cut entirely.  (Cutting
+// finer does not pay: every part repeats the group's skeleton walk; 16 parts ran 2.5 x slower at N = 16,384.)
+struct TailPlan { unsigned n_tail, parts; };
+struct TailLimits { unsigned n_tail_max; };  // groups
+__device__ __forceinline__ TailPlan tail_plan(const DevInfo *info, const TailLimits L) {
+  TailPlan p;
+  p.n_tail = min(L.n_tail_max, info->g_hi - info->g_lo);
+  p.parts = TAIL_PARTS;
+  return p;
 }
 
 __global__ void __launch_bounds__(256) task_cost_kernel(unsigned n_groups, const DevInfo *__restrict__ info,
                                                         uint32_t *__restrict__ a_cnt, uint32_t *__restrict__ gdone,
-                                                        uint32_t *__restrict__ gthresh, const double *__restrict__ gcost) {
+                                                        uint32_t *__restrict__ gthresh, const double *__restrict__ gcost,
+                                                        const TailLimits lim) {
   unsigned g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= n_groups) return;
+  const unsigned tail_parts = tail_plan(info, lim).parts;
   const double mean = (double)info->sched_cost / (double)n_groups;  // over ALL groups, also in a sharded pass
   const double cost = gcost[g];
   const bool mine = g >= info->g_lo && g < info->g_hi;
@@ -733,20 +810,14 @@ __global__ void __launch_bounds__(256) task_cost_kernel(unsigned n_groups, const
   a_cnt[g] = s;
   gdone[g] = 0;
   // about 16 dealt entries per part: particles opened ~ cost / 13 (an over-estimate)
-  const double per_entry = cost / 13.0 / (16.0 * (s ? s : TAIL_PARTS));
+  const double per_entry = cost / 13.0 / (16.0 * (s ? s : tail_parts));
   gthresh[g] = per_entry < 32.0 ? 32u : (per_entry > 1e9 ? 1000000000u : (unsigned)per_entry);
-}
-
-// the last groups of this context's range are cut into TAIL_PARTS so that the kernel ends on small tasks
-__device__ __forceinline__ unsigned tail_groups(const DevInfo *info, unsigned n_tail) {
-  const unsigned mine = info->g_hi - info->g_lo;
-  return min(n_tail, mine / 4u);
 }
 
 // after the exclusive scan of a_cnt (in place -> a_off): expensive groups that do not fit the
 // partial-sum buffer (a suffix of them, offsets are monotone) fall back to one part; classifies
 // every group of this context's range (head / body / tail) and writes the body counts
-__global__ void __launch_bounds__(256) task_class_kernel(unsigned n_groups, unsigned n_tail_max,
+__global__ void __launch_bounds__(256) task_class_kernel(unsigned n_groups, const TailLimits lim,
                                                          const uint32_t *__restrict__ a_off, const uint32_t *a_total,
                                                          unsigned head_cap, uint8_t *__restrict__ gparts,
                                                          uint32_t *__restrict__ b_cnt, uint2 *__restrict__ gcount,
@@ -757,7 +828,8 @@ __global__ void __launch_bounds__(256) task_class_kernel(unsigned n_groups, unsi
   if (g == 0 && tot <= head_cap) info->n_tasks_a = tot;
   const unsigned lo = info->g_lo, hi = info->g_hi;
   if (g < lo || g >= hi) { gparts[g] = 1; b_cnt[g] = 0u; return; }  // another context's group: its counts arrive by peer store
-  const unsigned n_tail = tail_groups(info, n_tail_max);
+  const TailPlan tp = tail_plan(info, lim);
+  const unsigned n_tail = tp.n_tail;
   const unsigned off = a_off[g];
   const unsigned nxt = (g + 1 < n_groups) ? a_off[g + 1] : tot;
   unsigned s = nxt - off;
@@ -766,12 +838,12 @@ __global__ void __launch_bounds__(256) task_class_kernel(unsigned n_groups, unsi
     s = 0;
   }
   const bool tail = g >= hi - n_tail;
-  gparts[g] = (uint8_t)(s ? (s | PARTS_HEAD) : (tail ? TAIL_PARTS : 1u));
+  gparts[g] = (uint8_t)(s ? (s | PARTS_HEAD) : (tail ? tp.parts : 1u));
   b_cnt[g] = (s || tail) ? 0u : 1u;
   gcount[g] = make_uint2(0u, 0u);
 }
 
-__global__ void __launch_bounds__(256) task_fill_kernel(unsigned n_groups, unsigned n_tail_max,
+__global__ void __launch_bounds__(256) task_fill_kernel(unsigned n_groups, const TailLimits lim,
                                                         const uint32_t *__restrict__ a_off,
                                                         const uint32_t *__restrict__ b_off, const uint32_t *b_total,
                                                         const uint8_t *__restrict__ gparts, uint32_t *__restrict__ tasks,
@@ -779,10 +851,11 @@ __global__ void __launch_bounds__(256) task_fill_kernel(unsigned n_groups, unsig
   unsigned g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= n_groups) return;
   const unsigned lo = info->g_lo, hi = info->g_hi;
-  const unsigned n_tail = tail_groups(info, n_tail_max);
+  const TailPlan tp = tail_plan(info, lim);
+  const unsigned n_tail = tp.n_tail;
   const unsigned a_end = info->n_tasks_a;
   const unsigned tail_start = a_end + *b_total;
-  if (g == 0) { info->n_tasks = tail_start + n_tail * TAIL_PARTS; info->tail_start = tail_start; }
+  if (g == 0) { info->n_tasks = tail_start + n_tail * tp.parts; info->tail_start = tail_start; }
   if (g < lo || g >= hi) return;
   const unsigned gp = gparts[g], s = gp & PARTS_MASK;
   const bool head = gp & PARTS_HEAD;
@@ -794,8 +867,8 @@ __global__ void __launch_bounds__(256) task_fill_kernel(unsigned n_groups, unsig
     tasks[a_end + b_off[g]] = g;
   }
   if (tail) {  // fixed slots; an expensive group inside the tail range leaves a hole here
-    const unsigned base = tail_start + (g - (hi - n_tail)) * TAIL_PARTS;
-    for (unsigned j = 0; j < TAIL_PARTS; ++j) tasks[base + j] = head ? TASK_NONE : (g | (j << TASK_GROUP_BITS));
+    const unsigned base = tail_start + (g - (hi - n_tail)) * tp.parts;
+    for (unsigned j = 0; j < tp.parts; ++j) tasks[base + j] = head ? TASK_NONE : (g | (j << TASK_GROUP_BITS));
   }
 }
 
@@ -957,22 +1030,27 @@ static int launch_walk(tree_ctx *t, const WalkParams &P, unsigned grid) {
                                                t->b.gcost);
   BH_LAUNCH_CHECK("group_cost");
   if (t->shard_world > 1) {
-    shard_partition_kernel<<<1, PARTITION_THREADS, 0, t->stream>>>(ng, t->b.gcost, (unsigned)t->shard_rank,
-                                                                   (unsigned)t->shard_world, info);
-    BH_LAUNCH_CHECK("shard_partition");
+    const unsigned nb = (ng + PART_BLOCK - 1) / PART_BLOCK;  // <= 2^16: sched_b (one word per group) has room
+    unsigned long long *bsum = reinterpret_cast<unsigned long long *>(t->b.sched_b);
+    shard_blocksum_kernel<<<nb, 256, 0, t->stream>>>(ng, t->b.gcost, bsum);
+    BH_LAUNCH_CHECK("shard_blocksum");
+    shard_bounds_kernel<<<1, PART_BLOCK, 0, t->stream>>>(ng, nb, t->b.gcost, bsum, (unsigned)t->shard_rank,
+                                                         (unsigned)t->shard_world, info);
+    BH_LAUNCH_CHECK("shard_bounds");
   }
   // 2. task list of this context's range: split expensive groups, longest work first
-  task_cost_kernel<<<gb, 256, 0, t->stream>>>(ng, info, t->b.sched_a, t->b.gdone, t->b.gthresh, t->b.gcost);
+  TailLimits lim;
+  lim.n_tail_max = (unsigned)std::min<long long>(TAIL_PER_SM * t->sm_count, t->tail_cap / (long long)TAIL_PARTS);
+  task_cost_kernel<<<gb, 256, 0, t->stream>>>(ng, info, t->b.sched_a, t->b.gdone, t->b.gthresh, t->b.gcost, lim);
   BH_LAUNCH_CHECK("task_cost");
   int rc = device_excl_scan(t, t->b.sched_a, ng, tot);
   if (rc) return rc;
-  const unsigned n_tail = (unsigned)std::min<long long>(TAIL_PER_SM * t->sm_count, t->tail_cap / (long long)TAIL_PARTS);
-  task_class_kernel<<<gb, 256, 0, t->stream>>>(ng, n_tail, t->b.sched_a, tot, (unsigned)t->head_cap, t->b.gparts,
+  task_class_kernel<<<gb, 256, 0, t->stream>>>(ng, lim, t->b.sched_a, tot, (unsigned)t->head_cap, t->b.gparts,
                                                t->b.sched_b, t->b.gcount, info);
   BH_LAUNCH_CHECK("task_class");
   rc = device_excl_scan(t, t->b.sched_b, ng, tot + 1);
   if (rc) return rc;
-  task_fill_kernel<<<gb, 256, 0, t->stream>>>(ng, n_tail, t->b.sched_a, t->b.sched_b, tot + 1, t->b.gparts, t->b.tasks,
+  task_fill_kernel<<<gb, 256, 0, t->stream>>>(ng, lim, t->b.sched_a, t->b.sched_b, tot + 1, t->b.gparts, t->b.tasks,
                                               info);
   BH_LAUNCH_CHECK("task_fill");
   if (t->ev_valid[EV_SCHED]) cudaEventRecord(t->ev[EV_SCHED], t->stream);

@@ -5,7 +5,7 @@ Every rank (one process per GPU, ``torch.distributed``) holds all N particles an
 tree; rank r walks one contiguous, cost-balanced range of the Peano-Hilbert-sorted groups
  and its walk kernel stores the results straight into every rank's result
 buffers (peer stores over NVLink).  The only collective is the barrier between the two halves of a
-pass; it is one small all-reduce that also sums the interaction totals and ORs the error flags.
+pass: one 8-byte all-reduce on the stream the context works on.
 
 This module is host logic only: set-up (exchange of the IPC handles), the begin / barrier / end
 sequence, the reduced totals.  It drives any object with the ``Tree`` methods it names, so the
