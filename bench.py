@@ -312,8 +312,10 @@ def run_ours(args):
         flops = effective_flops(pp_tot, pc_tot)
         ach = flops / (phase_ms["walk"] * 1e-3) / 1e12
         traffic, traffic_src = _ncu_traffic(cfg["name"])
+        peak_meas = t.fp32_peak()  # register-only FFMA kernel, run now on this GPU
         roof = {"bound": "alu", "kernel": "walk_force_kernel", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
-                "frac": ach / peak, "traffic": traffic, "traffic_unit": "bytes of DRAM read+write per launch",
+                "frac": ach / peak, "peak_measured": peak_meas, "frac_of_measured": ach / peak_meas if peak_meas else None,
+                "traffic": traffic, "traffic_unit": "bytes of DRAM read+write per launch",
                 "traffic_source": traffic_src,
                 "peak_source": f"derived: {props.multi_processor_count} SMs x 128 FP32 lanes x 2 x 1.965 GHz "
                                "(MEASURED_PEAKS.json has no FP32 figure)",

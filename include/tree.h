@@ -186,6 +186,11 @@ int tree_leapfrog_end(tree_ctx *t);
  * pass, to HOST memory (any pointer may be NULL).  Synchronises. */
 int tree_shard_range(tree_ctx *t, long long *g_lo, long long *g_hi, long long *s_lo, long long *s_hi);
 
+/* Measurement aid: the FP32 FMA rate in TFLOP/s this GPU sustains on register operands
+ * (a short register-only FFMA kernel, best of 3), written to a HOST double: the measured denominator
+ * reported beside the nominal FP32 peak in the roofline of the fused walk+force kernel.  Synchronises. */
+int tree_fp32_peak(tree_ctx *t, double *tflops);
+
 /* Number of kernels this library launched on the context since tree_create (for accounting). */
 long long tree_launch_count(const tree_ctx *t);
 

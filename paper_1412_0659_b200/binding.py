@@ -49,6 +49,7 @@ _SIGS = {
     "tree_leapfrog_begin": (C.c_int, [C.c_void_p, C.c_float]),
     "tree_leapfrog_end": (C.c_int, [C.c_void_p]),
     "tree_shard_range": (C.c_int, [C.c_void_p] + [C.POINTER(C.c_longlong)] * 4),
+    "tree_fp32_peak": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
     "tree_launch_count": (C.c_longlong, [C.c_void_p]),
     "tree_last_error": (C.c_char_p, [C.c_void_p]),
 }
@@ -244,6 +245,12 @@ class Tree:
         pp, pc = C.c_ulonglong(0), C.c_ulonglong(0)
         _check(self.h, load_library().tree_get_stats(self.h, ms, C.byref(pp), C.byref(pc)))
         return dict(zip(PHASES, list(ms))), int(pp.value), int(pc.value)
+
+    def fp32_peak(self) -> float:
+        """Measured register-operand FFMA rate of this GPU in TFLOP/s (tree_fp32_peak)."""
+        v = C.c_double(0)
+        _check(self.h, load_library().tree_fp32_peak(self.h, C.byref(v)))
+        return v.value
 
     def launch_count(self) -> int:
         return int(load_library().tree_launch_count(self.h))

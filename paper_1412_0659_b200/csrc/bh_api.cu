@@ -651,6 +651,13 @@ int tree_get_stats(tree_ctx *t, double *ms, unsigned long long *n_pp, unsigned l
   return TREE_OK;
 }
 
+int tree_fp32_peak(tree_ctx *t, double *tflops) {
+  if (!t) return TREE_ERR_ARG;
+  if (!tflops) return set_err(t, TREE_ERR_ARG, "tree_fp32_peak: NULL");
+  BH_CUDA(cudaSetDevice(t->device));
+  return run_fp32_peak(t, tflops);
+}
+
 long long tree_launch_count(const tree_ctx *t) { return t ? t->launches : 0; }
 
 const char *tree_last_error(const tree_ctx *t) { return t ? t->err.c_str() : ""; }

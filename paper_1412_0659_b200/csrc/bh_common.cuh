@@ -158,6 +158,7 @@ int run_energy(tree_ctx *t);
 int run_set_velocity(tree_ctx *t, const float *vel);
 int run_get_state(tree_ctx *t, float *pos, float *vel, float *acc, float *pot);
 int run_direct(tree_ctx *t, const long long *idx, long long n, float eps, double *acc, double *pot);
+int run_fp32_peak(tree_ctx *t, double *tflops);
 int ensure_cells(tree_ctx *t, long long n_cells);
 void build_hilbert_lut(uint8_t out[24 * 8]);
 int device_excl_scan(tree_ctx *t, uint32_t *a, long long n, uint32_t *total_out);

@@ -1003,6 +1003,55 @@ __global__ void __launch_bounds__(DIRECT_THREADS) direct_kernel(const float4 *__
 }
 
 // ------------------------------------------------------------------------------------------
+// Measurement aid: the FP32 FMA rate this GPU sustains on register operands, the measured
+// denominator beside the nominal peak of the roofline.  Eight independent FFMA chains per thread with one
+// fresh register operand each (multiplier and addend repeat, so they come from the operand-reuse cache /
+// immediates): the form that reaches one FFMA per clock and scheduler.
+// ------------------------------------------------------------------------------------------
+constexpr int PEAK_THREADS = 256, PEAK_CHAINS = 8, PEAK_UNROLL = 32;
+__global__ void __launch_bounds__(PEAK_THREADS) fp32_peak_kernel(float *out, int iters, float mul, float add) {
+  float a[PEAK_CHAINS];
+#pragma unroll
+  for (int k = 0; k < PEAK_CHAINS; ++k) a[k] = (float)(threadIdx.x + k) * 1e-3f;
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int u = 0; u < PEAK_UNROLL; ++u) {
+#pragma unroll
+      for (int k = 0; k < PEAK_CHAINS; ++k) a[k] = fmaf(a[k], mul, add);
+    }
+  }
+  float s = 0.f;
+#pragma unroll
+  for (int k = 0; k < PEAK_CHAINS; ++k) s += a[k];
+  if (s == 123.456f) out[0] = s;  // never true for these inputs; keeps the chains alive
+}
+
+int run_fp32_peak(tree_ctx *t, double *tflops) {
+  cudaEvent_t e0, e1;
+  BH_CUDA(cudaEventCreate(&e0));
+  BH_CUDA(cudaEventCreate(&e1));
+  const int blocks = t->sm_count * 8, iters = 2048;
+  float *sink = reinterpret_cast<float *>(t->d_hlut);  // never written (see the kernel)
+  double best = 0.0;
+  for (int rep = 0; rep < 4; ++rep) {  // first repetition warms up
+    cudaEventRecord(e0, t->stream);
+    fp32_peak_kernel<<<blocks, PEAK_THREADS, 0, t->stream>>>(sink, iters, 0.999999f, 1e-7f);
+    cudaEventRecord(e1, t->stream);
+    cudaError_t e = cudaEventSynchronize(e1);
+    if (e != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); return set_err(t, TREE_ERR_CUDA, "fp32_peak", e); }
+    t->launches++;
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    const double flop = 2.0 * PEAK_CHAINS * PEAK_UNROLL * (double)iters * PEAK_THREADS * (double)blocks;
+    if (rep > 0 && ms > 0.f) best = fmax(best, flop / (ms * 1e-3) / 1e12);
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  *tflops = best;
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------
 // host launchers
 // ------------------------------------------------------------------------------------------
 static inline unsigned blocks_for(long long n, int threads) { return (unsigned)((n + threads - 1) / threads); }

@@ -214,3 +214,14 @@ def test_clumpy_disk_full_parity():
     assert ot.cells()[:, 0].max() >= 12  # the clumps do deepen the tree
     ms, pp, pc = t.stats()  # raises if the walk stack guard fired
     t.close()
+
+
+def test_fp32_peak_probe_is_plausible():
+    """tree_fp32_peak (measured denominator of the roofline): a register-only FFMA kernel must land
+    near SMs x 128 lanes x 2 x clock; far below means the probe is broken, above is impossible."""
+    t = Tree(device=0)
+    v = t.fp32_peak()
+    props = torch.cuda.get_device_properties(0)
+    nominal = props.multi_processor_count * 128 * 2 * 1.965e9 / 1e12
+    assert 0.7 * nominal < v <= 1.03 * nominal, (v, nominal)
+    t.close()
