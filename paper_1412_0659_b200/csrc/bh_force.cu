@@ -1030,7 +1030,7 @@ int run_fp32_peak(tree_ctx *t, double *tflops) {
   cudaEvent_t e0, e1;
   BH_CUDA(cudaEventCreate(&e0));
   BH_CUDA(cudaEventCreate(&e1));
-  const int blocks = t->sm_count * 8, iters = 2048;
+  const int blocks = t->sm_count * 8, iters = 512;
   float *sink = reinterpret_cast<float *>(t->d_hlut);  // never written (see the kernel)
   double best = 0.0;
   for (int rep = 0; rep < 4; ++rep) {  // first repetition warms up
