@@ -703,7 +703,10 @@ __global__ void __launch_bounds__(256) moments_top_kernel(int ltop, const DevInf
 // ------------------------------------------------------------------------------------------
 // host launchers
 // ------------------------------------------------------------------------------------------
-constexpr int MOMENTS_TOP_CELLS = 2048;
+#ifndef BH_MOMENTS_TOP_CELLS
+#define BH_MOMENTS_TOP_CELLS 128
+#endif
+constexpr int MOMENTS_TOP_CELLS = BH_MOMENTS_TOP_CELLS;  // levels 0..ltop with at most this many cells in total: one block
 
 static inline int grid_for(tree_ctx *t, long long n, int threads, int per_sm) {
   long long need = (n + threads - 1) / threads;

@@ -57,6 +57,11 @@ __global__ void __launch_bounds__(256) opening_kernel(long long n_cells, const D
 constexpr int PP_UNROLL = BH_PP_UNROLL, PC_UNROLL = BH_PC_UNROLL;  // sources per unrolled evaluator loop body
 constexpr int WALK_WARPS = 4;
 constexpr int WALK_MINB = BH_WALK_MINB;  // resident blocks per SM the register budget is sized for
+#ifndef BH_WALK_MINB4
+#define BH_WALK_MINB4 3
+#endif
+// four targets per lane (group 128) keep twice the per-target state in registers: fewer, fatter blocks
+constexpr int walk_minb(int tpl) { return tpl >= 4 ? BH_WALK_MINB4 : WALK_MINB; }
 constexpr int COUNT_MINB = 8;            // same for the counting pre-pass (38 registers; shared memory allows 8 blocks)
 #ifndef BH_COUNT_TRUNC
 #define BH_COUNT_TRUNC 256
@@ -578,7 +583,7 @@ __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, con
 }
 
 template <int TPL, bool COUNT>
-__global__ void __launch_bounds__(WALK_WARPS * 32, COUNT ? COUNT_MINB : WALK_MINB) walk_force_kernel(const WalkParams P) {
+__global__ void __launch_bounds__(WALK_WARPS * 32, COUNT ? COUNT_MINB : walk_minb(TPL)) walk_force_kernel(const WalkParams P) {
   __shared__ WarpSmem smem[WALK_WARPS];
   WarpSmem &ws = smem[threadIdx.x >> 5];
   const int lane = threadIdx.x & 31;
@@ -1127,7 +1132,7 @@ int run_walk(tree_ctx *t, float eps) {
   walk_reset_kernel<<<1, 32, 0, t->stream>>>(t->d_info, (unsigned)t->n_groups);
   BH_LAUNCH_CHECK("walk_reset");
   long long want = (t->n_groups + WALK_WARPS - 1) / WALK_WARPS;
-  long long cap = (long long)t->sm_count * WALK_MINB;
+  long long cap = (long long)t->sm_count * walk_minb(t->group / 32);
   unsigned grid = (unsigned)(want < cap ? want : cap);
   if (t->ev_valid[EV_OPEN]) cudaEventRecord(t->ev[EV_OPEN], t->stream);
   int rc;
