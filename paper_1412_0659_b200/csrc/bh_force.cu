@@ -64,7 +64,7 @@ constexpr int WALK_MINB = BH_WALK_MINB;  // resident blocks per SM the register 
 constexpr int walk_minb(int tpl) { return tpl >= 4 ? BH_WALK_MINB4 : WALK_MINB; }
 constexpr int COUNT_MINB = 8;            // same for the counting pre-pass (38 registers; shared memory allows 8 blocks)
 #ifndef BH_COUNT_TRUNC
-#define BH_COUNT_TRUNC 256
+#define BH_COUNT_TRUNC 1024
 #endif
 constexpr unsigned COUNT_TRUNC = BH_COUNT_TRUNC;  // the counting walk treats cells this small as opened leaves
 constexpr int FOLD_EVERY = 4;    // tiles (of 32 sources) summed in plain FP32 between compensated folds
