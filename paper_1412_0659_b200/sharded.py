@@ -43,10 +43,17 @@ class ShardedTree:
             mine = t.shard_export()
             handles = [None] * self.world
             dist.all_gather_object(handles, mine, group=self.group)
-            for r, h in enumerate(handles):
-                if r != self.rank:
-                    t.shard_attach(r, h)
-            self._barrier()  # nobody starts a pass before everybody has attached
+            err = None
+            try:
+                for r, h in enumerate(handles):
+                    if r != self.rank:
+                        t.shard_attach(r, h)
+            except Exception as e:  # e.g. GPUs that are not peer-capable
+                err = e
+            # every rank learns whether all attached (also: nobody starts a pass before everybody has attached)
+            if self._sum([0 if err else 1])[0] != self.world:
+                t.shard_config(0, 1)
+                raise RuntimeError(f"sharded set-up failed on at least one rank (this rank: {err})")
         self.connected = True
 
     # -- the exchange step: one all-reduce, enqueued on the stream the context works on.  It carries no
