@@ -152,3 +152,41 @@ def test_sharded_call_order_errors():
     t.force_end(acc2)
     assert torch.equal(acc, acc2)
     t.close()
+
+
+def test_sharded_bench_size_config2_sampled_against_oracle():
+    """BASELINE config 2 (Plummer N = 1,048,576), the size `bench.py --sharded` runs, on 4 contexts: interaction counts of
+    every group equal the single-context pass (itself compared with the oracle at this size in
+    test_bench_size_sampled_parity_config2); forces against the oracle on every 64th group within 1e-5."""
+    from nbody_inputs import config
+    cfg, pos, vel, mass = config(1, with_vel=False)
+    n, world = cfg["n"], 4
+    dpos, dmass = pos.cuda(), mass.cuda()
+    single = Tree(device=0)
+    single.build(dpos, dmass); single.force(cfg["theta"], cfg["eps"])
+    ref_cnt = single.debug("counts")
+    single.close()
+    trees = _make(world, n)
+    acc = torch.zeros((n, 3), device="cuda"); pot = torch.zeros(n, device="cuda")
+    for t in trees:
+        t.build(dpos, dmass)
+    force_local(trees, cfg["theta"], cfg["eps"], [(acc, pot)] + [(None, None)] * (world - 1))
+    torch.cuda.synchronize()
+    ranges = [t.shard_range() for t in trees]
+    assert ranges[0][0] == 0 and ranges[-1][1] == (n + 63) // 64
+    assert all(a[1] == b[0] for a, b in zip(ranges[:-1], ranges[1:]))
+    assert min(r[1] - r[0] for r in ranges) > 0
+    for t in trees:
+        assert np.array_equal(t.debug("counts"), ref_cnt)
+    ot = oracle.Tree(pos.numpy(), mass.numpy())
+    _, order, _ = ot.keys()
+    stride = 64
+    oacc, opot, onpp, onpc = ot.force(cfg["theta"], cfg["eps"], g0=7, stride=stride)
+    gsel = np.arange(7, ot.n_groups, stride)
+    assert np.array_equal(ref_cnt[gsel, 0], onpp[gsel]) and np.array_equal(ref_cnt[gsel, 1], onpc[gsel])
+    sel = np.concatenate([order[64 * g: 64 * g + 64] for g in gsel])
+    a = acc.cpu().numpy().astype(np.float64)[sel]; p = pot.cpu().numpy().astype(np.float64)[sel]
+    rel = np.linalg.norm(a - oacc[sel], axis=1) / np.linalg.norm(oacc[sel], axis=1)
+    assert rel.max() <= TOL, rel.max()
+    assert (np.abs(p - opot[sel]) / np.abs(opot[sel])).max() <= TOL
+    _close(trees)
