@@ -513,6 +513,11 @@ __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, con
   fold_tile<TPL>(T, R);
   if (prefix && part != 0) { n_pp = 0; n_pc = 0; }  // walk ended inside the prefix: counted by part 0
   if (lane == 0) {
+    unsigned long long t_end;
+    unsigned smid;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_end));
+    asm volatile("mov.u32 %0, %smid;" : "=r"(smid));
+    const unsigned dur = (unsigned)(t_end - t_start);
     if (nparts == 1) {
       P.gcount[g] = make_uint2(n_pp, n_pc);
       for (int q = 0; q < P.n_peers; ++q) P.peer_gcount[q][g] = make_uint2(n_pp, n_pc);
@@ -522,11 +527,7 @@ __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, con
     }
     atomicAdd(&P.info->n_pp, (unsigned long long)n_pp * gsize);
     atomicAdd(&P.info->n_pc, (unsigned long long)n_pc * gsize);
-    unsigned long long t_end;
-    unsigned smid;
-    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_end));
-    asm volatile("mov.u32 %0, %smid;" : "=r"(smid));
-    P.trace[item] = make_uint4((unsigned)(t_start - P.info->t0_ns), (unsigned)(t_end - t_start), smid, P.tasks[item]);
+    P.trace[item] = make_uint4((unsigned)(t_start - P.info->t0_ns), dur, smid, P.tasks[item]);
   }
   // ---- results
   float4 res[TPL];
@@ -624,6 +625,10 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, COUNT ? COUNT_MINB : walk_min
 constexpr double SPLIT_FINE = BH_SPLIT_FINE;  // parts per mean-cost unit of an expensive group
 constexpr double SPLIT_AT = BH_SPLIT_AT;      // a group is expensive above this multiple of the mean cost
 constexpr unsigned MAX_PARTS = 63;
+#ifndef BH_SUSPECT_AT
+#define BH_SUSPECT_AT 3.0
+#endif
+constexpr double SUSPECT_AT = BH_SUSPECT_AT;  // a run's box diagonal against its neighbours' (task_cost_kernel)
 #ifndef BH_TAIL_PER_SM
 #define BH_TAIL_PER_SM 16
 #endif
@@ -647,8 +652,8 @@ __device__ __forceinline__ double prev_cost(const uint2 *__restrict__ gcount, un
   return 13.0 * (double)c.x + 37.0 * (double)c.y;
 }
 
-// Cost estimate of every group for this pass: the counting walk's (left in gdone), or -- tree_leapfrog,
-// the same particles one step later -- the exact counts of the previous pass (the neighbours cover a
+// Cost estimate of every group for this pass (unit: 13 n_pp + 37 n_pc): the counting walk's (left in gdone), or --
+// tree_leapfrog, the same particles one step later -- the exact counts of the previous pass (the neighbours cover a
 // shift of the runs by up to two); in that case their sum is formed here.
 __global__ void __launch_bounds__(256) group_cost_kernel(unsigned n_groups, DevInfo *info, const uint32_t *__restrict__ gdone,
                                                          const uint2 *__restrict__ prev, double *__restrict__ gcost) {
@@ -799,7 +804,7 @@ __device__ __forceinline__ TailPlan tail_plan(const DevInfo *info, const TailLim
 __global__ void __launch_bounds__(256) task_cost_kernel(unsigned n_groups, const DevInfo *__restrict__ info,
                                                         uint32_t *__restrict__ a_cnt, uint32_t *__restrict__ gdone,
                                                         uint32_t *__restrict__ gthresh, const double *__restrict__ gcost,
-                                                        const TailLimits lim) {
+                                                        const float *__restrict__ suspect_gbox, const TailLimits lim) {
   unsigned g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= n_groups) return;
   const unsigned tail_parts = tail_plan(info, lim).parts;
@@ -811,6 +816,22 @@ __global__ void __launch_bounds__(256) task_cost_kernel(unsigned n_groups, const
     double want = ceil(SPLIT_FINE * cost / mean);
     s = want > (double)MAX_PARTS ? MAX_PARTS : (unsigned)want;
     if (s < 2) s = 0;
+  }
+  // The previous pass's counts (suspect_gbox != nullptr) cannot predict a group that has just become expensive: when
+  // a far particle joins a run of 64, its box suddenly spans a dense region (measured at N = 33 M: 85 k -> 1.7 M cost
+  // units from one step to the next, three such groups among 65 k, each a 5-7 ms task that ended one rank's kernel
+  // 3-5 ms after the others on 8 ranks).  Such a run shows in its box: a diagonal more than SUSPECT_AT x the mean of
+  // its four neighbours'.  It is listed at the front as one task, where its length cannot delay the end.
+  if (mine && s == 0 && suspect_gbox && n_groups >= 5) {
+    auto diag = [&](unsigned q) {
+      const float *b = suspect_gbox + 6ull * q;
+      const float dx = b[3] - b[0], dy = b[4] - b[1], dz = b[5] - b[2];
+      return sqrtf(dx * dx + dy * dy + dz * dz);
+    };
+    const unsigned c = g < 2 ? 2u : (g + 2 >= n_groups ? n_groups - 3 : g);  // window centre kept inside the array
+    float sum = 0.f;
+    for (unsigned q = c - 2; q <= c + 2; ++q) if (q != g) sum += diag(q);
+    if (diag(g) > (float)SUSPECT_AT * 0.25f * sum) s = 1;
   }
   a_cnt[g] = s;
   gdone[g] = 0;
@@ -1095,7 +1116,8 @@ static int launch_walk(tree_ctx *t, const WalkParams &P, unsigned grid) {
   // 2. task list of this context's range: split expensive groups, longest work first
   TailLimits lim;
   lim.n_tail_max = (unsigned)std::min<long long>(TAIL_PER_SM * t->sm_count, t->tail_cap / (long long)TAIL_PARTS);
-  task_cost_kernel<<<gb, 256, 0, t->stream>>>(ng, info, t->b.sched_a, t->b.gdone, t->b.gthresh, t->b.gcost, lim);
+  task_cost_kernel<<<gb, 256, 0, t->stream>>>(ng, info, t->b.sched_a, t->b.gdone, t->b.gthresh, t->b.gcost,
+                                              reuse ? t->b.gbox : nullptr, lim);
   BH_LAUNCH_CHECK("task_cost");
   int rc = device_excl_scan(t, t->b.sched_a, ng, tot);
   if (rc) return rc;
