@@ -611,8 +611,10 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, COUNT ? COUNT_MINB : walk_min
 
 // ------------------------------------------------------------------------------------------
 // Task list (scheduling only; results depend on it only through the fixed-order partial sums).
-// cost(g) = 13 n_pp + 37 n_pc, estimated by the truncated counting walk. Task list layout:
-//   head : parts of EXPENSIVE groups (cost > 2 x mean: s = ceil(cost / mean) parts), longest first
+// cost(g) = 13 n_pp + 37 n_pc, estimated by the truncated counting walk or taken from the previous pass's exact
+// counts (tree_leapfrog). Task list of the groups this context walks (all of them unless the pass is sharded):
+//   head : parts of EXPENSIVE groups (cost > 2 x mean over all groups: s = ceil(cost / mean) parts) and, as single
+//          tasks, SUSPECT runs whose cost the previous pass cannot know (task_cost_kernel); they start first
 //   body : one task per ordinary group, in Peano-Hilbert order (L1/L2 locality between warps)
 //   tail : the last n_tail groups, TAIL_PARTS parts each, so that the kernel ends on small tasks
 // ------------------------------------------------------------------------------------------
@@ -640,7 +642,7 @@ __global__ void walk_reset_kernel(DevInfo *info, unsigned n_groups) {
     info->group_ticket = 0; info->task_ticket = 0; info->n_pp = 0; info->n_pc = 0; info->n_tasks = 0;
     info->sched_cost = 0;  // summed by the counting walk, or by group_cost_kernel from the previous pass's counts
     info->walk_overflow = 0;
-    info->g_lo = 0; info->g_hi = n_groups;  // narrowed by shard_partition_kernel in a sharded pass
+    info->g_lo = 0; info->g_hi = n_groups;  // narrowed by shard_bounds_kernel in a sharded pass
     unsigned long long now;
     asm volatile("mov.u64 %0, %globaltimer;" : "=l"(now));
     info->t0_ns = now;
