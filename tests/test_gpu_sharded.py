@@ -78,6 +78,27 @@ def test_sharded_pass_equals_oracle_on_every_rank(model, n, seed, world):
     _close(trees)
 
 
+@pytest.mark.parametrize("leaf,group", [(16, 32), (8, 128)])
+def test_sharded_pass_other_group_and_leaf_sizes(leaf, group):
+    n, theta, eps, world = 25013, 0.5, 0.02, 3
+    pos, _, mass = plummer(n, 17, with_vel=False)
+    trees = _make(world, n, leaf=leaf, group=group)
+    acc = torch.zeros((n, 3), device="cuda"); pot = torch.zeros(n, device="cuda")
+    for t in trees:
+        t.build(pos.cuda(), mass.cuda())
+    force_local(trees, theta, eps, [(acc, pot)] + [(None, None)] * (world - 1))
+    torch.cuda.synchronize()
+    ot = oracle.Tree(pos.numpy(), mass.numpy(), leaf_size=leaf, group_size=group)
+    oacc, opot, onpp, onpc = ot.force(theta, eps)
+    for t in trees:
+        cnt = t.debug("counts")
+        assert np.array_equal(cnt[:, 0], onpp) and np.array_equal(cnt[:, 1], onpc)
+    a = acc.cpu().numpy().astype(np.float64); p = pot.cpu().numpy().astype(np.float64)
+    assert (np.linalg.norm(a - oacc, axis=1) / np.linalg.norm(oacc, axis=1)).max() <= TOL
+    assert (np.abs(p - opot) / np.abs(opot)).max() <= TOL
+    _close(trees)
+
+
 def test_sharded_leapfrog_matches_single_context_and_ranks_agree_bitwise():
     n, theta, eps, dt, steps, world = 30011, 0.4, 0.01, 1e-3, 4, 3
     pos, vel, mass = plummer(n, 21)
