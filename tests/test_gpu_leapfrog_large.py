@@ -186,3 +186,43 @@ def test_full_size_sampled_parity_config3():
     assert rel.max() <= 1e-5, rel.max()
     assert (np.abs(p - opot[sel]) / np.abs(opot[sel])).max() <= 1e-5
     t.close()
+
+
+def test_leapfrog_suspect_runs_are_listed_first_and_results_stay_exact():
+    # A run of 64 sorted particles that catches a far particle has a box spanning a dense region and a cost the
+    # previous pass's counts do not predict; in leapfrog steps such runs (box diagonal > 3 x their neighbours') are
+    # listed at the front of the task list as single tasks.  Scheduling only: counts stay
+    # bit-exact and forces within 1e-5 of the oracle on the step's positions.
+    n0, theta, eps, dt = 60_000, 0.4, 0.01, 0.001
+    pos, vel, mass = plummer(n0, 77)
+    # every 1250th particle of the cluster is moved out to r = 30 in a seeded random direction: in Peano-Hilbert
+    # order these few particles are neighbours of runs that lie far from them
+    idx = torch.arange(0, n0, 1250)
+    d = torch.randn(len(idx), 3, generator=torch.Generator().manual_seed(5), dtype=torch.float64)
+    pos[idx] = (30.0 * d / d.norm(dim=1, keepdim=True)).float()
+    n = mass.numel()
+    t = Tree(device=0)
+    t.build(pos.cuda(), mass.cuda()); t.set_velocity(vel.cuda()); t.force(theta, eps)
+    for _ in range(2):
+        t.leapfrog(dt)
+    p, v, a, ph = _state(t, n)
+    ot = oracle.Tree(p, mass.numpy())
+    oacc, opot, onpp, onpc = ot.force(theta, eps)
+    cnt = t.debug("counts")
+    assert np.array_equal(cnt[:, 0], onpp) and np.array_equal(cnt[:, 1], onpc)
+    rel = np.linalg.norm(a.astype(np.float64) - oacc, axis=1) / np.linalg.norm(oacc, axis=1)
+    assert rel.max() <= 1e-5 and (np.abs(ph - opot) / np.abs(opot)).max() <= 1e-5
+    # the task list: head (expensive and suspect groups, by group id), then the body by group id
+    tr = t.debug("task_trace")
+    gid = (tr[:, 3] & ((1 << 26) - 1)).astype(np.int64); part = tr[:, 3] >> 26
+    desc = np.nonzero(np.diff(gid) < 0)[0]
+    assert len(desc) >= 1
+    head = slice(0, desc[0] + 1)
+    hg, hc = np.unique(gid[head], return_counts=True)
+    singles = hg[hc == 1]
+    assert len(singles) >= 1, "no single-task (suspect) group at the front of the list"
+    gb = t.debug("group_boxes"); diag = np.linalg.norm(gb[:, 3:] - gb[:, :3], axis=1)
+    s = singles[(singles >= 2) & (singles < len(diag) - 2)]
+    nb = (diag[s - 2] + diag[s - 1] + diag[s + 1] + diag[s + 2]) / 4
+    assert (diag[s] > 3.0 * nb).any()
+    t.close()
