@@ -67,7 +67,10 @@ constexpr int COUNT_MINB = 8;            // same for the counting pre-pass (38 r
 #define BH_COUNT_TRUNC 1024
 #endif
 constexpr unsigned COUNT_TRUNC = BH_COUNT_TRUNC;  // the counting walk treats cells this small as opened leaves
-constexpr int FOLD_EVERY = 4;    // tiles (of 32 sources) summed in plain FP32 between compensated folds
+#ifndef BH_FOLD_EVERY
+#define BH_FOLD_EVERY 2
+#endif
+constexpr int FOLD_EVERY = BH_FOLD_EVERY;  // tiles (of 32 sources) summed in plain FP32 between compensated folds
 constexpr int DEFER_CAP = 256;   // deferred child ranges one part of a split group may own
 constexpr int STACK_CAP = 1024;  // >= 32 per level (depth-first: 32 x 22) + DEFER_CAP
 
@@ -118,13 +121,16 @@ struct Targets {
   uint32_t slot[TPL];
 };
 
-// Running totals as unevaluated (hi, lo) pairs: each tile's partial sum is folded in with an
-// error-free two-sum, so the FP32 result does not drift with the list length (S14).
-template <int TPL>
-struct Totals {
-  float hi[4][TPL], lo[4][TPL];
-};
-
+// Running totals (S14).  The per-lane FP32 sums over the last FOLD_EVERY tiles are folded into
+// totals that do not drift with the list length: FP64 accumulators (one conversion + one DADD per value; the
+// FP64 pipe of sm_100a is otherwise idle here), or with BH_FOLD_F64 = 0 unevaluated FP32 (hi, lo) pairs
+// updated by an error-free two-sum (7 FADD per value).
+#ifndef BH_FOLD_F64
+#define BH_FOLD_F64 0
+#endif
+#ifndef BH_FOLD_PLAIN_POT
+#define BH_FOLD_PLAIN_POT 1
+#endif
 __device__ __forceinline__ void two_sum_fold(float &hi, float &lo, float x) {
   float s = __fadd_rn(hi, x);
   float bb = __fsub_rn(s, hi);
@@ -133,14 +139,50 @@ __device__ __forceinline__ void two_sum_fold(float &hi, float &lo, float x) {
   lo = __fadd_rn(lo, e);
 }
 
+#if BH_FOLD_F64
+template <int TPL>
+struct Totals {
+  double s[4][TPL];
+  __device__ __forceinline__ void clear() {
+#pragma unroll
+    for (int t = 0; t < TPL; ++t)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) s[c][t] = 0.0;
+  }
+  __device__ __forceinline__ void add(int c, int t, float x) { s[c][t] += (double)x; }
+  __device__ __forceinline__ void add_same_sign(int t, float x) { s[3][t] += (double)x; }
+  __device__ __forceinline__ float get(int c, int t) const { return (float)s[c][t]; }
+};
+#else
+template <int TPL>
+struct Totals {
+  float hi[4][TPL], lo[4][TPL];
+  __device__ __forceinline__ void clear() {
+#pragma unroll
+    for (int t = 0; t < TPL; ++t)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) { hi[c][t] = 0.0f; lo[c][t] = 0.0f; }
+  }
+  __device__ __forceinline__ void add(int c, int t, float x) { two_sum_fold(hi[c][t], lo[c][t], x); }
+  // the potential is a sum of terms of one sign (the quadrupole part is a small correction): no cancellation, so a
+  // plain FP32 total over the folds (one rounding per fold, random sign) stays below 1e-6 relative
+#if BH_FOLD_PLAIN_POT
+  __device__ __forceinline__ void add_same_sign(int t, float x) { hi[3][t] = __fadd_rn(hi[3][t], x); }
+#else
+  __device__ __forceinline__ void add_same_sign(int t, float x) { two_sum_fold(hi[3][t], lo[3][t], x); }
+#endif
+  __device__ __forceinline__ float get(int c, int t) const { return __fadd_rn(hi[c][t], lo[c][t]); }
+};
+#endif
+
 template <int TPL>
 __device__ __forceinline__ void fold_tile(Targets<TPL> &T, Totals<TPL> &R) {
 #pragma unroll
   for (int t = 0; t < TPL; ++t) {
-    two_sum_fold(R.hi[0][t], R.lo[0][t], T.ax[t]);
-    two_sum_fold(R.hi[1][t], R.lo[1][t], T.ay[t]);
-    two_sum_fold(R.hi[2][t], R.lo[2][t], T.az[t]);
-    two_sum_fold(R.hi[3][t], R.lo[3][t], fmaf(-0.2f, T.phq[t], T.ph[t]));
+    R.add(0, t, T.ax[t]);
+    R.add(1, t, T.ay[t]);
+    R.add(2, t, T.az[t]);
+    R.add_same_sign(t, fmaf(-0.2f, T.phq[t], T.ph[t]));
     T.ax[t] = T.ay[t] = T.az[t] = T.ph[t] = T.phq[t] = 0.0f;
   }
 }
@@ -336,11 +378,7 @@ __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, con
   const unsigned gsize = rem < (long long)GS ? (unsigned)rem : GS;
   Targets<TPL> T;
   Totals<TPL> R;
-#pragma unroll
-  for (int t = 0; t < TPL; ++t) {
-#pragma unroll
-    for (int c = 0; c < 4; ++c) { R.hi[c][t] = 0.0f; R.lo[c][t] = 0.0f; }
-  }
+  R.clear();
 #pragma unroll
   for (int t = 0; t < TPL; ++t) {
     unsigned j = lane + 32u * t;
@@ -533,8 +571,7 @@ __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, con
   float4 res[TPL];
 #pragma unroll
   for (int t = 0; t < TPL; ++t)
-    res[t] = make_float4(__fadd_rn(R.hi[0][t], R.lo[0][t]), __fadd_rn(R.hi[1][t], R.lo[1][t]),
-                         __fadd_rn(R.hi[2][t], R.lo[2][t]), __fadd_rn(R.hi[3][t], R.lo[3][t]));
+    res[t] = make_float4(R.get(0, t), R.get(1, t), R.get(2, t), R.get(3, t));
   if (nparts == 1) {
 #pragma unroll
     for (int t = 0; t < TPL; ++t) {
