@@ -225,3 +225,37 @@ def test_fp32_peak_probe_is_plausible():
     nominal = props.multi_processor_count * 128 * 2 * 1.965e9 / 1e12
     assert 0.7 * nominal < v <= 1.03 * nominal, (v, nominal)
     t.close()
+
+
+def test_error_recovery_out_of_memory_and_no_leak():
+    """Non-finite input and an impossible reservation return their codes and leave the context usable; creating and
+    destroying contexts returns all device memory."""
+    n = 5000
+    pos, vel, mass = plummer(n, 3)
+    t = Tree(device=0)
+    for bad_pos, bad_mass in [(pos.clone().index_put_((torch.tensor([17]), torch.tensor([1])), torch.tensor(float("nan"))), mass),
+                              (pos.clone().index_put_((torch.tensor([99]), torch.tensor([2])), torch.tensor(float("inf"))), mass),
+                              (pos, mass.clone().index_put_((torch.tensor([5]),), torch.tensor(float("nan"))))]:
+        with pytest.raises(TreeError) as e:
+            t.build(bad_pos.cuda(), bad_mass.cuda())
+        assert e.value.code == -5
+        with pytest.raises(TreeError) as e:
+            t.force(0.4, 0.01)
+        assert e.value.code == -4
+    with pytest.raises(TreeError) as e:
+        t.reserve(2**31 - 1)  # ~365 GB of particle buffers
+    assert e.value.code == -2
+    acc = torch.empty((n, 3), device="cuda"); pot = torch.empty(n, device="cuda")
+    t.build(pos.cuda(), mass.cuda()); t.force(0.4, 0.01, acc, pot)
+    torch.cuda.synchronize()
+    ot = oracle.Tree(pos.numpy(), mass.numpy())
+    _compare_force(t, acc.cpu().numpy().astype(np.float64), pot.cpu().numpy().astype(np.float64), ot, 0.4, 0.01)
+    t.close()
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]
+    for _ in range(10):
+        tt = Tree(device=0)
+        tt.build(pos.cuda(), mass.cuda()); tt.force(0.4, 0.01)
+        tt.close()
+    torch.cuda.synchronize()
+    assert abs(torch.cuda.mem_get_info()[0] - free0) < (64 << 20)
