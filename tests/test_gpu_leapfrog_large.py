@@ -226,3 +226,39 @@ def test_leapfrog_suspect_runs_are_listed_first_and_results_stay_exact():
     nb = (diag[s - 2] + diag[s - 1] + diag[s + 1] + diag[s + 2]) / 4
     assert (diag[s] > 3.0 * nb).any()
     t.close()
+
+
+def test_long_run_trajectory_and_energy_match_oracle_and_sharded_run():
+    # 60 KDK steps at N = 30,000: FP32 state advanced with fmaf from forces that differ from the oracle's by ~1e-6, so
+    # positions stay within a few ulp of the oracle's and the energy drift is the same; a 4-context sharded run of the
+    # same steps agrees with the single context to 1e-6 of the system size (the task lists differ: a few partial sums are
+    # ordered differently).
+    from paper_1412_0659_b200.sharded import connect_local, force_local, leapfrog_local
+    n, dt, theta, eps, steps = 30_000, 0.005, 0.4, 0.01, 60
+    pos, vel, mass = plummer(n, 9)
+    t = Tree(device=0)
+    t.build(pos.cuda(), mass.cuda()); t.set_velocity(vel.cuda()); t.force(theta, eps)
+    e0 = sum(t.energy())
+    for _ in range(steps):
+        t.leapfrog(dt)
+    e1 = sum(t.energy())
+    p, v, _, _ = _state(t, n)
+    op, ov, oa, oph, en = oracle.leapfrog(pos.numpy(), vel.numpy(), mass.numpy(), dt, steps, theta, eps)
+    scale = np.abs(op).max()
+    assert np.abs(p - op).max() <= 1e-6 * scale and np.abs(v - ov).max() <= 1e-5 * np.abs(ov).max()
+    drift_gpu = abs(e1 - e0) / abs(e0); drift_cpu = abs(en[-1].sum() - en[0].sum()) / abs(en[0].sum())
+    assert drift_gpu < 1e-4 and abs(drift_gpu - drift_cpu) < 1e-6
+    trees = [Tree(device=0) for _ in range(4)]
+    for q in trees:
+        q.reserve(n)
+    connect_local(trees)
+    for q in trees:
+        q.build(pos.cuda(), mass.cuda()); q.set_velocity(vel.cuda())
+    force_local(trees, theta, eps)
+    for _ in range(steps):
+        leapfrog_local(trees, dt)
+    p2, _, _, _ = _state(trees[2], n)
+    assert np.abs(p2 - p).max() <= 1e-6 * scale
+    t.close()
+    for q in trees:
+        q.close()
