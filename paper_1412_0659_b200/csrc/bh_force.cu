@@ -7,12 +7,14 @@
 
 namespace bh {
 
-__device__ __forceinline__ unsigned warp_incl_scan_u(unsigned v, int lane) {
+// Inclusive scan over the warp.  shfl.up reports through its predicate whether the source lane exists, so each
+// step is SHFL + predicated IADD (the portable form needs a lane compare and a select per step as well).
+__device__ __forceinline__ unsigned warp_incl_scan_u(unsigned v, int /*lane*/) {
 #pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    unsigned n = __shfl_up_sync(0xffffffffu, v, o);
-    if (lane >= o) v += n;
-  }
+  for (int o = 1; o < 32; o <<= 1)
+    asm volatile("{ .reg .pred p; .reg .b32 r; shfl.sync.up.b32 r|p, %0, %1, 0, 0xffffffff; @p add.u32 %0, %0, r; }"
+                 : "+r"(v)
+                 : "r"(o));
   return v;
 }
 
@@ -522,6 +524,7 @@ __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, con
         if (++S.unfolded >= FOLD_EVERY) { fold_tile<TPL>(T, R); S.unfolded = 0; }
         __syncwarp();
       }
+      // (a ring buffer instead of this shift costs a register: the kernel then spills and runs 1.6 % slower)
       const unsigned mv = (lane + 32 < S.pc_pending) ? ws.pcq[lane + 32] : 0u;
       __syncwarp();
       ws.pcq[lane] = mv;
