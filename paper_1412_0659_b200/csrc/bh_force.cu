@@ -51,10 +51,13 @@ __global__ void __launch_bounds__(256) opening_kernel(long long n_cells, const D
 #define BH_WALK_MINB 5
 #endif
 #ifndef BH_PP_UNROLL
-#define BH_PP_UNROLL 8
+#define BH_PP_UNROLL 16
 #endif
 #ifndef BH_PC_UNROLL
 #define BH_PC_UNROLL 8
+#endif
+#ifndef BH_PACKED
+#define BH_PACKED 1
 #endif
 constexpr int PP_UNROLL = BH_PP_UNROLL, PC_UNROLL = BH_PC_UNROLL;  // sources per unrolled evaluator loop body
 constexpr int WALK_WARPS = 4;
@@ -252,8 +255,99 @@ __device__ __forceinline__ void pc_one(const float4 a, const float4 b, const flo
   }
 }
 
+// ------------------------------------------------------------------------------------------
+// Packed evaluators for two targets per lane (group size 64): sm_100a has FP32x2 instructions (FADD2 / FMUL2 /
+// FFMA2) that work on aligned register pairs and take a scalar register as a broadcast operand, so one instruction
+// serves both targets of a lane with the source operand read once.  Same operations in the same order as pp_one /
+// pc_one, each IEEE round-to-nearest: the results are bit-identical.  The pair operands are always spread over both
+// register-file banks, which is what the scalar form cannot arrange:
+// in isolation the p-c loop runs at 0.77 of the FP32 peak against 0.69 (micro-benchmark), with half the instructions.
+// ------------------------------------------------------------------------------------------
+typedef unsigned long long f32x2;  // (lo = target 0, hi = target 1)
+__device__ __forceinline__ f32x2 pk2(float lo, float hi) { f32x2 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ f32x2 bc2(float s) { return pk2(s, s); }
+__device__ __forceinline__ void up2(f32x2 v, float &lo, float &hi) { asm("mov.b64 {%0,%1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+
+struct Targets2 {  // the packed view of Targets<2> during one tile
+  f32x2 x, y, z, ax, ay, az, ph, phq;
+  __device__ __forceinline__ explicit Targets2(const Targets<2> &T)
+      : x(pk2(T.x[0], T.x[1])), y(pk2(T.y[0], T.y[1])), z(pk2(T.z[0], T.z[1])), ax(pk2(T.ax[0], T.ax[1])),
+        ay(pk2(T.ay[0], T.ay[1])), az(pk2(T.az[0], T.az[1])), ph(pk2(T.ph[0], T.ph[1])), phq(pk2(T.phq[0], T.phq[1])) {}
+  __device__ __forceinline__ void store(Targets<2> &T) const {
+    up2(ax, T.ax[0], T.ax[1]); up2(ay, T.ay[0], T.ay[1]); up2(az, T.az[0], T.az[1]);
+    up2(ph, T.ph[0], T.ph[1]); up2(phq, T.phq[0], T.phq[1]);
+  }
+};
+
+template <bool MASK>
+__device__ __forceinline__ void pp_one2(const float4 s, uint32_t sidx, const uint32_t (&slot)[2], Targets2 &T, f32x2 eps2) {
+  const f32x2 dx = sub2(bc2(s.x), T.x), dy = sub2(bc2(s.y), T.y), dz = sub2(bc2(s.z), T.z);
+  f32x2 r2 = fma2(dx, dx, eps2);
+  r2 = fma2(dy, dy, r2);
+  r2 = fma2(dz, dz, r2);
+  float r2a, r2b, m0 = s.w, m1 = s.w;
+  up2(r2, r2a, r2b);
+  if (MASK) {
+    if (sidx == slot[0]) { m0 = 0.0f; r2a = 1.0f; }
+    if (sidx == slot[1]) { m1 = 0.0f; r2b = 1.0f; }
+  }
+  const f32x2 ri = pk2(rsqrt_fast(r2a), rsqrt_fast(r2b));
+  const f32x2 ri2 = mul2(ri, ri);
+  const f32x2 mr = mul2(MASK ? pk2(m0, m1) : bc2(s.w), ri);
+  const f32x2 mr3 = mul2(mr, ri2);
+  T.ax = fma2(mr3, dx, T.ax);
+  T.ay = fma2(mr3, dy, T.ay);
+  T.az = fma2(mr3, dz, T.az);
+  T.ph = sub2(T.ph, mr);
+}
+
+// see pc_one for the formulas; a = (cx,cy,cz,M), b = 2.5 (Q'xx,Q'yy,Q'zz, tr(Q) eps^2), c = 2.5 (Q'xy,Q'xz,Q'yz)
+__device__ __forceinline__ void pc_one2(const float4 a, const float4 b, const float4 c, Targets2 &T, f32x2 eps2) {
+  const f32x2 dx = sub2(bc2(a.x), T.x), dy = sub2(bc2(a.y), T.y), dz = sub2(bc2(a.z), T.z);
+  f32x2 r2 = fma2(dx, dx, eps2);
+  r2 = fma2(dy, dy, r2);
+  r2 = fma2(dz, dz, r2);
+  float r2a, r2b;
+  up2(r2, r2a, r2b);
+  const f32x2 ri = pk2(rsqrt_fast(r2a), rsqrt_fast(r2b));
+  const f32x2 vx = fma2(bc2(c.y), dz, fma2(bc2(c.x), dy, mul2(bc2(b.x), dx)));
+  const f32x2 vy = fma2(bc2(c.z), dz, fma2(bc2(b.y), dy, mul2(bc2(c.x), dx)));
+  const f32x2 vz = fma2(bc2(b.z), dz, fma2(bc2(c.z), dy, mul2(bc2(c.y), dx)));
+  const f32x2 w = fma2(dz, vz, fma2(dy, vy, fma2(dx, vx, bc2(-b.w))));
+  const f32x2 ri2 = mul2(ri, ri);
+  const f32x2 ri3 = mul2(ri, ri2);
+  const f32x2 ri4 = mul2(ri2, ri2);
+  const f32x2 ri5 = mul2(ri3, ri2);
+  T.ph = fma2(bc2(-a.w), ri, T.ph);
+  T.phq = fma2(w, ri5, T.phq);
+  const f32x2 g = mul2(fma2(w, ri4, bc2(a.w)), ri3);
+  const f32x2 k = mul2(bc2(-0.4f), ri5);
+  T.ax = fma2(k, vx, fma2(g, dx, T.ax));
+  T.ay = fma2(k, vy, fma2(g, dy, T.ay));
+  T.az = fma2(k, vz, fma2(g, dz, T.az));
+}
+
 template <int TPL>
 __device__ __forceinline__ void eval_pp_tile(const WarpSmem &ws, int cnt, bool mask, Targets<TPL> &T, float eps2) {
+  if constexpr (TPL == 2 && BH_PACKED) {
+    Targets2 P2(T);
+    const f32x2 e2 = bc2(eps2);
+    const uint32_t slot[2] = {T.slot[0], T.slot[1]};
+    if (!mask && cnt == 32) {
+#pragma unroll(PP_UNROLL)
+      for (int j = 0; j < 32; ++j) pp_one2<false>(ws.pp[j], 0u, slot, P2, e2);
+    } else if (!mask) {
+      for (int j = 0; j < cnt; ++j) pp_one2<false>(ws.pp[j], 0u, slot, P2, e2);
+    } else {
+#pragma unroll 2
+      for (int j = 0; j < cnt; ++j) pp_one2<true>(ws.pp[j], ws.ppidx[j], slot, P2, e2);
+    }
+    P2.store(T);
+    return;
+  }
   if (!mask && cnt == 32) {
 #pragma unroll(PP_UNROLL)
     for (int j = 0; j < 32; ++j) pp_one<TPL, false>(ws.pp[j], 0u, T, eps2);
@@ -267,6 +361,18 @@ __device__ __forceinline__ void eval_pp_tile(const WarpSmem &ws, int cnt, bool m
 
 template <int TPL>
 __device__ __forceinline__ void eval_pc_tile(const WarpSmem &ws, int cnt, Targets<TPL> &T, float eps2) {
+  if constexpr (TPL == 2 && BH_PACKED) {
+    Targets2 P2(T);
+    const f32x2 e2 = bc2(eps2);
+    if (cnt == 32) {
+#pragma unroll(PC_UNROLL)
+      for (int j = 0; j < 32; ++j) pc_one2(ws.pc0[j], ws.pc1[j], ws.pc2[j], P2, e2);
+    } else {
+      for (int j = 0; j < cnt; ++j) pc_one2(ws.pc0[j], ws.pc1[j], ws.pc2[j], P2, e2);
+    }
+    P2.store(T);
+    return;
+  }
   if (cnt == 32) {
 #pragma unroll(PC_UNROLL)
     for (int j = 0; j < 32; ++j) pc_one<TPL>(ws.pc0[j], ws.pc1[j], ws.pc2[j], T, eps2);
