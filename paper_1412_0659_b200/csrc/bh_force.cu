@@ -56,9 +56,6 @@ __global__ void __launch_bounds__(256) opening_kernel(long long n_cells, const D
 #ifndef BH_PC_UNROLL
 #define BH_PC_UNROLL 8
 #endif
-#ifndef BH_PACKED
-#define BH_PACKED 1
-#endif
 constexpr int PP_UNROLL = BH_PP_UNROLL, PC_UNROLL = BH_PC_UNROLL;  // sources per unrolled evaluator loop body
 constexpr int WALK_WARPS = 4;
 constexpr int WALK_MINB = BH_WALK_MINB;  // resident blocks per SM the register budget is sized for
@@ -136,6 +133,20 @@ struct Targets {
 #ifndef BH_FOLD_PLAIN_POT
 #define BH_FOLD_PLAIN_POT 1
 #endif
+// FP32x2 register pairs (see "Packed evaluators" below)
+#ifndef BH_PACKED
+#define BH_PACKED 1
+#endif
+typedef unsigned long long f32x2;  // (lo = target 0, hi = target 1)
+__device__ __forceinline__ f32x2 pk2(float lo, float hi) { f32x2 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ f32x2 bc2(float s) { return pk2(s, s); }
+__device__ __forceinline__ void up2(f32x2 v, float &lo, float &hi) { asm("mov.b64 {%0,%1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+
+
 __device__ __forceinline__ void two_sum_fold(float &hi, float &lo, float x) {
   float s = __fadd_rn(hi, x);
   float bb = __fsub_rn(s, hi);
@@ -182,6 +193,28 @@ struct Totals {
 
 template <int TPL>
 __device__ __forceinline__ void fold_tile(Targets<TPL> &T, Totals<TPL> &R) {
+#if BH_PACKED && !BH_FOLD_F64
+  if constexpr (TPL == 2) {  // the same two-sums on register pairs: both targets per instruction
+    float *const comp[3] = {T.ax, T.ay, T.az};
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const f32x2 hi = pk2(R.hi[c][0], R.hi[c][1]), x = pk2(comp[c][0], comp[c][1]);
+      const f32x2 s = add2(hi, x);
+      const f32x2 bb = sub2(s, hi);
+      const f32x2 e = add2(sub2(hi, sub2(s, bb)), sub2(x, bb));
+      const f32x2 lo = add2(pk2(R.lo[c][0], R.lo[c][1]), e);
+      up2(s, R.hi[c][0], R.hi[c][1]);
+      up2(lo, R.lo[c][0], R.lo[c][1]);
+    }
+    // (keeping the low words in shared memory instead frees 6 registers but ran 2.5 % slower)
+#pragma unroll
+    for (int t = 0; t < 2; ++t) {
+      R.add_same_sign(t, fmaf(-0.2f, T.phq[t], T.ph[t]));
+      T.ax[t] = T.ay[t] = T.az[t] = T.ph[t] = T.phq[t] = 0.0f;
+    }
+    return;
+  }
+#endif
 #pragma unroll
   for (int t = 0; t < TPL; ++t) {
     R.add(0, t, T.ax[t]);
@@ -263,14 +296,6 @@ __device__ __forceinline__ void pc_one(const float4 a, const float4 b, const flo
 // register-file banks, which is what the scalar form cannot arrange:
 // in isolation the p-c loop runs at 0.77 of the FP32 peak against 0.69 (micro-benchmark), with half the instructions.
 // ------------------------------------------------------------------------------------------
-typedef unsigned long long f32x2;  // (lo = target 0, hi = target 1)
-__device__ __forceinline__ f32x2 pk2(float lo, float hi) { f32x2 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
-__device__ __forceinline__ f32x2 bc2(float s) { return pk2(s, s); }
-__device__ __forceinline__ void up2(f32x2 v, float &lo, float &hi) { asm("mov.b64 {%0,%1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
-__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
-
 struct Targets2 {  // the packed view of Targets<2> during one tile
   f32x2 x, y, z, ax, ay, az, ph, phq;
   __device__ __forceinline__ explicit Targets2(const Targets<2> &T)
