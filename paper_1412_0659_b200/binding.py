@@ -6,12 +6,15 @@ every step of the path runs inside libbhtree.so.
 from __future__ import annotations
 
 import ctypes as C
+import os
 from pathlib import Path
 
 import numpy as np
 
 _HERE = Path(__file__).resolve().parent
-_LIBPATH = _HERE / "libbhtree.so"
+# BHTREE_LIB names another build of the same library (e.g. `build.build_variant`, used by the test that compares the
+# packed and the scalar evaluators byte for byte); there is still no fallback: the named file must exist.
+_LIBPATH = Path(os.environ["BHTREE_LIB"]).resolve() if os.environ.get("BHTREE_LIB") else _HERE / "libbhtree.so"
 _lib = None
 
 # Flop convention of PAPER.md L190-192: 23 per particle-particle, 65 per particle-cell interaction.

@@ -65,5 +65,25 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     return LIB
 
 
+def build_variant(out: Path, defines: list[str]) -> Path:
+    """Build the same library with extra -D switches (e.g. ``["-DBH_PACKED=0"]``: scalar evaluators) into ``out``;
+    load it with the environment variable BHTREE_LIB.  Objects go next to ``out``."""
+    out = Path(out)
+    objs = []
+    for src, extra in UNITS.items():
+        obj = out.parent / (out.stem + "." + src + ".o")
+        cmd = [_nvcc(), *ARCH, *COMMON, *extra, *defines, "-c", str(CSRC / src), "-o", str(obj)]
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if r.returncode:
+            sys.stderr.write(r.stdout + r.stderr)
+            raise RuntimeError(f"nvcc failed on {src}")
+        objs.append(str(obj))
+    r = subprocess.run([_nvcc(), *ARCH, "-shared", "-o", str(out), *objs], capture_output=True, text=True)
+    if r.returncode:
+        sys.stderr.write(r.stdout + r.stderr)
+        raise RuntimeError("link failed")
+    return out
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose=True))

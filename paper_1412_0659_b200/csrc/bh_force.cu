@@ -121,6 +121,7 @@ struct Targets {
   float ax[TPL], ay[TPL], az[TPL], ph[TPL];  // sums over the tiles evaluated since the last fold
   float phq[TPL];                            // quadrupole part of the potential, scaled (see pc_one)
   uint32_t slot[TPL];
+  unsigned long long xp, yp, zp;             // two targets per lane, packed evaluators: x, y, z as FP32x2 register pairs
 };
 
 // Running totals (S14).  The per-lane FP32 sums over the last FOLD_EVERY tiles are folded into
@@ -136,6 +137,11 @@ struct Targets {
 // FP32x2 register pairs (see "Packed evaluators" below)
 #ifndef BH_PACKED
 #define BH_PACKED 1
+#endif
+// 1: the target positions live in aligned register pairs for the whole task (packed once when they are loaded);
+// 0: they live in scalar registers and every tile packs them (ptxas then re-packs them at every use: 6-7 MOV per source)
+#ifndef BH_PACK_HOME
+#define BH_PACK_HOME 1
 #endif
 typedef unsigned long long f32x2;  // (lo = target 0, hi = target 1)
 __device__ __forceinline__ f32x2 pk2(float lo, float hi) { f32x2 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
@@ -299,7 +305,13 @@ __device__ __forceinline__ void pc_one(const float4 a, const float4 b, const flo
 struct Targets2 {  // the packed view of Targets<2> during one tile
   f32x2 x, y, z, ax, ay, az, ph, phq;
   __device__ __forceinline__ explicit Targets2(const Targets<2> &T)
-      : x(pk2(T.x[0], T.x[1])), y(pk2(T.y[0], T.y[1])), z(pk2(T.z[0], T.z[1])), ax(pk2(T.ax[0], T.ax[1])),
+      :
+#if BH_PACK_HOME
+        x(T.xp), y(T.yp), z(T.zp),
+#else
+        x(pk2(T.x[0], T.x[1])), y(pk2(T.y[0], T.y[1])), z(pk2(T.z[0], T.z[1])),
+#endif
+        ax(pk2(T.ax[0], T.ax[1])),
         ay(pk2(T.ay[0], T.ay[1])), az(pk2(T.az[0], T.az[1])), ph(pk2(T.ph[0], T.ph[1])), phq(pk2(T.phq[0], T.phq[1])) {}
   __device__ __forceinline__ void store(Targets<2> &T) const {
     up2(ax, T.ax[0], T.ax[1]); up2(ay, T.ay[0], T.ay[1]); up2(az, T.az[0], T.az[1]);
@@ -521,6 +533,19 @@ __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, con
     T.x[t] = p.x; T.y[t] = p.y; T.z[t] = p.z;
     T.ax[t] = T.ay[t] = T.az[t] = T.ph[t] = T.phq[t] = 0.0f;
     if (j >= gsize) T.slot[t] = 0xffffffffu;
+  }
+  if constexpr (TPL == 2 && BH_PACKED && BH_PACK_HOME && !COUNT) {
+    // scalar loads: the halves of a pair can then be the load destinations themselves (the quad of an LDG.128 cannot be
+    // an aligned pair of two different targets, and ptxas would copy quad -> pair before every use)
+    const unsigned j0 = lane < gsize ? lane : gsize - 1, j1 = lane + 32u < gsize ? lane + 32u : gsize - 1;
+    const float *a0 = reinterpret_cast<const float *>(P.spos + g0 + j0), *a1 = reinterpret_cast<const float *>(P.spos + g0 + j1);
+    float c0[3], c1[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      asm volatile("ld.global.f32 %0, [%1];" : "=f"(c0[c]) : "l"(a0 + c));
+      asm volatile("ld.global.f32 %0, [%1];" : "=f"(c1[c]) : "l"(a1 + c));
+    }
+    T.xp = pk2(c0[0], c1[0]); T.yp = pk2(c0[1], c1[1]); T.zp = pk2(c0[2], c1[2]);
   }
   const float *gb = P.gbox + 6ll * g;
   const float bx0 = gb[0], by0 = gb[1], bz0 = gb[2], bx1 = gb[3], by1 = gb[4], bz1 = gb[5];
