@@ -54,7 +54,7 @@ __global__ void __launch_bounds__(256) opening_kernel(long long n_cells, const D
 #define BH_PP_UNROLL 16
 #endif
 #ifndef BH_PC_UNROLL
-#define BH_PC_UNROLL 8
+#define BH_PC_UNROLL 16
 #endif
 constexpr int PP_UNROLL = BH_PP_UNROLL, PC_UNROLL = BH_PC_UNROLL;  // sources per unrolled evaluator loop body
 constexpr int WALK_WARPS = 4;
