@@ -65,6 +65,8 @@ static int ensure_particles(tree_ctx *t, long long N) {
   BH_TRY(dev_alloc(t, b.lv, cap));
   long long ng = (cap + t->group - 1) / t->group;
   BH_TRY(dev_alloc(t, b.gbox, 6 * ng));
+  BH_TRY(dev_alloc(t, b.gbox_prev, 6 * ng));
+  t->prev_valid = false;
   {
     char *slab = (char *)b.shard_slab;
     BH_TRY(dev_alloc(t, slab, (long long)slab_bytes(cap, ng)));
@@ -125,7 +127,7 @@ static void free_all(tree_ctx *t) {
   detach_peers(t);
   Buffers &b = t->b;
   void *ptrs[] = {b.posm, b.vel, b.acc, b.key[0], b.key[1], b.idx[0], b.idx[1], b.scan_tmp, b.scan_blk, b.sort_hist, b.sort_status, b.spos, b.shard_slab, b.gcost,
-                  b.lv, b.gbox, b.sched_a, b.sched_b, b.gdone, b.gparts, b.gthresh, b.tasks, b.part, b.trace, b.c_level, b.c_first, b.c_count, b.c_fcall, b.c_link, b.c_cm, b.c_qa, b.c_qb,
+                  b.lv, b.gbox, b.gbox_prev, b.sched_a, b.sched_b, b.gdone, b.gparts, b.gthresh, b.tasks, b.part, b.trace, b.c_level, b.c_first, b.c_count, b.c_fcall, b.c_link, b.c_cm, b.c_qa, b.c_qb,
                   b.c_test, b.in_pos, b.in_mass, b.out_acc, b.out_pot};
   for (void *p : ptrs) if (p) cudaFree(p);
   b = Buffers();
@@ -160,7 +162,22 @@ static int force_begin_impl(tree_ctx *t, float theta, float eps) {
   t->b.gcount = t->b.gcount2[t->pass & 1];
   rec(t, EV_F0);
   BH_TRY(run_opening(t, theta));
-  BH_TRY(run_walk(t, eps));  // records EV_OPEN before and EV_WALK after the walk kernel
+  // A force pass after a fresh tree_build normally estimates the cost of every group with a counting walk.  If the
+  // previous pass on this context saw the same number of particles and nearly every group's box is where it was (the
+  // caller integrates the particles itself and rebuilds every step, or asks for another theta), that pass's exact
+  // counts are the better estimate, as in tree_leapfrog: no counting walk, a better-balanced task list.
+  const bool was_reuse = t->reuse_costs;
+  if (!was_reuse && t->shard_world <= 1 && t->prev_valid && t->prev_N == t->N) {
+    bool same = false;
+    BH_TRY(run_box_check(t, &same));
+    t->reuse_costs = same;
+  }
+  const int wrc = run_walk(t, eps);  // records EV_OPEN before and EV_WALK after the walk kernel
+  t->reuse_costs = was_reuse;
+  if (wrc) return wrc;
+  BH_CUDA(cudaMemcpyAsync(t->b.gbox_prev, t->b.gbox, (size_t)t->n_groups * 6 * sizeof(float), cudaMemcpyDeviceToDevice, t->stream));
+  t->prev_valid = true;
+  t->prev_N = t->N;
   t->theta = theta; t->eps = eps;
   t->have_force = false;
   t->force_open = true;

@@ -34,6 +34,7 @@ struct DevInfo {
   unsigned int sched_tot[2];      // totals of the two scheduling scans
   unsigned int g_lo, g_hi;        // groups this context walks in the current force pass (all of them unless sharded)
   double ekin, epot;
+  unsigned int moved_groups;      // groups whose box is not where the previous force pass saw it (box_moved_kernel)
 };
 
 struct Buffers {
@@ -56,6 +57,7 @@ struct Buffers {
   uint16_t *lv = nullptr;   // per slot: L0 | Lleaf << 5
   // groups
   float *gbox = nullptr;    // [n_groups][6]
+  float *gbox_prev = nullptr;  // the group boxes of the previous force pass (is this build the same particles, moved a little?)
   uint2 *gcount2[2] = {nullptr, nullptr};  // [n_groups] n_pp, n_pc, double-buffered like sacc2
   uint2 *gcount = nullptr;                 // = gcount2[pass & 1]
   double *gcost = nullptr;  // [n_groups] cost estimate of the current pass (task list and shard partition)
@@ -97,6 +99,8 @@ struct tree_ctx {
   long long staging_cap = 0;         // capacity of the host-call staging buffers
   float theta = 0.f, eps = 0.f;
   bool reuse_costs = false;          // this force pass may schedule by the previous pass's per-group counts
+  bool prev_valid = false;           // b.gbox_prev and the other parity's gcount describe a finished pass over prev_N particles
+  long long prev_N = 0;
   // sharded force pass: this context walks one contiguous cost-balanced range of groups and
   // stores the results into every attached context's result buffers
   int shard_rank = 0, shard_world = 1;
@@ -150,6 +154,7 @@ int run_tree(tree_ctx *t);      // octree construction; synchronises once (cell 
 int run_groups_moments(tree_ctx *t);
 int run_opening(tree_ctx *t, float theta);
 int run_walk(tree_ctx *t, float eps);
+int run_box_check(tree_ctx *t, bool *same);  // are the group boxes where the previous force pass saw them?
 void shard_views(const tree_ctx *t, void *base, int parity, float4 **sacc, uint2 **gcount);
 int run_unpermute(tree_ctx *t, float *acc, float *pot);
 int run_kick_drift(tree_ctx *t, float dt);

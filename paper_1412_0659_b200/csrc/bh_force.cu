@@ -2,6 +2,7 @@
 // leapfrog and energy.  The walk+force kernel is bound by the FP32 FMA pipe;
 // it is not a dense contraction, so no tensor cores (north_star).
 #include <algorithm>
+#include <cmath>
 
 #include "bh_common.cuh"
 
@@ -1284,6 +1285,47 @@ int run_opening(tree_ctx *t, float theta) {
   opening_kernel<<<blocks_for(t->n_cells, 256), 256, 0, t->stream>>>(t->n_cells, t->d_info, theta, t->b.c_level,
                                                                      t->b.c_cm, t->b.c_qa, t->b.c_test);
   BH_LAUNCH_CHECK("opening");
+  return 0;
+}
+
+// Is this build the particle set of the previous force pass, moved a little?  Counts, among up to 65,536 sampled groups,
+// those whose box centre lies outside the hull of the previous pass's boxes of the runs g-W..g+W, or whose box is not
+// finite.  (Particles that change their place in the Peano-Hilbert order shift every run between their old and new place
+// by one particle, so run g of this build is some run near g of the last one; the net shift grows like sqrt(N):
+// W = max(8, sqrt(N) / 128).)  Scheduling hint only.
+__global__ void __launch_bounds__(256) box_moved_kernel(unsigned n_groups, unsigned n_samples, unsigned stride, unsigned window,
+                                                        const float *__restrict__ gbox, const float *__restrict__ gbox_prev,
+                                                        DevInfo *info) {
+  const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
+  bool moved = false;
+  if (i < n_samples) {
+    const unsigned g = i * stride;
+    const float *a = gbox + 6ull * g;
+    const float cx = 0.5f * (a[0] + a[3]), cy = 0.5f * (a[1] + a[4]), cz = 0.5f * (a[2] + a[5]);
+    const unsigned q0 = g >= window ? g - window : 0u;
+    const unsigned q1 = g + window < n_groups ? g + window : n_groups - 1u;
+    float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+    for (unsigned q = q0; q <= q1; ++q) {
+      const float *b = gbox_prev + 6ull * q;
+#pragma unroll
+      for (int c = 0; c < 3; ++c) { lo[c] = fminf(lo[c], b[c]); hi[c] = fmaxf(hi[c], b[3 + c]); }
+    }
+    moved = !(cx >= lo[0] && cx <= hi[0] && cy >= lo[1] && cy <= hi[1] && cz >= lo[2] && cz <= hi[2]);
+  }
+  const unsigned m = __ballot_sync(0xffffffffu, moved);
+  if ((threadIdx.x & 31) == 0 && m) atomicAdd(&info->moved_groups, (unsigned)__popc(m));
+}
+
+int run_box_check(tree_ctx *t, bool *same) {
+  const unsigned ng = (unsigned)t->n_groups;
+  const unsigned stride = (ng + 65535u) / 65536u, ns = (ng + stride - 1u) / stride;
+  const unsigned window = std::max(8u, (unsigned)(std::sqrt((double)t->N) / 128.0));
+  BH_CUDA(cudaMemsetAsync(&t->d_info->moved_groups, 0, sizeof(unsigned), t->stream));
+  box_moved_kernel<<<(ns + 255) / 256, 256, 0, t->stream>>>(ng, ns, stride, window, t->b.gbox, t->b.gbox_prev, t->d_info);
+  BH_LAUNCH_CHECK("box_moved");
+  BH_CUDA(cudaMemcpyAsync(&t->h_info->moved_groups, &t->d_info->moved_groups, sizeof(unsigned), cudaMemcpyDeviceToHost, t->stream));
+  BH_CUDA(cudaStreamSynchronize(t->stream));
+  *same = (unsigned long long)t->h_info->moved_groups * 8ull <= ns;  // measured: 0-2 % for a drifted set, 99.7 % for an unrelated one
   return 0;
 }
 
