@@ -61,7 +61,11 @@ int tree_build(tree_ctx *t, const float *pos, const float *mass, long long N);
  * this theta, fused walk + evaluation, results to caller order.
  * theta >= 0 (0 = open everything = direct summation, L31); eps >= 0 (Plummer softening).
  * acc: DEV float[N][3] or NULL; pot: DEV float[N] or NULL.  The result is also kept inside the
- * context for tree_leapfrog / tree_get_state. */
+ * context for tree_leapfrog / tree_get_state.
+ * Scheduling (results do not depend on it beyond the rounding of partial sums of split groups): the cost of every
+ * group comes from a counting walk, or, when the previous pass on this context saw the same N and the group
+ * boxes have hardly moved (checked on the device; one 4-byte read-back and stream synchronise), from that pass's
+ * exact per-group counts. */
 int tree_force(tree_ctx *t, float theta, float eps, float *acc, float *pot);
 
 /* One kick-drift-kick step of size dt: v += a dt/2; x += v dt; rebuild the tree;

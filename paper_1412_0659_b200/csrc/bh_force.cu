@@ -810,8 +810,9 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, COUNT ? COUNT_MINB : walk_min
 // Task list (scheduling only; results depend on it only through the fixed-order partial sums).
 // cost(g) = 13 n_pp + 37 n_pc, estimated by the truncated counting walk or taken from the previous pass's exact
 // counts (tree_leapfrog). Task list of the groups this context walks (all of them unless the pass is sharded):
-//   head : parts of EXPENSIVE groups (cost > 2 x mean over all groups: s = ceil(cost / mean) parts) and, as single
-//          tasks, SUSPECT runs whose cost the previous pass cannot know (task_cost_kernel); they start first
+//   head : parts of EXPENSIVE groups (cost > 2 x mean over all groups: s = ceil(cost / mean) parts); in passes scheduled
+//          by the previous pass's counts also, as single tasks, SUSPECT runs whose cost that pass cannot know, and, cut
+//          into 16 parts, runs whose box is a large part of the system (task_cost_kernel); they start first
 //   body : one task per ordinary group, in Peano-Hilbert order (L1/L2 locality between warps)
 //   tail : the last n_tail groups, TAIL_PARTS parts each, so that the kernel ends on small tasks
 // ------------------------------------------------------------------------------------------
@@ -827,6 +828,11 @@ constexpr unsigned MAX_PARTS = 63;
 #ifndef BH_SUSPECT_AT
 #define BH_SUSPECT_AT 3.0
 #endif
+#ifndef BH_BIG_BOX
+#define BH_BIG_BOX 0.25
+#endif
+constexpr double BIG_BOX = BH_BIG_BOX;  // a run's box diagonal against the bounding box's (task_cost_kernel)
+constexpr unsigned BIG_PARTS = 16;
 constexpr double SUSPECT_AT = BH_SUSPECT_AT;  // a run's box diagonal against its neighbours' (task_cost_kernel)
 #ifndef BH_TAIL_PER_SM
 #define BH_TAIL_PER_SM 16
@@ -1032,10 +1038,25 @@ __global__ void __launch_bounds__(256) task_cost_kernel(unsigned n_groups, const
     for (unsigned q = c - 2; q <= c + 2; ++q) if (q != g) sum += diag(q);
     if (diag(g) > (float)SUSPECT_AT * 0.25f * sum) s = 1;
   }
+  // What the previous pass cannot predict at all is a run of far-apart particles (outskirts) whose box, already a large
+  // part of the system, grows a little and now reaches into the dense centre: measured at N = 1 M, one step in ten had
+  // such a run (box diagonal 54 -> 64, cost 0.75 -> 20 x the mean, neighbours unchanged), a single task of 9-20 ms in
+  // a kernel of 8.2 ms.  Every run whose box diagonal exceeds BIG_BOX x the system's is therefore cut into BIG_PARTS parts
+  // as if it cost BIG_PARTS x the mean (a few dozen runs; if they are cheap the parts are short).
+  double assumed = cost;
+  if (mine && s <= 1 && suspect_gbox) {
+    const float *b = suspect_gbox + 6ull * g;
+    const float dx = b[3] - b[0], dy = b[4] - b[1], dz = b[5] - b[2];
+    const float sx = info->hi[0] - info->lo[0], sy = info->hi[1] - info->lo[1], sz = info->hi[2] - info->lo[2];
+    if (dx * dx + dy * dy + dz * dz > (float)(BIG_BOX * BIG_BOX) * (sx * sx + sy * sy + sz * sz)) {
+      s = BIG_PARTS;
+      assumed = fmax(cost, (double)BIG_PARTS * mean);
+    }
+  }
   a_cnt[g] = s;
   gdone[g] = 0;
   // about 16 dealt entries per part: particles opened ~ cost / 13 (an over-estimate)
-  const double per_entry = cost / 13.0 / (16.0 * (s ? s : tail_parts));
+  const double per_entry = assumed / 13.0 / (16.0 * (s ? s : tail_parts));
   gthresh[g] = per_entry < 32.0 ? 32u : (per_entry > 1e9 ? 1000000000u : (unsigned)per_entry);
 }
 
