@@ -829,10 +829,13 @@ constexpr unsigned MAX_PARTS = 63;
 #define BH_SUSPECT_AT 3.0
 #endif
 #ifndef BH_BIG_BOX
-#define BH_BIG_BOX 0.25
+#define BH_BIG_BOX 0.35
 #endif
 constexpr double BIG_BOX = BH_BIG_BOX;  // a run's box diagonal against the bounding box's (task_cost_kernel)
-constexpr unsigned BIG_PARTS = 16;
+#ifndef BH_BIG_PARTS
+#define BH_BIG_PARTS 16
+#endif
+constexpr unsigned BIG_PARTS = BH_BIG_PARTS;
 constexpr double SUSPECT_AT = BH_SUSPECT_AT;  // a run's box diagonal against its neighbours' (task_cost_kernel)
 #ifndef BH_TAIL_PER_SM
 #define BH_TAIL_PER_SM 16
