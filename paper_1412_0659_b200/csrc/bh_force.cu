@@ -58,7 +58,10 @@ __global__ void __launch_bounds__(256) opening_kernel(long long n_cells, const D
 #define BH_PC_UNROLL 16
 #endif
 constexpr int PP_UNROLL = BH_PP_UNROLL, PC_UNROLL = BH_PC_UNROLL;  // sources per unrolled evaluator loop body
-constexpr int WALK_WARPS = 4;
+#ifndef BH_WALK_WARPS
+#define BH_WALK_WARPS 4
+#endif
+constexpr int WALK_WARPS = BH_WALK_WARPS;  // warps per block of the walk kernels
 constexpr int WALK_MINB = BH_WALK_MINB;  // resident blocks per SM the register budget is sized for
 #ifndef BH_WALK_MINB4
 #define BH_WALK_MINB4 3
