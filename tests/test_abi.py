@@ -75,3 +75,17 @@ def test_no_product_import_of_oracle():
     for f in os.listdir(os.path.join(ROOT, "oracle")):
         if f.endswith((".py", ".cpp")):
             assert "paper_1412_0659_b200" not in open(os.path.join(ROOT, "oracle", f)).read(), f
+
+
+def test_bhtree_lib_names_the_library_and_a_missing_one_raises(tmp_path):
+    # BHTREE_LIB selects another build of the library (tests/test_gpu_variants.py); there is still no fallback
+    import subprocess, sys, os
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    code = ("from paper_1412_0659_b200 import binding\n"
+            "print(binding.library_path())\n"
+            "try:\n    binding.load_library()\nexcept RuntimeError as e:\n    print('raised', 'no CPU fallback' in str(e))\n")
+    env = dict(os.environ, BHTREE_LIB=str(tmp_path / "nothing.so"), PYTHONPATH=root)
+    r = subprocess.run([sys.executable, "-c", code], env=env, cwd=root, capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0, r.stderr[-1000:]
+    out = r.stdout.strip().splitlines()
+    assert out[0].endswith("nothing.so") and out[1] == "raised True"
