@@ -4,22 +4,27 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
 
 A "step" is one pass of the whole hot path over one batch of synthetic input: one
-``tree_leapfrog(dt)`` = kick + drift, bbox, PH keys, radix sort, permute, octree, groups, moments,
-opening radii, fused walk+force, un-permute, kick.  The workload is
-BASELINE.json ``configs[1]`` (Plummer sphere, N = 1,048,576, eps = 0.005, theta = 0.4) unless
-``--config`` says otherwise (0-based index into ``configs``).  Prints ONE JSON line.
+``tree_leapfrog(dt)`` = kick + drift, bbox, PH keys, radix sort, octree, groups, moments, opening
+radii, fused walk+force, kick.  The workload is the largest
+single-GPU configuration of BASELINE.json, ``configs[3]`` (Milky-Way-shaped model, N = 134,217,728,
+eps = 0.005, theta = 0.4; BASELINE.json's metric names no configuration), unless ``--config`` says
+otherwise (0-based index into ``configs``).  Prints ONE JSON line.
 
-metric  : tree-force interactions per second = (p-p + p-c interactions) / step time
-value   : whole-job, inputs resident in HBM, timed with CUDA events on the library's stream,
-          L2 flushed between steps (inputs at N = 1M are smaller than the 126 MB L2)
-e2e     : the same metric through the C ABI with HOST buffers (tree_build_host + tree_force_host:
-          H2D of pos+mass and D2H of acc+pot inside the timed region)
-roofline: the fused walk+force kernel against the FP32 FMA peak (bound "alu")
-N > 1   : the path is partitioned by independent problems: every rank runs its own replica of the
-          workload (seed + rank), no data-path collective; scaling "weak".
-          ``--sharded``: ONE problem over the N GPUs instead (every rank builds the same tree,
-          walks a cost-balanced range of groups and peer-stores its results into all ranks); scaling "strong".
+metric   : tree-force interactions per second = (p-p + p-c interactions) / step time
+value    : whole-job, inputs resident in HBM, timed with CUDA events on the library's stream; L2 is
+           flushed between steps (and the inputs of the headline workload are far larger than L2)
+e2e      : the same metric through the C ABI with HOST buffers (tree_build_host + tree_force_host:
+           H2D of pos+mass and D2H of acc+pot inside the timed region)
+roofline : the fused walk+force kernel against the FP32 FMA peak (bound "alu")
+accuracy : median relative force error of the tree force against direct summation (tree_direct,
+           FP64 on the device) on a 65,536-particle subsample (BASELINE.json configs 2 and 4 ask for it)
+configs  : one summary per other BASELINE.json configuration, measured in the same process (N = 1 only;
+           ``--no-configs`` skips them); configs[4] runs its 16 leapfrog steps and reports the energy
+           drift beside the CPU oracle's on the 262,144-particle version of the same model
+N > 1    : ONE problem over the N GPUs (sharded force pass, peer stores fused into the
+           walk kernel), "scaling": "strong".  ``--replicas``: N independent replicas instead, "weak".
 ``--impl reference`` times the CPU oracle (oracle/) on the host cores on a bounded sample.
+``--table NAME`` prints one of the measurement tables kept under profiles/ (see ``TABLES``).
 """
 from __future__ import annotations
 
@@ -37,12 +42,18 @@ if ROOT not in sys.path:
 
 METRIC = "tree-force interactions/s and effective FP32 Tflops (fraction of peak)"
 UNIT = "interactions/s"
+HEADLINE_CONFIG = 3  # mw_134m: the largest single-GPU configuration of BASELINE.json
 # FP32 peak: 148 SMs x 128 FP32 lanes x 2 flop (FMA) x 1.965 GHz (B200_PROFILING.md: 148 SMs,
 # clocks.max.sm 1965 MHz); MEASURED_PEAKS.json holds no FP32 number.  DESIGN.md "Roofline".
 FP32_LANES_PER_SM = 128
+SM_MHZ = 1965.0
+# What the evaluators execute per interaction (bh_force.cu pp_one / pc_one): FP32 instructions and flops
+# (an FMA = 2, add / mul / rsqrt = 1).  The paper's CONVENTION is 23 / 65.
+INSTR_PP, INSTR_PC = 13, 33
+XFLOP_PP, XFLOP_PC = 20, 55
 
 
-def _peak_tflops(sm_count: int, sm_mhz: float) -> float:
+def _peak_tflops(sm_count: int, sm_mhz: float = SM_MHZ) -> float:
     return sm_count * FP32_LANES_PER_SM * 2 * sm_mhz * 1e6 / 1e12
 
 
@@ -115,61 +126,93 @@ def _ncu_traffic(workload: str):
     return None, None
 
 
-def _cpu_oracle_sample(cfg, pos, mass, budget_s: float = 15.0):
-    """Time the oracle's tree force (as it stands) on a bounded sample of groups of this workload."""
-    import numpy as np
-    import oracle
+def _config_dict(cfg, world: int, sharded: bool) -> dict:
+    """The `config` object of the JSON line; both arms (ours / reference) print the same one."""
+    n = cfg["n"]
+    par = (f"sharded force pass x{world} (replicated tree, peer stores)" if sharded else f"replicas x{world}")
+    return {"workload": cfg["name"], ("n_total" if sharded else "n_per_gpu"): n, "model": cfg["model"],
+            "theta": cfg["theta"], "eps": cfg["eps"], "dt": cfg.get("dt", 1e-3), "leaf_size": 16, "group_size": 64,
+            "step": "tree_leapfrog = kick/drift + keys + sort + build + moments + walk+force + kick",
+            "l2": "flushed between steps (256 MB write); inputs larger than L2 from config 2 up",
+            "parallelism": par}
 
-    t0 = time.perf_counter()
-    ot = oracle.Tree(pos, mass)
-    t_build = time.perf_counter() - t0
-    ng = ot.n_groups
-    # calibrate on a few groups, then size the sample for ~budget_s
-    probe = max(1, ng // 64)
-    t0 = time.perf_counter()
-    ot.force(cfg["theta"], cfg["eps"], g0=0, stride=max(1, ng // probe))
-    t_probe = time.perf_counter() - t0
-    per_group = t_probe / max(1, len(range(0, ng, max(1, ng // probe))))
-    want = int(min(ng, max(probe, budget_s / max(per_group, 1e-9))))
-    stride = max(1, ng // want)
-    t0 = time.perf_counter()
-    _, _, npp, npc = ot.force(cfg["theta"], cfg["eps"], g0=0, stride=stride)
-    dt = time.perf_counter() - t0
-    gsel = np.arange(0, ng, stride)
-    gs = np.minimum(64, ot.n - 64 * gsel)
-    inter = int(((npp[gsel].astype(np.int64) + npc[gsel].astype(np.int64)) * gs).sum())
-    flops = int(((23 * npp[gsel].astype(np.int64) + 65 * npc[gsel].astype(np.int64)) * gs).sum())
-    return dict(value=inter / dt, unit=UNIT, cores=oracle.num_threads(), kind="oracle",
-                sample=f"oracle tree force (FP64 accumulate) on every {stride}th group "
-                       f"({len(gsel)} of {ng} groups, {dt:.1f} s) of the same workload; "
-                       f"oracle tree build of all N took {t_build:.1f} s",
-                tflops_effective=flops / dt / 1e12, seconds=dt, build_seconds=t_build)
+
+# ---- the CPU oracle, timed as it stands (cpu_baseline leg and --impl reference) -------------------------------------
+class OracleSampler:
+    """Builds the oracle's tree of one workload ONCE; every call of ``sample`` times its tree force on a bounded,
+    strided sample of groups."""
+
+    def __init__(self, cfg, pos, mass):
+        import oracle
+        self.oracle = oracle
+        self.cfg = cfg
+        t0 = time.perf_counter()
+        self.ot = oracle.Tree(pos, mass)
+        self.build_seconds = time.perf_counter() - t0
+        self.per_group = None
+
+    def sample(self, budget_s: float, g0: int = 0):
+        import numpy as np
+        ot, cfg = self.ot, self.cfg
+        ng = ot.n_groups
+        if self.per_group is None:  # calibrate on a few groups, then size the sample for ~budget_s
+            probe = max(1, min(ng, 64))
+            ps = max(1, ng // probe)
+            t0 = time.perf_counter()
+            ot.force(cfg["theta"], cfg["eps"], g0=0, stride=ps)
+            self.per_group = (time.perf_counter() - t0) / len(range(0, ng, ps))
+        want = int(min(ng, max(16, budget_s / max(self.per_group, 1e-9))))
+        stride = max(1, ng // want)
+        g0 = g0 % stride
+        t0 = time.perf_counter()
+        _, _, npp, npc = ot.force(cfg["theta"], cfg["eps"], g0=g0, stride=stride)
+        dt = time.perf_counter() - t0
+        gsel = np.arange(g0, ng, stride)
+        gs = np.minimum(64, ot.n - 64 * gsel)
+        inter = int(((npp[gsel].astype(np.int64) + npc[gsel].astype(np.int64)) * gs).sum())
+        flops = int(((23 * npp[gsel].astype(np.int64) + 65 * npc[gsel].astype(np.int64)) * gs).sum())
+        label = "full pass" if stride == 1 else f"extrapolated from every {stride}th group"
+        return dict(value=inter / dt, unit=UNIT, cores=self.oracle.num_threads(), kind="oracle",
+                    sample=f"oracle tree force (FP64 accumulate, as it stands) on {len(gsel)} of {ng} groups "
+                           f"({label}, {dt:.1f} s) of the same workload; oracle tree build of all N took "
+                           f"{self.build_seconds:.1f} s (once, not in the rate)",
+                    tflops_effective=flops / dt / 1e12, seconds=dt, build_seconds=self.build_seconds)
 
 
 def run_reference(args):
-    """--impl reference: the CPU oracle, as it stands, on the host cores (rank 0 only)."""
+    """--impl reference: the CPU oracle, as it stands, on the host cores (rank 0 only).  The oracle's tree of the
+    workload is built once; every step times its tree force on a bounded sample of groups (another offset each step)."""
     rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
     if rank != 0:
         return 0
-    from nbody_inputs import config
-    cfg, pos, vel, mass = config(args.config, with_vel=False)
-    pos, mass = pos.numpy(), mass.numpy()
-    per_step_budget = max(2.0, min(15.0, 120.0 / max(1, args.steps + args.warmup)))
-    vals = []
-    last = None
-    for i in range(args.warmup + args.steps):
-        r = _cpu_oracle_sample(cfg, pos, mass, budget_s=per_step_budget)
+    import torch
+    from nbody_inputs import CONFIGS, milky_way, plummer
+    cfg = dict(CONFIGS[args.config])
+    if args.n:
+        cfg["n"] = args.n
+    gen = plummer if cfg["model"] == "plummer" else milky_way
+    gen_dev = "cuda" if (torch.cuda.is_available() and cfg["n"] > (1 << 22)) else "cpu"  # generation only
+    pos, _, mass = gen(cfg["n"], cfg["seed"], device=gen_dev, with_vel=False)
+    pos, mass = pos.cpu().numpy(), mass.cpu().numpy()
+    smp = OracleSampler(cfg, pos, mass)
+    total = max(1, args.steps + args.warmup)
+    per_step_budget = max(1.0, min(15.0, 100.0 / total))
+    vals, last = [], None
+    for i in range(total):
+        r = smp.sample(per_step_budget, g0=i)
         if i >= args.warmup:
             vals.append(r)
         last = r
     v = sum(x["value"] for x in vals) / len(vals)
-    ms = 1e3 * sum(x["seconds"] + x["build_seconds"] for x in vals) / len(vals)
+    ms = 1e3 * sum(x["seconds"] for x in vals) / len(vals)
+    sharded = world > 1 and not args.replicas
     line = {
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic",
-        "config": {"workload": cfg["name"], "n": cfg["n"], "theta": cfg["theta"], "eps": cfg["eps"],
-                   "note": "each step = oracle tree build + oracle tree force on a bounded sample of groups"},
+        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "strong" if sharded else "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": _config_dict(cfg, world, sharded),
+        "note": "each step = the oracle's tree force on a bounded sample of groups of the workload (tree built once)",
         "cpu_baseline": {"value": v, "unit": UNIT, "cores": last["cores"], "kind": "oracle", "sample": last["sample"]},
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -178,11 +221,114 @@ def run_reference(args):
     return 0
 
 
+# ---- our arm ------------------------------------------------------------------------------------------------------
+def _roofline(pp, pc, walk_ms_sum, steps, step_ms_sum, sm_count, peak_meas, workload):
+    """Roofline of the fused walk+force kernel (bound: FP32 ALUs).  `achieved` follows the contract of SURVEY.md
+    §8(d): ALGORITHMIC flops = the paper's 23 / 65 per interaction; the executed-flop and pipe-slot fractions of the
+    same launch are reported beside it (what the hardware really issued)."""
+    from paper_1412_0659_b200 import effective_flops
+    peak = _peak_tflops(sm_count)
+    t = walk_ms_sum * 1e-3
+    ach = effective_flops(pp, pc) / t / 1e12
+    ach_x = (XFLOP_PP * pp + XFLOP_PC * pc) / t / 1e12
+    slots = (INSTR_PP * pp + INSTR_PC * pc) / t / (sm_count * FP32_LANES_PER_SM * SM_MHZ * 1e6)
+    traffic, traffic_src = _ncu_traffic(workload)
+    return {"bound": "alu", "kernel": "walk_force_kernel", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+            "frac": ach / peak,
+            "frac_basis": "algorithmic flops, the paper's convention: 23 per p-p, 65 per p-c (PAPER.md L190-192)",
+            "achieved_executed": ach_x, "frac_executed": ach_x / peak,
+            "frac_executed_basis": f"flops the evaluators execute: {XFLOP_PP} per p-p, {XFLOP_PC} per p-c (FMA = 2)",
+            "fma_pipe_slot_frac": slots,
+            "fma_pipe_slot_basis": f"FP32 instruction slots of the evaluators ({INSTR_PP} per p-p, {INSTR_PC} per p-c) / "
+                                   "(SMs x 128 lanes x clock): the share of FMA-pipe issue slots the interactions fill",
+            "peak_measured": peak_meas, "frac_of_measured": ach / peak_meas if peak_meas else None,
+            "traffic": traffic, "traffic_unit": "bytes of DRAM read+write per launch", "traffic_source": traffic_src,
+            "peak_source": f"derived: {sm_count} SMs x 128 FP32 lanes x 2 x 1.965 GHz "
+                           "(MEASURED_PEAKS.json has no FP32 figure)",
+            "kernel_ms_avg": walk_ms_sum / steps, "kernel_share_of_step": walk_ms_sum / step_ms_sum,
+            "interactions_per_s_kernel": (pp + pc) / t}
+
+
+def _accuracy(t, n, eps, acc, nsub=65536):
+    """Median relative force error of the tree force in `acc` against tree_direct on a seeded subsample."""
+    import numpy as np
+    import torch
+    from nbody_inputs import subsample_indices
+    dev = acc.device
+    idx = subsample_indices(n, nsub, device=dev)
+    ad = torch.empty((idx.numel(), 3), dtype=torch.float64, device=dev)
+    pd = torch.empty(idx.numel(), dtype=torch.float64, device=dev)
+    t.direct(idx, eps, ad, pd)
+    err = ((acc[idx].double() - ad).norm(dim=1) / ad.norm(dim=1)).cpu().numpy()
+    return {"vs": "tree_direct (FP64 direct summation on the device) on a seeded subsample", "n_sub": int(idx.numel()),
+            "median_rel_force_err": float(np.median(err)), "p99_rel_force_err": float(np.percentile(err, 99)),
+            "bound": 2e-3}
+
+
+def _generate(cfg, dev):
+    from nbody_inputs import milky_way, plummer
+    gen = plummer if cfg["model"] == "plummer" else milky_way
+    gen_dev = dev if cfg["n"] > (1 << 22) else "cpu"
+    pos, vel, mass = gen(cfg["n"], cfg["seed"], device=gen_dev)
+    return pos.to(dev), vel.to(dev), mass.to(dev)
+
+
+def _config_summary(k, dev, stream, flush, sm_count, with_oracle):
+    """One BASELINE.json configuration in short: device-resident steps only (the headline line carries e2e)."""
+    import torch
+    from nbody_inputs import CONFIGS, milky_way
+    from paper_1412_0659_b200 import Tree, effective_flops
+    cfg = dict(CONFIGS[k])
+    n, dt = cfg["n"], cfg.get("dt", 1e-3)
+    steps = cfg.get("steps", 10 if n <= (1 << 20) else 5)
+    warm = 0 if "steps" in cfg else 3  # configs[4] IS its 16 steps: nothing runs before them
+    pos, vel, mass = _generate(cfg, dev)
+    t = Tree(device=dev.index, stream=stream.cuda_stream)
+    acc = torch.empty((n, 3), device=dev); pot = torch.empty(n, device=dev)
+    t.build(pos, mass); t.set_velocity(vel); t.force(cfg["theta"], cfg["eps"], acc, pot)
+    accuracy = _accuracy(t, n, cfg["eps"], acc)
+    ke0, pe0 = t.energy()
+    for _ in range(warm):
+        t.leapfrog(dt)
+    torch.cuda.synchronize(dev)
+    ph, pp_t, pc_t, step_ms = {}, 0, 0, 0.0
+    for s in range(steps):
+        flush.fill_(s & 0xff)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        t.leapfrog(dt)
+        e1.record(stream)
+        ms, pp, pc = t.stats()
+        step_ms += e0.elapsed_time(e1)
+        for key, v in ms.items():
+            ph[key] = ph.get(key, 0.0) + v / steps
+        pp_t += pp; pc_t += pc
+    ke1, pe1 = t.energy()
+    out = {"config": k + 1, "workload": cfg["name"], "n": n, "steps": steps, "warmup": warm, "dt": dt,
+           "ms_per_step": step_ms / steps, "value": (pp_t + pc_t) / (step_ms * 1e-3), "unit": UNIT,
+           "effective_tflops_step": effective_flops(pp_t, pc_t) / (step_ms * 1e-3) / 1e12,
+           "roofline_frac": effective_flops(pp_t, pc_t) / (ph["walk"] * steps * 1e-3) / 1e12 / _peak_tflops(sm_count),
+           "pp_per_particle": pp_t / steps / n, "pc_per_particle": pc_t / steps / n,
+           "phase_ms": ph, "accuracy": accuracy,
+           "energy": {"steps": warm + steps, "rel_drift": abs((ke1 + pe1) - (ke0 + pe0)) / abs(ke0 + pe0)}}
+    t.close()
+    del pos, vel, mass, acc, pot
+    torch.cuda.empty_cache()
+    if "steps" in cfg and with_oracle:  # configs[4]: the oracle's drift on its 262,144-particle version, same steps
+        import oracle
+        op, ov, om = milky_way(262144, 1006)
+        t0 = time.perf_counter()
+        *_, en = oracle.leapfrog(op.numpy(), ov.numpy(), om.numpy(), dt, steps, cfg["theta"], cfg["eps"])
+        out["energy"]["oracle_262144"] = {"steps": steps, "seconds": time.perf_counter() - t0,
+                                          "rel_drift": abs(en[-1].sum() - en[0].sum()) / abs(en[0].sum())}
+    return out
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
 
-    from nbody_inputs import config
+    from nbody_inputs import CONFIGS
     from paper_1412_0659_b200 import Tree, effective_flops
     from paper_1412_0659_b200.replicas import replica_seed, reduce_max_sum, whole_job_rate
 
@@ -196,21 +342,17 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    from nbody_inputs import CONFIGS
     cfg = dict(CONFIGS[args.config])
     if args.n:
         cfg["n"] = args.n
-    sharded = bool(args.sharded)
+    sharded = world > 1 and not args.replicas
     if not sharded:
         cfg["seed"] = replica_seed(cfg["seed"], rank)  # every rank its own replica of the workload
-    from nbody_inputs import plummer, milky_way
-    gen = plummer if cfg["model"] == "plummer" else milky_way
-    gen_dev = dev if cfg["n"] > (1 << 22) else "cpu"
-    pos, vel, mass = gen(cfg["n"], cfg["seed"], device=gen_dev)
+    pos, vel, mass = _generate(cfg, dev)
     n = cfg["n"]
     dt = cfg.get("dt", 1e-3)
+    d_pos, d_vel, d_mass = pos, vel, mass
     h_pos, h_mass = pos.cpu().pin_memory(), mass.cpu().pin_memory()
-    d_pos, d_vel, d_mass = pos.to(dev), vel.to(dev), mass.to(dev)
     h_acc = torch.empty((n, 3)).pin_memory(); h_pot = torch.empty(n).pin_memory()
 
     stream = torch.cuda.current_stream(dev)
@@ -218,12 +360,7 @@ def run_ours(args):
     if sharded:  # one problem over all ranks: same particles everywhere, the force pass is cut
         from paper_1412_0659_b200.sharded import ShardedTree
         drv = ShardedTree(t, device=dev)
-        try:
-            drv.connect(n)
-        except RuntimeError as e:  # no peer access between these GPUs: every rank falls back to its own replica
-            sys.stderr.write(f"[bench] --sharded unavailable ({e}); running replicas\n")
-            sharded = False
-            drv = t
+        drv.connect(n)  # raises if the GPUs are not peer-capable: no silent fall-back to replicas
     else:
         drv = t
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
@@ -234,7 +371,10 @@ def run_ours(args):
         torch.cuda.synchronize(dev)
 
     # ---- device-resident steps: tree_leapfrog
-    drv.build(d_pos, d_mass); drv.set_velocity(d_vel); drv.force(cfg["theta"], cfg["eps"])
+    acc0 = torch.empty((n, 3), device=dev); pot0 = torch.empty(n, device=dev)
+    drv.build(d_pos, d_mass); drv.set_velocity(d_vel); drv.force(cfg["theta"], cfg["eps"], acc0, pot0)
+    accuracy = None if (args.no_accuracy or rank != 0) else _accuracy(t, n, cfg["eps"], acc0)
+    del acc0, pot0
     ke0, pe0 = t.energy()  # synchronised velocities: E(0) of the KDK run (T12)
     for _ in range(args.warmup):
         drv.leapfrog(dt)
@@ -264,7 +404,7 @@ def run_ours(args):
     clocks = sampler.stop()
     step_ms = sum(a.elapsed_time(b) for a, b in ev)
     mx, sm = reduce_max_sum([step_ms, float(pp_tot), float(pc_tot), phase_ms["walk"]], dev)
-    step_ms_max, walk_ms_max = mx[0], mx[3]
+    step_ms_max = mx[0]
     pp_all, pc_all = sm[1], sm[2]
     value = (pp_all + pc_all) / (step_ms_max * 1e-3)
 
@@ -323,55 +463,44 @@ def run_ours(args):
 
     if rank == 0:
         props = torch.cuda.get_device_properties(dev)
-        peak = _peak_tflops(props.multi_processor_count, 1965.0)
-        flops = effective_flops(pp_tot, pc_tot)
-        ach = flops / (phase_ms["walk"] * 1e-3) / 1e12
-        traffic, traffic_src = _ncu_traffic(cfg["name"])
+        smc = props.multi_processor_count
         peak_meas = t.fp32_peak()  # register-only FFMA kernel, run now on this GPU
-        roof = {"bound": "alu", "kernel": "walk_force_kernel", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
-                "frac": ach / peak, "peak_measured": peak_meas, "frac_of_measured": ach / peak_meas if peak_meas else None,
-                "traffic": traffic, "traffic_unit": "bytes of DRAM read+write per launch",
-                "traffic_source": traffic_src,
-                "peak_source": f"derived: {props.multi_processor_count} SMs x 128 FP32 lanes x 2 x 1.965 GHz "
-                               "(MEASURED_PEAKS.json has no FP32 figure)",
-                "flops_convention": "23 per p-p, 65 per p-c (PAPER.md L190-192)",
-                "kernel_ms_avg": phase_ms["walk"] / args.steps,
-                "kernel_share_of_step": phase_ms["walk"] / step_ms,
-                "interactions_per_s_kernel": (pp_tot + pc_tot) / (phase_ms["walk"] * 1e-3)}
+        roof = _roofline(pp_tot, pc_tot, phase_ms["walk"], args.steps, step_ms, smc, peak_meas, cfg["name"])
         cpu = None
+        others = None
+        host_pos, host_mass = pos.cpu().numpy(), mass.cpu().numpy()
+    drv.close()
+    del pos, vel, mass, d_pos, d_vel, d_mass, h_acc, h_pot, h_pos, h_mass, h_vel
+    torch.cuda.empty_cache()
+    if rank == 0:
         if world == 1 and not args.no_cpu:
-            cpu = _cpu_oracle_sample(cfg, pos.cpu().numpy(), mass.cpu().numpy(), budget_s=15.0)
-            if "steps" in cfg:  # config 5: energy drift of the oracle on its 262,144-particle version
-                import oracle
-                op, ov, om = gen(262144, 1006)
-                t0 = time.perf_counter()
-                *_, en = oracle.leapfrog(op.numpy(), ov.numpy(), om.numpy(), dt, args.warmup + args.steps,
-                                         cfg["theta"], cfg["eps"])
-                energy["oracle_262144"] = {"steps": args.warmup + args.steps, "seconds": time.perf_counter() - t0,
-                                           "rel_drift": abs(en[-1].sum() - en[0].sum()) / abs(en[0].sum())}
+            cpu = OracleSampler(cfg, host_pos, host_mass).sample(15.0)
+        del host_pos, host_mass
+        if world == 1 and not args.no_configs:
+            others = []
+            for k in sorted(CONFIGS):
+                if k != args.config:
+                    others.append(_config_summary(k, dev, stream, flush, smc, with_oracle=not args.no_cpu))
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": step_ms_max / args.steps, "higher_is_better": True,
             "scaling": "strong" if sharded else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": cfg["name"], ("n_total" if sharded else "n_per_gpu"): n, "model": cfg["model"], "theta": cfg["theta"],
-                       "eps": cfg["eps"], "dt": dt, "leaf_size": 16, "group_size": 64,
-                       "step": "tree_leapfrog = kick/drift + keys + sort + build + moments + walk+force + kick",
-                       "l2": "flushed between steps (256 MB write)", "parallelism": (f"sharded force pass x{world} (replicated tree, peer stores)" if sharded
-                                       else f"replicas x{world}")},
+            "config": _config_dict(cfg, world, sharded),
             "effective_tflops_step": effective_flops(pp_all, pc_all) / (step_ms_max * 1e-3) / 1e12,
             "pp_per_particle": (pp_all if sharded else pp_tot) / args.steps / n,
             "pc_per_particle": (pc_all if sharded else pc_tot) / args.steps / n,
             "phase_ms": {k: v / args.steps for k, v in phase_ms.items()},
             "roofline": roof,
+            "accuracy": accuracy,
             "energy": energy,
             "cpu_baseline": cpu,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 16 * n,
                     "ms_per_step": 1e3 * e2e_s / args.steps, "phase_ms": e_phase,
                     "call": "tree_build_host + tree_force_host (pinned host buffers; host positions drift by dt * v between steps)"},
             "gpu_launches": launches, "clocks": clocks, "wall_s_timed_region": wall,
+            "configs": others,
         }
         print(json.dumps(line))
-    drv.close()
     if world > 1:
         dist.destroy_process_group()
     return 0
@@ -382,12 +511,15 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1, help="0-based index into BASELINE.json configs")
+    ap.add_argument("--config", type=int, default=HEADLINE_CONFIG, help="0-based index into BASELINE.json configs")
     ap.add_argument("--n", type=int, default=0, help="override N (debugging only)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
-    ap.add_argument("--sharded", action="store_true",
-                    help="N > 1: one problem over all GPUs (sharded force pass, strong scaling) instead of replicas")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (and the oracle's drift run)")
+    ap.add_argument("--no-configs", action="store_true", help="skip the summaries of the other BASELINE.json configs")
+    ap.add_argument("--no-accuracy", action="store_true", help="skip the error against direct summation")
+    ap.add_argument("--replicas", action="store_true",
+                    help="N > 1: N independent replicas (weak scaling) instead of ONE problem over all GPUs")
+    ap.add_argument("--sharded", action="store_true", help="(default for N > 1; kept for older command lines)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

@@ -26,6 +26,11 @@
  *    tree_build synchronises that stream once (it reads the cell count back to size the cell
  *    arrays); tree_force / tree_leapfrog return after enqueueing (tree_leapfrog contains a build);
  *    the *_host variants, tree_get_debug, tree_get_stats and tree_energy synchronise.
+ *  - Every call works on the context's device and restores the caller's current CUDA device before it returns.
+ *  - The force walk keeps its stack in shared memory behind a guard (the bound is 32 entries per
+ *    level); should the guard ever fire, the results of that pass are invalid and the NEXT call that synchronises
+ *    (tree_build, tree_leapfrog's rebuild, tree_force_host, tree_energy, tree_get_stats, tree_shard_range) returns
+ *    TREE_ERR_CUDA once ("stack overflow"), however many asynchronous passes were enqueued in between.
  *  - "Caller order" is the particle order of the arrays given to tree_build.  Outputs are always
  *    in caller order.  Masses must be > 0.  No two particles may share a position unless eps > 0
  *    (the self term is skipped by index, "N-1 interactions").
@@ -166,7 +171,11 @@ int tree_get_stats(tree_ctx *t, double *ms, unsigned long long *n_pp, unsigned l
 /* Allocate the particle-sized buffers for up to N particles now (they are otherwise grown by
  * tree_build). */
 int tree_reserve(tree_ctx *t, long long N);
-/* This context is `rank` of `world` (1 <= world <= TREE_SHARD_MAX_WORLD); world = 1 undoes it. */
+/* This context is `rank` of `world` (1 <= world <= TREE_SHARD_MAX_WORLD); world = 1 undoes it.  Synchronises the
+ * stream.  A pass writes into one of two result buffers chosen by the parity of the context's pass count, and peers
+ * store into the same parity: every call of tree_shard_config therefore restarts that count (and forgets the last
+ * force: tree_get_state(acc) / tree_leapfrog need a new force pass), so that contexts with different histories can
+ * share a pass.  From then on all contexts of a world must run the same sequence of passes. */
 int tree_shard_config(tree_ctx *t, int rank, int world);
 /* Write this context's result-buffer handle (a CUDA IPC handle and the reserved sizes) to
  * HOST memory handle[TREE_SHARD_HANDLE_BYTES].  Needs tree_reserve. */

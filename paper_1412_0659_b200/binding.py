@@ -150,7 +150,8 @@ class Tree:
         self.device = torch.device("cuda", device)
         if stream is None:
             stream = torch.cuda.current_stream(self.device).cuda_stream
-        self.h = tree_create(device, int(stream), leaf_size, group_size)
+        self.stream = int(stream)  # the cudaStream_t every call of this context enqueues on
+        self.h = tree_create(device, self.stream, leaf_size, group_size)
         self.n = 0
         self.group_size = group_size
         self.leaf_size = leaf_size

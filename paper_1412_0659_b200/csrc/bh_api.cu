@@ -16,6 +16,13 @@ int set_err(tree_ctx *t, int code, const char *what, cudaError_t ce) {
   return code;
 }
 
+int check_sticky(tree_ctx *t) {
+  if (!t->h_info->walk_overflow_sticky) return 0;
+  t->h_info->walk_overflow_sticky = 0;
+  cudaMemsetAsync(&t->d_info->walk_overflow_sticky, 0, sizeof(unsigned), t->stream);
+  return set_err(t, TREE_ERR_CUDA, "force walk: stack overflow in a force pass since the last check, results invalid");
+}
+
 template <typename T>
 static int dev_alloc(tree_ctx *t, T *&p, long long n) {
   if (p) { cudaFree(p); p = nullptr; }
@@ -30,6 +37,20 @@ static int dev_alloc(tree_ctx *t, T *&p, long long n) {
 }
 
 #define BH_TRY(x) do { int _rc = (x); if (_rc) return _rc; } while (0)
+
+// Every entry point works on the context's device and leaves the caller's current device as it found it.
+struct DeviceScope {
+  int prev = -1;
+  cudaError_t err = cudaSuccess;
+  explicit DeviceScope(int dev) {
+    err = cudaGetDevice(&prev);
+    if (err == cudaSuccess && prev != dev) err = cudaSetDevice(dev); else if (err == cudaSuccess) prev = -1;
+  }
+  ~DeviceScope() { if (prev >= 0) cudaSetDevice(prev); }
+};
+#define BH_DEVICE(t)                                                                        \
+  bh::DeviceScope _dev_scope((t)->device);                                                  \
+  if (_dev_scope.err != cudaSuccess) return bh::set_err((t), TREE_ERR_CUDA, "cudaSetDevice", _dev_scope.err)
 
 static size_t slab_bytes(long long cap, long long ng) { return 2 * (size_t)cap * sizeof(float4) + 2 * (size_t)ng * sizeof(uint2); }
 
@@ -246,7 +267,8 @@ int tree_create(tree_ctx **out, int device, void *cuda_stream, int leaf_size, in
   t->group = group_size;
   for (int i = 0; i < 24; ++i) t->ev_valid[i] = false;
   for (int i = 0; i < TREE_NPHASE; ++i) t->ms[i] = 0.0;
-  if (cudaSetDevice(device) != cudaSuccess) { delete t; return TREE_ERR_CUDA; }
+  DeviceScope scope(device);
+  if (scope.err != cudaSuccess) { delete t; return TREE_ERR_CUDA; }
   cudaDeviceProp prop;
   if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) t->sm_count = prop.multiProcessorCount;
   if (cudaMalloc((void **)&t->d_info, sizeof(DevInfo)) != cudaSuccess ||
@@ -268,7 +290,7 @@ int tree_create(tree_ctx **out, int device, void *cuda_stream, int leaf_size, in
 
 int tree_destroy(tree_ctx *t) {
   if (!t) return TREE_ERR_ARG;
-  cudaSetDevice(t->device);
+  DeviceScope scope(t->device);
   cudaStreamSynchronize(t->stream);
   free_all(t);
   if (t->d_info) cudaFree(t->d_info);
@@ -283,7 +305,7 @@ int tree_destroy(tree_ctx *t) {
 int tree_build(tree_ctx *t, const float *pos, const float *mass, long long N) {
   if (!t) return TREE_ERR_ARG;
   if (!pos || !mass || N <= 0 || N > 2147483647LL) return set_err(t, TREE_ERR_ARG, "tree_build: bad argument");
-  BH_CUDA(cudaSetDevice(t->device));
+  BH_DEVICE(t);
   if (t->force_open || t->step_open) return set_err(t, TREE_ERR_ORDER, "tree_build inside an open force pass");
   t->built = false;
   t->have_force = false;
@@ -303,7 +325,7 @@ int tree_force(tree_ctx *t, float theta, float eps, float *acc, float *pot) {
   if (!t->built) return set_err(t, TREE_ERR_ORDER, "tree_force before tree_build");
   if (t->force_open || t->step_open) return set_err(t, TREE_ERR_ORDER, "tree_force inside an open force pass");
   if (t->shard_world > 1) return set_err(t, TREE_ERR_ORDER, "sharded context: use tree_force_begin / barrier / tree_force_end");
-  BH_CUDA(cudaSetDevice(t->device));
+  BH_DEVICE(t);
   return force_impl(t, theta, eps, acc, pot);
 }
 
@@ -319,7 +341,7 @@ int tree_leapfrog(tree_ctx *t, float dt) {
   if (!t) return TREE_ERR_ARG;
   BH_TRY(leapfrog_check(t, dt));
   if (t->shard_world > 1) return set_err(t, TREE_ERR_ORDER, "sharded context: use tree_leapfrog_begin / barrier / tree_leapfrog_end");
-  BH_CUDA(cudaSetDevice(t->device));
+  BH_DEVICE(t);
   BH_TRY(leapfrog_begin_impl(t, dt));
   return leapfrog_end_impl(t);
 }
@@ -327,14 +349,14 @@ int tree_leapfrog(tree_ctx *t, float dt) {
 int tree_leapfrog_begin(tree_ctx *t, float dt) {
   if (!t) return TREE_ERR_ARG;
   BH_TRY(leapfrog_check(t, dt));
-  BH_CUDA(cudaSetDevice(t->device));
+  BH_DEVICE(t);
   return leapfrog_begin_impl(t, dt);
 }
 
 int tree_leapfrog_end(tree_ctx *t) {
   if (!t) return TREE_ERR_ARG;
   if (!t->step_open) return set_err(t, TREE_ERR_ORDER, "tree_leapfrog_end without tree_leapfrog_begin");
-  BH_CUDA(cudaSetDevice(t->device));
+  BH_DEVICE(t);
   return leapfrog_end_impl(t);
 }
 
@@ -349,21 +371,21 @@ static int force_check(tree_ctx *t, float theta, float eps) {
 int tree_force_begin(tree_ctx *t, float theta, float eps) {
   if (!t) return TREE_ERR_ARG;
   BH_TRY(force_check(t, theta, eps));
-  BH_CUDA(cudaSetDevice(t->device));
+  BH_DEVICE(t);
   return force_begin_impl(t, theta, eps);
 }
 
 int tree_force_end(tree_ctx *t, float *acc, float *pot) {
   if (!t) return TREE_ERR_ARG;
   if (!t->force_open || t->step_open) return set_err(t, TREE_ERR_ORDER, "tree_force_end without tree_force_begin");
-  BH_CUDA(cudaSetDevice(t->device));
+  BH_DEVICE(t);
   return force_end_impl(t, acc, pot);
 }
 
 int tree_reserve(tree_ctx *t, long long N) {
   if (!t) return TREE_ERR_ARG;
   if (N <= 0 || N > 2147483647LL) return set_err(t, TREE_ERR_ARG, "tree_reserve: bad N");
-  BH_CUDA(cudaSetDevice(t->device));
+  BH_DEVICE(t);
   return ensure_particles(t, N);
 }
 
@@ -373,11 +395,19 @@ int tree_shard_config(tree_ctx *t, int rank, int world) {
     return set_err(t, TREE_ERR_ARG, "tree_shard_config: need 0 <= rank < world <= TREE_SHARD_MAX_WORLD");
   if (t->force_open || t->step_open) return set_err(t, TREE_ERR_ORDER, "tree_shard_config inside an open force pass");
   if (world > 1 && t->cap <= 0) return set_err(t, TREE_ERR_ORDER, "tree_shard_config before tree_reserve");
-  BH_CUDA(cudaSetDevice(t->device));
+  BH_DEVICE(t);
   BH_CUDA(cudaStreamSynchronize(t->stream));
   if (world != t->shard_world || rank != t->shard_rank) detach_peers(t);
   t->shard_rank = rank;
   t->shard_world = world;
+  // The result buffers are selected by the parity of `pass`, and a sharded pass stores into the SAME parity of every
+  // attached context: all contexts of a world must therefore count passes alike.  Every (re)configuration restarts the
+  // count, so contexts with different histories (one ran an unsharded tree_force before, one is fresh) still agree.
+  t->pass = 0;
+  t->b.sacc = t->b.sacc2[0];
+  t->b.gcount = t->b.gcount2[0];
+  t->prev_valid = false;   // the other parity no longer holds "the previous pass"
+  t->have_force = false;
   return TREE_OK;
 }
 
@@ -395,7 +425,7 @@ int tree_shard_export(tree_ctx *t, void *handle) {
   if (!t) return TREE_ERR_ARG;
   if (!handle) return set_err(t, TREE_ERR_ARG, "tree_shard_export: NULL");
   if (t->cap <= 0 || !t->b.shard_slab) return set_err(t, TREE_ERR_ORDER, "tree_shard_export before tree_reserve");
-  BH_CUDA(cudaSetDevice(t->device));
+  BH_DEVICE(t);
   ShardBlob blob;
   memset(&blob, 0, sizeof(blob));
   BH_CUDA(cudaIpcGetMemHandle(&blob.ipc, t->b.shard_slab));
@@ -420,7 +450,7 @@ int tree_shard_attach(tree_ctx *t, int peer_rank, const void *handle) {
   ShardBlob blob;
   memcpy(&blob, handle, sizeof(blob));
   BH_TRY(attach_check(t, peer_rank, blob.cap, blob.group));
-  BH_CUDA(cudaSetDevice(t->device));
+  BH_DEVICE(t);
   void *base = nullptr;
   BH_CUDA(cudaIpcOpenMemHandle(&base, blob.ipc, cudaIpcMemLazyEnablePeerAccess));
   t->peer_base[peer_rank] = base;
@@ -432,7 +462,7 @@ int tree_shard_attach_local(tree_ctx *t, int peer_rank, tree_ctx *peer) {
   if (!t) return TREE_ERR_ARG;
   if (!peer || peer == t || !peer->b.shard_slab) return set_err(t, TREE_ERR_ARG, "tree_shard_attach_local: bad peer");
   BH_TRY(attach_check(t, peer_rank, peer->cap, peer->group));
-  BH_CUDA(cudaSetDevice(t->device));
+  BH_DEVICE(t);
   if (peer->device != t->device) {
     int can = 0;
     BH_CUDA(cudaDeviceCanAccessPeer(&can, t->device, peer->device));
@@ -449,7 +479,7 @@ int tree_shard_attach_local(tree_ctx *t, int peer_rank, tree_ctx *peer) {
 int tree_shard_range(tree_ctx *t, long long *g_lo, long long *g_hi, long long *s_lo, long long *s_hi) {
   if (!t) return TREE_ERR_ARG;
   if (!t->have_force && !t->force_open) return set_err(t, TREE_ERR_ORDER, "tree_shard_range before a force pass");
-  BH_CUDA(cudaSetDevice(t->device));
+  BH_DEVICE(t);
   BH_CUDA(cudaMemcpyAsync(t->h_info, t->d_info, sizeof(DevInfo), cudaMemcpyDeviceToHost, t->stream));
   BH_CUDA(cudaStreamSynchronize(t->stream));
   const long long lo = t->h_info->g_lo, hi = t->h_info->g_hi;
@@ -464,7 +494,7 @@ int tree_set_velocity(tree_ctx *t, const float *vel) {
   if (!t) return TREE_ERR_ARG;
   if (!vel) return set_err(t, TREE_ERR_ARG, "tree_set_velocity: NULL");
   if (t->N <= 0 || !t->b.vel) return set_err(t, TREE_ERR_ORDER, "tree_set_velocity before tree_build");
-  BH_CUDA(cudaSetDevice(t->device));
+  BH_DEVICE(t);
   BH_TRY(run_set_velocity(t, vel));
   t->have_vel = true;
   return TREE_OK;
@@ -475,7 +505,7 @@ int tree_get_state(tree_ctx *t, float *pos, float *vel, float *acc, float *pot) 
   if (t->N <= 0) return set_err(t, TREE_ERR_ORDER, "tree_get_state before tree_build");
   if (vel && !t->have_vel) return set_err(t, TREE_ERR_ORDER, "tree_get_state: no velocities set");
   if ((acc || pot) && !t->have_force) return set_err(t, TREE_ERR_ORDER, "tree_get_state: no force computed");
-  BH_CUDA(cudaSetDevice(t->device));
+  BH_DEVICE(t);
   return run_get_state(t, pos, vel, acc, pot);
 }
 
@@ -484,14 +514,14 @@ int tree_direct(tree_ctx *t, const long long *idx, long long n, float eps, doubl
   if (!idx || !acc || !pot || n <= 0 || !(eps >= 0.0f) || !isfinite(eps))
     return set_err(t, TREE_ERR_ARG, "tree_direct: bad argument");
   if (t->N <= 0 || !t->b.posm) return set_err(t, TREE_ERR_ORDER, "tree_direct before tree_build");
-  BH_CUDA(cudaSetDevice(t->device));
+  BH_DEVICE(t);
   return run_direct(t, idx, n, eps, acc, pot);
 }
 
 int tree_build_host(tree_ctx *t, const float *pos, const float *mass, long long N) {
   if (!t) return TREE_ERR_ARG;
   if (!pos || !mass || N <= 0 || N > 2147483647LL) return set_err(t, TREE_ERR_ARG, "tree_build_host: bad argument");
-  BH_CUDA(cudaSetDevice(t->device));
+  BH_DEVICE(t);
   if (N > t->staging_cap) {
     t->staging_cap = 0;
     BH_TRY(dev_alloc(t, t->b.in_pos, 3 * N));
@@ -512,19 +542,20 @@ int tree_force_host(tree_ctx *t, float theta, float eps, float *acc, float *pot)
   if (rc) return rc;
   if (acc) BH_CUDA(cudaMemcpyAsync(acc, t->b.out_acc, (size_t)t->N * 12, cudaMemcpyDeviceToHost, t->stream));
   if (pot) BH_CUDA(cudaMemcpyAsync(pot, t->b.out_pot, (size_t)t->N * 4, cudaMemcpyDeviceToHost, t->stream));
-  BH_CUDA(cudaMemcpyAsync(&t->h_info->walk_overflow, &t->d_info->walk_overflow, sizeof(unsigned), cudaMemcpyDeviceToHost, t->stream));
+  BH_CUDA(cudaMemcpyAsync(&t->h_info->walk_overflow_sticky, &t->d_info->walk_overflow_sticky, sizeof(unsigned), cudaMemcpyDeviceToHost, t->stream));
   BH_CUDA(cudaStreamSynchronize(t->stream));
-  if (t->h_info->walk_overflow) return set_err(t, TREE_ERR_CUDA, "force walk: stack overflow, results invalid");
+  BH_TRY(check_sticky(t));
   return TREE_OK;
 }
 
 int tree_energy(tree_ctx *t, double *kinetic, double *potential) {
   if (!t) return TREE_ERR_ARG;
   if (!t->have_force) return set_err(t, TREE_ERR_ORDER, "tree_energy before tree_force");
-  BH_CUDA(cudaSetDevice(t->device));
+  BH_DEVICE(t);
   BH_TRY(run_energy(t));
   BH_CUDA(cudaMemcpyAsync(t->h_info, t->d_info, sizeof(DevInfo), cudaMemcpyDeviceToHost, t->stream));
   BH_CUDA(cudaStreamSynchronize(t->stream));
+  BH_TRY(check_sticky(t));
   if (kinetic) *kinetic = t->h_info->ekin;
   if (potential) *potential = t->h_info->epot;
   return TREE_OK;
@@ -540,7 +571,7 @@ int tree_get_debug(tree_ctx *t, int what, void *dst, long long *count) {
   if (!t) return TREE_ERR_ARG;
   if (!count) return set_err(t, TREE_ERR_ARG, "tree_get_debug: count is NULL");
   if (!t->built) return set_err(t, TREE_ERR_ORDER, "tree_get_debug before tree_build");
-  BH_CUDA(cudaSetDevice(t->device));
+  BH_DEVICE(t);
   const long long N = t->N, nc = t->n_cells, ng = t->n_groups;
   switch (what) {
     case TREE_DBG_KEYS: {
@@ -636,7 +667,7 @@ int tree_get_debug(tree_ctx *t, int what, void *dst, long long *count) {
 
 int tree_get_stats(tree_ctx *t, double *ms, unsigned long long *n_pp, unsigned long long *n_pc) {
   if (!t) return TREE_ERR_ARG;
-  BH_CUDA(cudaSetDevice(t->device));
+  BH_DEVICE(t);
   BH_CUDA(cudaStreamSynchronize(t->stream));
   auto el = [&](int a, int b) -> double {
     if (!t->ev_valid[a] || !t->ev_valid[b]) return 0.0;
@@ -663,7 +694,7 @@ int tree_get_stats(tree_ctx *t, double *ms, unsigned long long *n_pp, unsigned l
     BH_CUDA(cudaMemcpy(t->h_info, t->d_info, sizeof(DevInfo), cudaMemcpyDeviceToHost));
     if (n_pp) *n_pp = t->h_info->n_pp;
     if (n_pc) *n_pc = t->h_info->n_pc;
-    if (t->have_force && t->h_info->walk_overflow) return set_err(t, TREE_ERR_CUDA, "force walk: stack overflow, results invalid");
+    BH_TRY(check_sticky(t));
   }
   return TREE_OK;
 }
@@ -671,7 +702,7 @@ int tree_get_stats(tree_ctx *t, double *ms, unsigned long long *n_pp, unsigned l
 int tree_fp32_peak(tree_ctx *t, double *tflops) {
   if (!t) return TREE_ERR_ARG;
   if (!tflops) return set_err(t, TREE_ERR_ARG, "tree_fp32_peak: NULL");
-  BH_CUDA(cudaSetDevice(t->device));
+  BH_DEVICE(t);
   return run_fp32_peak(t, tflops);
 }
 

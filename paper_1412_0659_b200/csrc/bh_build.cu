@@ -4,6 +4,8 @@
 // is a single IEEE operation in a fixed order (S9, S13).
 #include "bh_common.cuh"
 
+#define BH_TRY_RC(x) do { int _rc = (x); if (_rc) return _rc; } while (0)
+
 namespace bh {
 
 // ------------------------------------------------------------------------------------------
@@ -740,11 +742,10 @@ int run_keys(tree_ctx *t) {
 }
 
 int run_sort(tree_ctx *t) {
-  static bool attr_set = false;
-  if (!attr_set) {
+  if (!t->sort_attr_set) {  // per context: function attributes are per device
     BH_CUDA(cudaFuncSetAttribute(sort_onesweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(OsSmem)));
     BH_CUDA(cudaFuncSetAttribute(sort_onesweep_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
-    attr_set = true;
+    t->sort_attr_set = true;
   }
   const unsigned ntiles = (unsigned)((t->N + OS_TILE - 1) / OS_TILE);
   uint32_t *ghist = t->b.sort_hist, *ticket = t->b.sort_hist + 8 * RADIX;
@@ -790,6 +791,7 @@ int run_tree(tree_ctx *t) {
   BH_CUDA(cudaMemcpyAsync(t->h_info, t->d_info, sizeof(DevInfo), cudaMemcpyDeviceToHost, t->stream));
   BH_CUDA(cudaStreamSynchronize(t->stream));
   if (t->h_info->nonfinite) return set_err(t, TREE_ERR_NONFINITE, "non-finite position or mass");
+  BH_TRY_RC(check_sticky(t));  // a walk-stack overflow of an earlier asynchronous pass surfaces here at the latest
   const long long nc = t->h_info->level_off[NLEVELS];
   if (nc <= 0 || nc >= (1ll << 28)) return set_err(t, TREE_ERR_ARG, "cell count out of range (needs < 2^28 cells)");
   rc = ensure_cells(t, nc);

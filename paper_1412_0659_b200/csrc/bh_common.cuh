@@ -31,6 +31,7 @@ struct DevInfo {
   unsigned int n_tasks, n_tasks_a;  // tasks in the list; of which parts of expensive groups (listed first)
   unsigned int tail_start;          // first task of the tail region (last groups, split into small tasks)
   unsigned int walk_overflow;       // set if a warp's walk stack would have overflowed (results invalid)
+  unsigned int walk_overflow_sticky;  // the same, but cleared only when a synchronising call has reported it
   unsigned int sched_tot[2];      // totals of the two scheduling scans
   unsigned int g_lo, g_hi;        // groups this context walks in the current force pass (all of them unless sharded)
   double ekin, epot;
@@ -94,6 +95,7 @@ struct tree_ctx {
   long long sort_status_cap = 0;     // words in b.sort_status
   unsigned long long sort_epoch = 0; // look-back epoch: one per sort pass, never reused before a clear
   long long head_cap = 0, tail_cap = 0;  // partial-sum slots for expensive-group parts / tail parts
+  bool sort_attr_set = false;        // the sort kernel's shared-memory attributes are set on this context's device
   int sorted = 0;                    // which of key[]/idx[] holds the sorted result
   bool built = false, have_vel = false, have_force = false;
   long long staging_cap = 0;         // capacity of the host-call staging buffers
@@ -130,6 +132,8 @@ enum { EV_B0 = 0, EV_KEYS, EV_SORT, EV_PERM, EV_BUILD, EV_MOM, EV_F0, EV_OPEN, E
        EV_I0, EV_I1, EV_I2, EV_I3, EV_COUNT };
 
 int set_err(tree_ctx *t, int code, const char *what, cudaError_t ce = cudaSuccess);
+// After a read-back of DevInfo into t->h_info: report (once) a walk-stack overflow of any force pass since the last report.
+int check_sticky(tree_ctx *t);
 
 #define BH_CUDA(call)                                                      \
   do {                                                                     \

@@ -651,7 +651,7 @@ __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, con
       if (open_int) ws.stack[sp + __popc(m & gt)] = (lk.x << 3) | ((lk.y & 0xfu) - 1u);
       sp += __popc(m);
       if (sp + dp + 32 > STACK_CAP) {  // cannot happen within the bounds of DESIGN.md §Walk; never write past the stack
-        if (lane == 0) P.info->walk_overflow = 1u;
+        if (lane == 0) { P.info->walk_overflow = 1u; P.info->walk_overflow_sticky = 1u; }
         sp = 0; dp = 0;
       }
     }

@@ -62,7 +62,17 @@ class ShardedTree:
         if self.world > 1:
             if getattr(self, "_flag", None) is None:
                 self._flag = torch.zeros(1, dtype=torch.int64, device=self.device)
-            dist.all_reduce(self._flag, op=dist.ReduceOp.SUM, group=self.group)
+            raw = getattr(self.tree, "stream", None)
+            if raw is None:  # a stand-in tree (CPU tests of the host sequence): nothing to order on a device
+                dist.all_reduce(self._flag, op=dist.ReduceOp.SUM, group=self.group)
+                return
+            # A real context: the all-reduce must be ordered on the stream the context's kernels run on, whatever
+            # torch's current stream is, and only a device-side (NCCL) collective orders anything there.
+            if dist.get_backend(self.group) != "nccl":
+                raise RuntimeError("ShardedTree needs the nccl backend: its barrier must be a collective on the GPU stream")
+            s = torch.cuda.ExternalStream(raw, device=self.device) if raw else torch.cuda.default_stream(self.device)
+            with torch.cuda.stream(s):
+                dist.all_reduce(self._flag, op=dist.ReduceOp.SUM, group=self.group)
 
     def _sum(self, values):
         v = torch.tensor([int(x) for x in values], dtype=torch.int64, device=self.device)

@@ -211,3 +211,117 @@ def test_sharded_bench_size_config2_sampled_against_oracle():
     assert rel.max() <= TOL, rel.max()
     assert (np.abs(p - opot[sel]) / np.abs(opot[sel])).max() <= TOL
     _close(trees)
+
+
+def test_contexts_with_different_pass_histories_share_a_pass():
+    # The result buffers are double-buffered by pass parity and peers store into the same parity: a context that has
+    # already run unsharded passes (odd pass count) must still pair with a fresh one (tree_shard_config restarts the count).
+    n, theta, eps = 12000, 0.4, 0.01
+    pos, _, mass = plummer(n, 5, with_vel=False)
+    dpos, dmass = pos.cuda(), mass.cuda()
+    a, b = Tree(device=0), Tree(device=0)
+    a.build(dpos, dmass); a.force(theta, eps)          # one unsharded pass on a only: a.pass = 1, b.pass = 0
+    for t in (a, b):
+        t.reserve(n)
+    connect_local([a, b])
+    outs = [(torch.zeros((n, 3), device="cuda"), torch.zeros(n, device="cuda")) for _ in range(2)]
+    for t in (a, b):
+        t.build(dpos, dmass)
+    for _ in range(3):                                  # odd and even parities
+        force_local([a, b], theta, eps, outs)
+        torch.cuda.synchronize()
+        assert torch.equal(outs[0][0], outs[1][0]) and torch.equal(outs[0][1], outs[1][1])
+    ot = oracle.Tree(pos.numpy(), mass.numpy())
+    oacc, opot, onpp, onpc = ot.force(theta, eps)
+    for t, (acc, pot) in zip((a, b), outs):
+        cnt = t.debug("counts")
+        assert np.array_equal(cnt[:, 0], onpp) and np.array_equal(cnt[:, 1], onpc)
+        rel = np.linalg.norm(acc.cpu().numpy().astype(np.float64) - oacc, axis=1) / np.linalg.norm(oacc, axis=1)
+        assert rel.max() <= TOL
+    # back to one context each: the unsharded call works again and gives the same forces
+    a.shard_config(0, 1)
+    acc1 = torch.zeros((n, 3), device="cuda"); pot1 = torch.zeros(n, device="cuda")
+    a.force(theta, eps, acc1, pot1)
+    torch.cuda.synchronize()
+    rel = np.linalg.norm(acc1.cpu().numpy().astype(np.float64) - oacc, axis=1) / np.linalg.norm(oacc, axis=1)
+    assert rel.max() <= TOL
+    _close([a, b])
+
+
+_IPC_WORKER = r"""
+import os, sys
+import numpy as np, torch, torch.distributed as dist
+sys.path.insert(0, os.environ["BH_ROOT"])
+from nbody_inputs import plummer
+from paper_1412_0659_b200 import Tree
+from paper_1412_0659_b200.sharded import ShardedTree
+torch.cuda.set_device(0)
+dist.init_process_group("gloo")   # handle exchange only; the barrier between the two halves is explicit below
+rank, world = dist.get_rank(), dist.get_world_size()
+n, theta, eps, dt = 30011, 0.4, 0.01, 0.002
+pos, vel, mass = plummer(n, 13)
+t = Tree(device=0)
+t.reserve(n); t.shard_config(rank, world)
+handles = [None] * world
+dist.all_gather_object(handles, t.shard_export())
+for r, h in enumerate(handles):
+    if r != rank:
+        t.shard_attach(r, h)            # cudaIpcOpenMemHandle on the other PROCESS's result slab
+dist.barrier()
+def host_barrier():
+    torch.cuda.synchronize(); dist.barrier()   # both ranks share one GPU: a device collective could deadlock them
+acc = torch.zeros((n, 3), device="cuda"); pot = torch.zeros(n, device="cuda")
+t.build(pos.cuda(), mass.cuda()); t.set_velocity(vel.cuda())
+t.force_begin(theta, eps); host_barrier(); t.force_end(acc, pot)
+for _ in range(2):
+    t.leapfrog_begin(dt); host_barrier(); t.leapfrog_end()
+p = torch.empty((n, 3), device="cuda"); a = torch.empty((n, 3), device="cuda"); ph = torch.empty(n, device="cuda")
+t.get_state(p, None, a, ph); torch.cuda.synchronize()
+lo, hi, _, _ = t.shard_range()
+np.savez(os.environ["BH_OUT"] + f".{rank}.npz", acc0=acc.cpu().numpy(), pot0=pot.cpu().numpy(), p=p.cpu().numpy(),
+         a=a.cpu().numpy(), ph=ph.cpu().numpy(), counts=t.debug("counts"), rng=np.array([lo, hi]))
+host_barrier()                          # nobody unmaps while the peer may still store
+t.close()
+dist.destroy_process_group()
+"""
+
+
+def test_cross_process_ipc_sharded_pass_two_processes_one_gpu(tmp_path):
+    # tree_shard_export / tree_shard_attach across PROCESSES (cudaIpcGetMemHandle / cudaIpcOpenMemHandle): two
+    # processes on cuda:0 share a force pass and two leapfrog steps; each process's kernel stores its groups into the
+    # other process's buffers.  Both must end with the complete result, bit-identical to each other and to
+    # connect_local contexts in one process, counts bit-exact against the oracle.
+    import os, subprocess, sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    script = tmp_path / "ipc_worker.py"; script.write_text(_IPC_WORKER)
+    env = dict(os.environ, BH_ROOT=root, BH_OUT=str(tmp_path / "out"), MASTER_ADDR="127.0.0.1", MASTER_PORT="29533",
+               WORLD_SIZE="2")
+    procs = [subprocess.Popen([sys.executable, str(script)], env=dict(env, RANK=str(r)), stdout=subprocess.PIPE,
+                              stderr=subprocess.STDOUT, text=True) for r in range(2)]
+    outs = [p.communicate(timeout=600)[0] for p in procs]
+    assert all(p.returncode == 0 for p in procs), "\n".join(outs)
+    r0, r1 = (np.load(str(tmp_path / f"out.{r}.npz")) for r in range(2))
+    for k in ("acc0", "pot0", "p", "a", "ph", "counts"):
+        assert np.array_equal(r0[k], r1[k]), k
+    assert r0["rng"][0] == 0 and r0["rng"][1] == r1["rng"][0] and r1["rng"][1] == len(r0["counts"])
+    # the same run with two contexts of ONE process
+    n, theta, eps, dt = 30011, 0.4, 0.01, 0.002
+    pos, vel, mass = plummer(n, 13)
+    trees = _make(2, n)
+    acc = torch.zeros((n, 3), device="cuda"); pot = torch.zeros(n, device="cuda")
+    for t in trees:
+        t.build(pos.cuda(), mass.cuda()); t.set_velocity(vel.cuda())
+    force_local(trees, theta, eps, [(acc, pot), (None, None)])
+    torch.cuda.synchronize()
+    assert np.array_equal(acc.cpu().numpy(), r0["acc0"]) and np.array_equal(pot.cpu().numpy(), r0["pot0"])
+    for _ in range(2):
+        leapfrog_local(trees, dt)
+    p = torch.empty((n, 3), device="cuda"); a = torch.empty((n, 3), device="cuda"); ph = torch.empty(n, device="cuda")
+    trees[0].get_state(p, None, a, ph); torch.cuda.synchronize()
+    assert np.array_equal(p.cpu().numpy(), r0["p"]) and np.array_equal(a.cpu().numpy(), r0["a"])
+    ot = oracle.Tree(r0["p"], mass.numpy())
+    oacc, opot, onpp, onpc = ot.force(theta, eps)
+    assert np.array_equal(r0["counts"][:, 0], onpp) and np.array_equal(r0["counts"][:, 1], onpc)
+    rel = np.linalg.norm(r0["a"].astype(np.float64) - oacc, axis=1) / np.linalg.norm(oacc, axis=1)
+    assert rel.max() <= TOL
+    _close(trees)
