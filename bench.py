@@ -24,7 +24,7 @@ configs  : one summary per other BASELINE.json configuration, measured in the sa
 N > 1    : ONE problem over the N GPUs (sharded force pass, peer stores fused into the
            walk kernel), "scaling": "strong".  ``--replicas``: N independent replicas instead, "weak".
 ``--impl reference`` times the CPU oracle (oracle/) on the host cores on a bounded sample.
-``--table NAME`` prints one of the measurement tables kept under profiles/ (see ``TABLES``).
+``--table NAME`` prints one of the measurement tables kept under profiles/ (bench_tables.py).
 """
 from __future__ import annotations
 
@@ -150,22 +150,25 @@ class OracleSampler:
         self.ot = oracle.Tree(pos, mass)
         self.build_seconds = time.perf_counter() - t0
         self.per_group = None
+        import numpy as np
+        # result arrays allocated once: at N = 134 M zeroing 4.3 GB per call would otherwise be timed as force work
+        self.out = (np.zeros((self.ot.n, 3), np.float64), np.zeros(self.ot.n, np.float64))
 
     def sample(self, budget_s: float, g0: int = 0):
         import numpy as np
         ot, cfg = self.ot, self.cfg
         ng = ot.n_groups
         if self.per_group is None:  # calibrate on a few groups, then size the sample for ~budget_s
-            probe = max(1, min(ng, 64))
+            probe = max(1, min(ng, 256))
             ps = max(1, ng // probe)
             t0 = time.perf_counter()
-            ot.force(cfg["theta"], cfg["eps"], g0=0, stride=ps)
-            self.per_group = (time.perf_counter() - t0) / len(range(0, ng, ps))
+            ot.force(cfg["theta"], cfg["eps"], g0=ps // 2, stride=ps, out=self.out)
+            self.per_group = (time.perf_counter() - t0) / len(range(ps // 2, ng, ps))
         want = int(min(ng, max(16, budget_s / max(self.per_group, 1e-9))))
         stride = max(1, ng // want)
         g0 = g0 % stride
         t0 = time.perf_counter()
-        _, _, npp, npc = ot.force(cfg["theta"], cfg["eps"], g0=g0, stride=stride)
+        _, _, npp, npc = ot.force(cfg["theta"], cfg["eps"], g0=g0, stride=stride, out=self.out)
         dt = time.perf_counter() - t0
         gsel = np.arange(g0, ng, stride)
         gs = np.minimum(64, ot.n - 64 * gsel)
@@ -520,7 +523,14 @@ def main():
     ap.add_argument("--replicas", action="store_true",
                     help="N > 1: N independent replicas (weak scaling) instead of ONE problem over all GPUs")
     ap.add_argument("--sharded", action="store_true", help="(default for N > 1; kept for older command lines)")
+    ap.add_argument("--table", default="", help="print a measurement table instead (bench_tables.py): kernels | "
+                                                "shard-scaling | mac-sweep")
+    ap.add_argument("--from-ncu", default="", help="--table kernels: the ncu CSV to read")
+    ap.add_argument("--worlds", default="1,2,4,8", help="--table shard-scaling: world sizes")
     args = ap.parse_args()
+    if args.table:
+        import bench_tables
+        return bench_tables.run(args)
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
     if args.impl == "reference":

@@ -1,0 +1,220 @@
+"""Measurement tables kept under profiles/ (markdown on stdout), run through ``python bench.py --table NAME``.
+
+  kernels        per-kernel launch time and DRAM traffic of the step's HBM-bound phases, from an ncu CSV
+                 (``--from-ncu FILE``: a ``--metrics gpu__time_duration.sum,dram__bytes_read.sum,dram__bytes_write.sum``
+                 pass), against the measured copy bandwidth of MEASURED_PEAKS.json and the algorithmic bytes of DESIGN.md §5
+  shard-scaling  per-rank cost of the sharded force pass measured on ONE GPU with W contexts
+  mac-sweep      error versus cost of the acceptance criteria: opening angle x criterion on a
+                 BASELINE.json configuration, force error against tree_direct on a 16,384 subsample
+
+Nothing here is on the product path; the tables only call the library through its binding.
+"""
+from __future__ import annotations
+
+import csv
+import json
+import os
+import re
+from collections import defaultdict
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+
+# Algorithmic bytes per particle (or per cell, marked "c") of each HBM-bound kernel of the step pipeline, DESIGN.md §5.
+# n_c = cells, N = particles.  (read + written)
+ALGO_BYTES = {
+    "kick_drift_bbox_kernel": ("N", 48 + 32),
+    "bbox_kernel": ("N", 16 + 16),
+    "keys_kernel": ("N", 16 + 8),
+    "sort_hist8_kernel": ("N", 8),
+    "sort_onesweep_kernel": ("N", 12 + 12),
+    "permute_step_kernel": ("N", 8 + 4 + 36 + 36),
+    "permute_build_kernel": ("N", 4 + 16 + 20),
+    "tree_levels_kernel": ("N", 8 + 2),
+    "tree_emit_kernel": ("N", 2),
+    "groups_kernel": ("N", 16),
+    "kick_kernel": ("N", 32 + 16),
+    "scatter_out_kernel": ("N", 20 + 16),
+}
+
+
+def _peak_gbs() -> float:
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return float(json.load(fh)["hbm_gbs"])
+    except Exception:
+        return 6555.8  # the driver's figure for this pool (B200_PROFILING.md fallback if absent)
+
+
+def table_kernels(path: str, n_particles: int, skip_walk: bool = True):
+    """ncu CSV (long format: one row per launch and metric) -> per-kernel averages."""
+    rows = []
+    with open(path, newline="") as fh:
+        lines = [ln for ln in fh if not ln.startswith("==")]
+    rd = csv.DictReader(lines)
+    per = defaultdict(lambda: defaultdict(dict))  # kernel -> launch id -> metric -> value
+    for r in rd:
+        name = re.sub(r"\(.*", "", r.get("Kernel Name", "")).strip()
+        name = re.sub(r"^void\s+", "", name)
+        name = re.sub(r"<.*", "", name).replace("bh::", "")
+        try:
+            v = float(r["Metric Value"].replace(",", ""))
+        except (KeyError, ValueError):
+            continue
+        unit = r.get("Metric Unit", "")
+        m = r["Metric Name"]
+        if m == "gpu__time_duration.sum":
+            v *= {"ns": 1e-3, "us": 1.0, "ms": 1e3, "s": 1e6}.get(unit, 1e-3)  # -> us
+        else:
+            v *= {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}.get(unit, 1.0)
+        per[name][r["ID"]][m] = v
+    peak = _peak_gbs()
+    print(f"| kernel | launches | avg us | DRAM MB / launch | DRAM GB/s | % of {peak:.1f} | algorithmic MB | algorithmic GB/s | % | DRAM / algorithmic |")
+    print("|---|---|---|---|---|---|---|---|---|---|")
+    tot = []
+    for name, launches in per.items():
+        if skip_walk and name.startswith("walk_force"):
+            continue
+        ts = [d.get("gpu__time_duration.sum", 0.0) for d in launches.values()]
+        by = [d.get("dram__bytes_read.sum", 0.0) + d.get("dram__bytes_write.sum", 0.0) for d in launches.values()]
+        us = sum(ts) / len(ts)
+        mb = sum(by) / len(by) / 1e6
+        tot.append((sum(ts), name, len(ts), us, mb))
+    for _, name, cnt, us, mb in sorted(tot, reverse=True):
+        gbs = mb / us * 1e3 if us else 0.0
+        algo = ALGO_BYTES.get(name)
+        if algo:
+            amb = algo[1] * n_particles / 1e6
+            agbs = amb / us * 1e3
+            extra = f"{amb:.1f} | {agbs:.0f} | {100 * agbs / peak:.0f} | {mb / amb:.2f}"
+        else:
+            extra = "- | - | - | -"
+        print(f"| {name} | {cnt} | {us:.1f} | {mb:.1f} | {gbs:.0f} | {100 * gbs / peak:.0f} | {extra} |")
+
+
+def _measure_shards(cfg, world: int, steps: int):
+    import torch
+    from nbody_inputs import milky_way, plummer
+    from paper_1412_0659_b200 import Tree
+    from paper_1412_0659_b200.sharded import connect_local, force_local, leapfrog_local
+    gen = plummer if cfg["model"] == "plummer" else milky_way
+    n = cfg["n"]
+    pos, vel, mass = gen(n, cfg["seed"], device="cuda" if n > (1 << 22) else "cpu")
+    pos, vel, mass = pos.cuda(), vel.cuda(), mass.cuda()
+    trees = [Tree(device=0) for _ in range(world)]
+    for t in trees:
+        t.reserve(n)
+    if world > 1:
+        connect_local(trees)
+    for t in trees:
+        t.build(pos, mass); t.set_velocity(vel)
+    force_local(trees, cfg["theta"], cfg["eps"])
+    leapfrog_local(trees, cfg.get("dt", 1e-3))  # warm-up; from here on the partition follows exact counts
+    rows = []
+    for _ in range(steps):
+        leapfrog_local(trees, cfg.get("dt", 1e-3))
+        torch.cuda.synchronize()
+        per_rank = []
+        for t in trees:
+            ms, pp, pc = t.stats()
+            g_lo, g_hi, _, _ = t.shard_range()
+            # phases this rank runs before the barrier (walk included) + its kick after it; the kick is timed from the
+            # barrier, which on one GPU includes the other contexts' kernels, so it is taken from the W = 1 run
+            own = ms["total"] - ms["integrate"] - ms["unpermute"]
+            per_rank.append(dict(total=own, walk=ms["walk"], sched=ms["sched"], rest=own - ms["walk"] - ms["sched"],
+                                 groups=g_hi - g_lo, flops=23 * pp + 65 * pc))
+        rows.append(per_rank)
+    for t in trees:
+        t.close()
+    return [{k: sum(row[r][k] for row in rows) / len(rows) for k in rows[0][r]} for r in range(world)]
+
+
+def table_shard_scaling(config: int, worlds, steps: int):
+    """For every world size W, W contexts on cuda:0 share the passes of a few leapfrog steps.  Their kernels run one
+    after the other, each with the whole GPU, as they would on W GPUs, so the library's per-phase CUDA-event times of
+    each context are the times one rank of a W-GPU run spends; what one GPU cannot show is the cost of the peer stores
+    over NVLink (16 bytes per particle and peer, spread over the walk kernel) and of the barrier."""
+    import torch
+    from nbody_inputs import CONFIGS
+    from paper_1412_0659_b200 import Tree
+    cfg = dict(CONFIGS[config])
+    # the integrate phase (kick + drift + bbox, and the sharded kick) of a single context, measured alone
+    t = Tree(device=0)
+    from nbody_inputs import milky_way, plummer
+    gen = plummer if cfg["model"] == "plummer" else milky_way
+    pos, vel, mass = gen(cfg["n"], cfg["seed"], device="cuda" if cfg["n"] > (1 << 22) else "cpu")
+    t.build(pos.cuda(), mass.cuda()); t.set_velocity(vel.cuda()); t.force(cfg["theta"], cfg["eps"])
+    t.leapfrog(cfg.get("dt", 1e-3)); t.leapfrog(cfg.get("dt", 1e-3))
+    integ = t.stats()[0]["integrate"] * 1.5  # + the sharded pass's own kick kernel (half the kick/drift pass's bytes)
+    t.close()
+    del pos, vel, mass
+    torch.cuda.empty_cache()
+    print(f"# sharded force pass, per-rank times on one GPU: {cfg['name']}, N = {cfg['n']:,}, theta {cfg['theta']}, "
+          f"eps {cfg['eps']}, {steps} leapfrog steps averaged")
+    print("| ranks | slowest rank: step ms | its walk ms | its build+rest ms | its task list ms | walk ms min..max over ranks "
+          "| flop share max / fair | step(1) / step(W) |")
+    print("|---|---|---|---|---|---|---|---|")
+    base = None
+    for w in worlds:
+        avg = _measure_shards(cfg, w, steps)
+        for r in avg:
+            r["total"] += integ; r["rest"] += integ
+        slow = max(avg, key=lambda r: r["total"])
+        if base is None:
+            base = slow["total"]
+        tot_flops = sum(r["flops"] for r in avg)
+        share = max(r["flops"] for r in avg) / (tot_flops / w)
+        walks = [r["walk"] for r in avg]
+        print(f"| {w} | {slow['total']:.3f} | {slow['walk']:.3f} | {slow['rest']:.3f} | {slow['sched']:.3f} | "
+              f"{min(walks):.3f} .. {max(walks):.3f} | {share:.3f} | {base / slow['total']:.2f} |", flush=True)
+
+
+def table_mac_sweep(config: int):
+    """Opening angle x acceptance criterion x grouping on one BASELINE.json configuration: interaction counts, walk
+    time, force error against tree_direct (FP64 direct summation on the device) on a 16,384 subsample."""
+    import numpy as np
+    import torch
+    from nbody_inputs import config as make_config, subsample_indices
+    from paper_1412_0659_b200 import Tree
+    cfg, pos, vel, mass = make_config(config, device="cuda", with_vel=False)
+    n, eps = cfg["n"], cfg["eps"]
+    idx = subsample_indices(n, 16384, device="cuda")
+    ad = torch.empty((idx.numel(), 3), dtype=torch.float64, device="cuda")
+    pd = torch.empty(idx.numel(), dtype=torch.float64, device="cuda")
+    acc = torch.empty((n, 3), device="cuda"); pot = torch.empty(n, device="cuda")
+    adn = None
+    print(f"# {cfg['name']}, N = {n:,}, eps {eps}: acceptance criterion x theta (group 64, leaf 16 unless stated)")
+    print("| criterion | group | leaf | theta | p-p / particle | p-c / particle | walk+sched ms | median err | 99% err | max err | eff. TFLOP/s |")
+    print("|---|---|---|---|---|---|---|---|---|---|---|")
+    from paper_1412_0659_b200.binding import MAC_KINDS
+    for mac_name, mac in MAC_KINDS.items():
+        for group, leaf in ((64, 16), (32, 16), (128, 16), (64, 8), (64, 32)):
+            if mac != 0 and (group, leaf) != (64, 16):
+                continue
+            t = Tree(device=0, leaf_size=leaf, group_size=group)
+            t.set_mac(mac)
+            t.build(pos, mass)
+            if adn is None:
+                t.direct(idx, eps, ad, pd); torch.cuda.synchronize(); adn = ad.cpu().numpy()
+            for theta in (0.3, 0.4, 0.5, 0.6, 0.75, 0.9):
+                ws = []
+                for _ in range(3):
+                    t.force(theta, eps, acc, pot); ms, pp, pc = t.stats(); ws.append(ms["walk"] + ms["sched"])
+                a = acc[idx].double().cpu().numpy()
+                err = np.linalg.norm(a - adn, axis=1) / np.linalg.norm(adn, axis=1)
+                print(f"| {mac_name} | {group} | {leaf} | {theta} | {pp / n:.0f} | {pc / n:.0f} | {min(ws):.2f} | "
+                      f"{np.median(err):.2e} | {np.percentile(err, 99):.2e} | {err.max():.2e} | "
+                      f"{(23 * pp + 65 * pc) / min(ws) / 1e9:.1f} |", flush=True)
+            t.close()
+
+
+def run(args) -> int:
+    if args.table == "kernels":
+        from nbody_inputs import CONFIGS
+        table_kernels(args.from_ncu, args.n or CONFIGS[args.config]["n"])
+    elif args.table == "shard-scaling":
+        table_shard_scaling(args.config, [int(x) for x in args.worlds.split(",")], args.steps)
+    elif args.table == "mac-sweep":
+        table_mac_sweep(args.config)
+    else:
+        raise SystemExit(f"unknown table {args.table!r}")
+    return 0

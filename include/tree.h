@@ -24,8 +24,23 @@
  *    keeps a caller pointer.  Its own buffers grow to the largest N seen and are reused.
  *  - All work is enqueued on the stream given to tree_create (NULL = the legacy default stream).
  *    tree_build synchronises that stream once (it reads the cell count back to size the cell
- *    arrays); tree_force / tree_leapfrog return after enqueueing (tree_leapfrog contains a build);
- *    the *_host variants, tree_get_debug, tree_get_stats and tree_energy synchronise.
+ *    arrays); tree_force and tree_leapfrog return after enqueueing and never wait for the device
+ *    (tree_leapfrog's rebuild uses the cell arrays up to a bound the device checks, and the cell count
+ *    travels back asynchronously for the next step); the *_host variants, tree_get_debug,
+ *    tree_get_stats, tree_energy and tree_shard_range synchronise.
+ *  - Asynchronous errors.  What an asynchronous tree_leapfrog can run into on the device is reported
+ *    ONCE, by the next call that synchronises (tree_build, tree_force_host, tree_get_debug,
+ *    tree_get_stats, tree_energy, tree_shard_range), however many steps were enqueued in between:
+ *      TREE_ERR_NOMEM     the rebuilt tree needed more cells than allocated (the allocation follows the
+ *                         last known cell count + 1/8 + 1024; the count moves by a fraction of a per
+ *                         cent per step).  From that step on the device does nothing: the state
+ *                         (positions after that step's drift, velocities after its first half kick) is
+ *                         frozen and can be read with tree_get_state; continue with tree_build.
+ *      TREE_ERR_NONFINITE a position became non-finite.
+ *      TREE_ERR_CUDA      the force walk's stack guard fired (see below).
+ *  - The library keeps its state (positions, velocities, forces) in the order of the last sort
+ *    ("slot order") and moves it into the next order inside tree_leapfrog; the caller's order is
+ *    restored only where a call hands arrays back (tree_force's acc / pot, tree_get_state).
  *  - Every call works on the context's device and restores the caller's current CUDA device before it returns.
  *  - The force walk keeps its stack in shared memory behind a guard (the bound is 32 entries per
  *    level); should the guard ever fire, the results of that pass are invalid and the NEXT call that synchronises
@@ -82,7 +97,21 @@ int tree_destroy(tree_ctx *t);
 
 /* ---- auxiliary ------------------------------------------------------------------------ */
 
-/* vel: DEV float[N][3], caller order, N of the last tree_build. */
+/* Acceptance criterion of the walk (PAPER.md L31 names only "a multipole acceptance criterion
+ * parameterized by an opening angle theta" and L133 fixes theta = 0.4 for accuracy, cost ~ theta^-3):
+ *   TREE_MAC_GEOMETRIC (default; S5)  accept iff D > l / theta + delta, l = side of the cell's octant,
+ *                                               delta = |centre of mass - centre of the octant|
+ *   TREE_MAC_BMAX                               accept iff D > b / theta, b = distance from the cell's centre of mass to
+ *                                               the farthest corner of the TIGHT bounding box of its particles (the
+ *                                               bounding-radius criterion of Salmon & Warren)
+ * D = distance from the group's bounding box to the cell's centre of mass in both.  Call before tree_build (the tight
+ * boxes are computed with the moments); a context that is already built must be built again. */
+#define TREE_MAC_GEOMETRIC 0
+#define TREE_MAC_BMAX 1
+int tree_set_mac(tree_ctx *t, int kind);
+
+/* vel: DEV float[N][3], caller order, N of the last tree_build.  tree_build forgets the velocities (it re-orders the
+ * state): set them after every tree_build that is followed by tree_leapfrog. */
 int tree_set_velocity(tree_ctx *t, const float *vel);
 
 /* Current state in caller order; any pointer may be NULL.  pos, vel, acc: DEV float[N][3];
@@ -124,21 +153,23 @@ int tree_direct(tree_ctx *t, const long long *idx, long long n, float eps, doubl
 #define TREE_DBG_LEVEL_OFFSETS 10 /* int32[24]  first cell id of each level 0..22, then n_cells   */
 #define TREE_DBG_TASK_TRACE 11 /* uint32[n_tasks][4] per task of the last force pass: start ns since the
                                   pass began, duration ns, SM id, group | part << 26 (scheduling trace) */
+#define TREE_DBG_TIGHT 12      /* float[n_cells][7] TREE_MAC_BMAX only: tight box lo x,y,z, hi x,y,z, bounding radius b */
 int tree_get_debug(tree_ctx *t, int what, void *dst, long long *count);
 
 /* Timings of the last tree_build / tree_force / tree_leapfrog in milliseconds (CUDA events on the
  * context's stream) and interaction totals of the last force pass, to HOST memory.
  * ms[TREE_NPHASE]: see TREE_PH_*.  n_pp / n_pc = sum over groups of group size x list length
  * ("as recorded during execution").  Synchronises. */
-#define TREE_PH_KEYS 0     /* bbox + grid + keys                 */
+#define TREE_PH_KEYS 0     /* bbox + grid + keys (tree_leapfrog: grid + keys; its bbox is fused into the kick/drift pass) */
 #define TREE_PH_SORT 1     /* radix sort of (key, index)         */
-#define TREE_PH_PERMUTE 2  /* gather particles into slot order   */
+#define TREE_PH_PERMUTE 2  /* gather the particles (tree_leapfrog: positions, velocities, caller indices) into slot order */
 #define TREE_PH_BUILD 3    /* octree construction + linking      */
 #define TREE_PH_MOMENTS 4  /* groups + multipole moments         */
 #define TREE_PH_OPENING 5  /* opening radii for theta            */
 #define TREE_PH_WALK 6     /* the fused walk + force kernel only */
-#define TREE_PH_UNPERMUTE 7 /* results back to caller order      */
-#define TREE_PH_INTEGRATE 8 /* leapfrog kicks + drift            */
+#define TREE_PH_UNPERMUTE 7 /* results to the caller's arrays (only if tree_force was given any) */
+#define TREE_PH_INTEGRATE 8 /* leapfrog: kick + drift + bbox pass (the closing kick runs in the walk's epilogue; sharded
+                               passes kick in a pass of their own after the barrier) */
 #define TREE_PH_SCHED 9    /* counting walk + task list (cost-aware scheduling of the force walk) */
 #define TREE_PH_TOTAL 10   /* sum of the above for the last call sequence */
 #define TREE_NPHASE 11

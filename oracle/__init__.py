@@ -59,6 +59,8 @@ def lib():
         L.orc_tree_force.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.c_void_p, C.c_int64, C.c_int64]
         L.orc_tree_get_counts.argtypes = [C.c_void_p] * 3
         L.orc_tree_get_ropen2.argtypes = [C.c_void_p] * 2
+        L.orc_tree_set_mac.argtypes = [C.c_void_p, C.c_int]
+        L.orc_tree_get_tight.argtypes = [C.c_void_p] * 2
         L.orc_tree_walk_lists.argtypes = [C.c_void_p, C.c_float, C.c_int64, C.c_void_p, C.POINTER(C.c_int64),
                                           C.c_void_p, C.POINTER(C.c_int64)]
         L.orc_leapfrog.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_float, C.c_int,
@@ -178,16 +180,32 @@ class Tree:
         lib().orc_tree_get_sorted(self._h, _p(out))
         return out
 
-    def force(self, theta: float, eps: float, g0: int = 0, stride: int = 1):
-        """T9-T11. Returns acc [N,3] f64, pot [N] f64 (original order), n_pp, n_pc per group."""
-        acc = np.zeros((self.n, 3), np.float64)
-        pot = np.zeros(self.n, np.float64)
+    def force(self, theta: float, eps: float, g0: int = 0, stride: int = 1, out=None):
+        """T9-T11. Returns acc [N,3] f64, pot [N] f64 (original order), n_pp, n_pc per group.
+        ``out`` = (acc, pot) arrays to write into (entries of groups that are not walked are left as they are)."""
+        if out is not None:
+            acc, pot = out
+            assert acc.shape == (self.n, 3) and pot.shape == (self.n,) and acc.dtype == np.float64 and pot.dtype == np.float64
+        else:
+            acc = np.zeros((self.n, 3), np.float64)
+            pot = np.zeros(self.n, np.float64)
         rc = lib().orc_tree_force(self._h, float(theta), float(eps), _p(acc), _p(pot), int(g0), int(stride))
         if rc:
             raise ValueError(f"orc_tree_force failed: {rc}")
         npp = np.zeros(self.n_groups, np.uint32); npc = np.zeros(self.n_groups, np.uint32)
         lib().orc_tree_get_counts(self._h, _p(npp), _p(npc))
         return acc, pot, npp, npc
+
+    def set_mac(self, kind: int):
+        """Acceptance criterion of later force / walk_lists calls: 0 = canonical (S5), 1 = "bmax" (option, NEXT-2)."""
+        if lib().orc_tree_set_mac(self._h, int(kind)):
+            raise ValueError("unknown criterion")
+
+    def tight(self):
+        """float32 [n_cells,7]: tight bounding box lo, hi of each cell's particles and its bounding radius b."""
+        out = np.zeros((self.n_cells, 7), np.float32)
+        lib().orc_tree_get_tight(self._h, _p(out))
+        return out
 
     def ropen2(self):
         out = np.zeros(self.n_cells, np.float32)

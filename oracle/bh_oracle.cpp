@@ -18,6 +18,13 @@
 // adjacency / parent property, tree invariants, moments vs direct second moments, partition
 // invariant of the walk, theta -> 0 == direct, p-c error ~ (size/distance)^3, a = grad phi,
 // leapfrog circular orbit / reversibility.
+// Option (not in PAPER.md): a second acceptance criterion, "bmax" (Salmon & Warren's bounding
+// radius: accept iff D > b / theta, b = distance from the cell's centre of mass to the farthest corner of the TIGHT
+// bounding box of its particles), selected with orc_tree_set_mac; the canonical criterion (S5) is the default and its
+// arithmetic is untouched.  Pins: b bounds the distance of every particle of the cell from its c.o.m.; boxes nest.
+// Parity unpinned: the MAC formula itself (S5: PAPER.md L31 names an opening angle and defers to its ref. [9]) and the
+// rounding order of T7 (S13: PAPER.md is silent on the precision of the moments) -- recorded readings, pinned only
+// through their consequences (tree-vs-direct error, partition invariant, theta -> 0).
 // Parity unpinned: the paper's interaction counts per particle (Table II) depend on
 // group/MAC details and initial conditions that PAPER.md does not print; only their order of
 // magnitude is comparable.
@@ -84,6 +91,8 @@ struct Tree {
   std::vector<float> sx, sy, sz, sm;   // sorted-slot order
   std::vector<Cell> cells;             // BFS order (T5)
   std::vector<float> cM, cx, cy, cz, qxx, qyy, qzz, qxy, qxz, qyz, delta;  // T7, FP32 stored
+  std::vector<float> tlo, thi, brad;   // option "bmax": tight box [n_cells][3] x 2 and bounding radius b about the c.o.m.
+  int mac = 0;                         // 0: S5 (l / theta + delta), 1: bmax (b / theta)
   std::vector<float> gmin, gmax;       // T8: [n_groups][3]
   std::vector<float> ropen2;           // T9, for the last theta
   std::vector<uint32_t> npp, npc;      // T10 per group
@@ -235,6 +244,32 @@ int build(Tree &t) {
     t.qxy[ci] = (float)Q[3]; t.qxz[ci] = (float)Q[4]; t.qyz[ci] = (float)Q[5];
     t.delta[ci] = (float)del;
   }
+  // ---- option "bmax": tight bounding box of every cell's particles, bottom-up (min / max are exact), and the
+  // bounding radius about the FP32 centre of mass, FP32 in this order: e_d = max(c_d - lo_d, hi_d - c_d);
+  // b2 = fma(e_z, e_z, fma(e_y, e_y, e_x * e_x)); b = sqrt(b2)
+  t.tlo.assign(3 * nc, 0); t.thi.assign(3 * nc, 0); t.brad.assign(nc, 0);
+  for (size_t ci = nc; ci-- > 0;) {
+    const Cell &c = t.cells[ci];
+    float lo[3], hi[3];
+    for (int d = 0; d < 3; ++d) { lo[d] = std::numeric_limits<float>::infinity(); hi[d] = -lo[d]; }
+    if (c.first_child < 0) {
+      for (uint32_t p = c.first; p < c.first + c.count; ++p) {
+        const float x[3] = {t.sx[p], t.sy[p], t.sz[p]};
+        for (int d = 0; d < 3; ++d) { lo[d] = std::min(lo[d], x[d]); hi[d] = std::max(hi[d], x[d]); }
+      }
+    } else {
+      for (int32_t ch = c.first_child; ch < c.first_child + c.n_child; ++ch)
+        for (int d = 0; d < 3; ++d) { lo[d] = std::min(lo[d], t.tlo[3 * ch + d]); hi[d] = std::max(hi[d], t.thi[3 * ch + d]); }
+    }
+    const float cc[3] = {t.cx[ci], t.cy[ci], t.cz[ci]};
+    float e[3];
+    for (int d = 0; d < 3; ++d) {
+      t.tlo[3 * ci + d] = lo[d]; t.thi[3 * ci + d] = hi[d];
+      e[d] = std::max(cc[d] - lo[d], hi[d] - cc[d]);
+    }
+    const float b2 = std::fmaf(e[2], e[2], std::fmaf(e[1], e[1], e[0] * e[0]));
+    t.brad[ci] = std::sqrt(b2);
+  }
   // ---- T8 groups: fixed runs of group_size sorted slots, tight AABB
   const int64_t ng = t.n_groups();
   t.gmin.assign(3 * ng, 0); t.gmax.assign(3 * ng, 0);
@@ -257,6 +292,12 @@ void set_opening(Tree &t, float theta) {
   const size_t nc = t.cells.size();
   t.ropen2.resize(nc);
   for (size_t c = 0; c < nc; ++c) {
+    if (t.mac == 1) {  // option "bmax": r = b / theta; r_open^2 = r * r
+      float r = t.brad[c] / theta;
+      if (theta == 0.0f) r = std::numeric_limits<float>::infinity();  // 0 / 0: theta = 0 still opens everything
+      t.ropen2[c] = r * r;
+      continue;
+    }
     float lc = std::ldexp(1.0f, t.k - t.cells[c].level);
     float r = lc / theta;
     r = r + t.delta[c];
@@ -492,6 +533,22 @@ void orc_tree_get_counts(void *h, uint32_t *npp, uint32_t *npc) {
   std::memcpy(npp, t->npp.data(), t->npp.size() * sizeof(uint32_t));
   std::memcpy(npc, t->npc.data(), t->npc.size() * sizeof(uint32_t));
 }
+// option "bmax": kind 0 = canonical (S5), 1 = bmax
+int orc_tree_set_mac(void *h, int kind) {
+  if (kind != 0 && kind != 1) return -1;
+  ((Tree *)h)->mac = kind;
+  return 0;
+}
+
+// [n_cells][7]: tight box lo x,y,z, hi x,y,z, bounding radius b
+void orc_tree_get_tight(void *h, float *out) {
+  Tree *t = (Tree *)h;
+  for (size_t c = 0; c < t->cells.size(); ++c) {
+    for (int d = 0; d < 3; ++d) { out[7 * c + d] = t->tlo[3 * c + d]; out[7 * c + 3 + d] = t->thi[3 * c + d]; }
+    out[7 * c + 6] = t->brad[c];
+  }
+}
+
 void orc_tree_get_ropen2(void *h, float *out) {
   Tree *t = (Tree *)h;
   std::memcpy(out, t->ropen2.data(), t->ropen2.size() * sizeof(float));

@@ -26,7 +26,8 @@ SHARD_HANDLE_BYTES = 128
 PHASES = ("keys", "sort", "permute", "build", "moments", "opening", "walk", "unpermute", "integrate", "sched", "total")
 
 DBG = dict(keys=0, order=1, sorted_keys=2, cells=3, moments=4, group_boxes=5, counts=6, grid=7, ropen2=8,
-           sorted_pos=9, level_offsets=10, task_trace=11)
+           sorted_pos=9, level_offsets=10, task_trace=11, tight=12)
+MAC_KINDS = dict(geometric=0, bmax=1)  # TREE_MAC_* of include/tree.h
 
 _SIGS = {
     "tree_create": (C.c_int, [C.POINTER(C.c_void_p), C.c_int, C.c_void_p, C.c_int, C.c_int]),
@@ -35,6 +36,7 @@ _SIGS = {
     "tree_leapfrog": (C.c_int, [C.c_void_p, C.c_float]),
     "tree_destroy": (C.c_int, [C.c_void_p]),
     "tree_set_velocity": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "tree_set_mac": (C.c_int, [C.c_void_p, C.c_int]),
     "tree_get_state": (C.c_int, [C.c_void_p] * 5),
     "tree_build_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_longlong]),
     "tree_force_host": (C.c_int, [C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.c_void_p]),
@@ -219,6 +221,10 @@ class Tree:
         _check(self.h, load_library().tree_shard_range(self.h, *[C.byref(x) for x in v]))
         return tuple(int(x.value) for x in v)
 
+    def set_mac(self, kind):
+        """Acceptance criterion (tree_set_mac): 0 / "geometric" (default) or 1 / "bmax"; before build."""
+        _check(self.h, load_library().tree_set_mac(self.h, int(MAC_KINDS.get(kind, kind))))
+
     def set_velocity(self, vel):
         assert vel.is_cuda and vel.numel() == 3 * self.n
         _check(self.h, load_library().tree_set_velocity(self.h, _ptr(vel)))
@@ -269,7 +275,7 @@ class Tree:
             "cells": ((n, 5), np.int32), "moments": ((n, 11), np.float32), "group_boxes": ((n, 6), np.float32),
             "counts": ((n, 2), np.uint32), "grid": ((n,), np.float32), "ropen2": ((n,), np.float32),
             "sorted_pos": ((n, 4), np.float32), "level_offsets": ((n,), np.int32),
-            "task_trace": ((n, 4), np.uint32),
+            "task_trace": ((n, 4), np.uint32), "tight": ((n, 7), np.float32),
         }[what]
         out = np.zeros(shape, dt)
         _check(self.h, load_library().tree_get_debug(self.h, code, _ptr(out), C.byref(cnt)))

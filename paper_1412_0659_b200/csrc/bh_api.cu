@@ -16,11 +16,34 @@ int set_err(tree_ctx *t, int code, const char *what, cudaError_t ce) {
   return code;
 }
 
+// Errors of asynchronous passes (tree.h "asynchronous errors"), looked at after a read-back of DevInfo into t->h_info:
+// each is reported once, by the first synchronising call after it happened.
 int check_sticky(tree_ctx *t) {
-  if (!t->h_info->walk_overflow_sticky) return 0;
-  t->h_info->walk_overflow_sticky = 0;
-  cudaMemsetAsync(&t->d_info->walk_overflow_sticky, 0, sizeof(unsigned), t->stream);
-  return set_err(t, TREE_ERR_CUDA, "force walk: stack overflow in a force pass since the last check, results invalid");
+  DevInfo *h = t->h_info;
+  if (h->cells_overflow) {
+    const long long need = h->cells_overflow;
+    h->cells_overflow = 0;
+    cudaMemsetAsync(&t->d_info->cells_overflow, 0, sizeof(unsigned), t->stream);
+    t->built = false;       // the state (positions, velocities, order) is intact, the tree and the last force are not
+    t->have_force = false;
+    t->n_cells = need;      // the next rebuild sizes its cell arrays for it
+    return set_err(t, TREE_ERR_NOMEM,
+                   "tree_leapfrog: the rebuilt tree needed more cells than were allocated; the state is frozen after that "
+                   "step's drift: read it with tree_get_state and call tree_build");
+  }
+  if (h->nonfinite_sticky) {
+    h->nonfinite_sticky = 0;
+    cudaMemsetAsync(&t->d_info->nonfinite_sticky, 0, sizeof(unsigned), t->stream);
+    t->built = false;
+    t->have_force = false;
+    return set_err(t, TREE_ERR_NONFINITE, "tree_leapfrog: a position became non-finite");
+  }
+  if (h->walk_overflow_sticky) {
+    h->walk_overflow_sticky = 0;
+    cudaMemsetAsync(&t->d_info->walk_overflow_sticky, 0, sizeof(unsigned), t->stream);
+    return set_err(t, TREE_ERR_CUDA, "force walk: stack overflow in a force pass since the last check, results invalid");
+  }
+  return 0;
 }
 
 template <typename T>
@@ -79,10 +102,13 @@ static int ensure_particles(tree_ctx *t, long long N) {
   Buffers &b = t->b;
   t->cap = 0;
   BH_TRY(dev_alloc(t, b.posm, cap));
-  BH_TRY(dev_alloc(t, b.vel, cap));
-  BH_TRY(dev_alloc(t, b.acc, cap));
-  for (int k = 0; k < 2; ++k) { BH_TRY(dev_alloc(t, b.key[k], cap)); BH_TRY(dev_alloc(t, b.idx[k], cap)); }
-  BH_TRY(dev_alloc(t, b.spos, cap));
+  for (int k = 0; k < 2; ++k) {
+    BH_TRY(dev_alloc(t, b.key[k], cap)); BH_TRY(dev_alloc(t, b.idx[k], cap));
+    BH_TRY(dev_alloc(t, b.spos2[k], cap)); BH_TRY(dev_alloc(t, b.svel2[k], cap)); BH_TRY(dev_alloc(t, b.order2[k], cap));
+  }
+  t->cur = 0;
+  b.spos = b.spos2[0]; b.svel = b.svel2[0]; b.order = b.order2[0];
+  t->state_valid = false;
   BH_TRY(dev_alloc(t, b.lv, cap));
   long long ng = (cap + t->group - 1) / t->group;
   BH_TRY(dev_alloc(t, b.gbox, 6 * ng));
@@ -140,6 +166,7 @@ int ensure_cells(tree_ctx *t, long long nc) {
   BH_TRY(dev_alloc(t, b.c_qa, cap));
   BH_TRY(dev_alloc(t, b.c_qb, cap));
   BH_TRY(dev_alloc(t, b.c_test, cap));
+  if (t->mac == TREE_MAC_BMAX) { BH_TRY(dev_alloc(t, b.c_tlo, cap)); BH_TRY(dev_alloc(t, b.c_thi, cap)); }
   t->cell_cap = cap;
   return 0;
 }
@@ -147,23 +174,26 @@ int ensure_cells(tree_ctx *t, long long nc) {
 static void free_all(tree_ctx *t) {
   detach_peers(t);
   Buffers &b = t->b;
-  void *ptrs[] = {b.posm, b.vel, b.acc, b.key[0], b.key[1], b.idx[0], b.idx[1], b.scan_tmp, b.scan_blk, b.sort_hist, b.sort_status, b.spos, b.shard_slab, b.gcost,
+  void *ptrs[] = {b.posm, b.key[0], b.key[1], b.idx[0], b.idx[1], b.spos2[0], b.spos2[1], b.svel2[0], b.svel2[1], b.order2[0], b.order2[1],
+                  b.scan_tmp, b.scan_blk, b.sort_hist, b.sort_status, b.shard_slab, b.gcost,
                   b.lv, b.gbox, b.gbox_prev, b.sched_a, b.sched_b, b.gdone, b.gparts, b.gthresh, b.tasks, b.part, b.trace, b.c_level, b.c_first, b.c_count, b.c_fcall, b.c_link, b.c_cm, b.c_qa, b.c_qb,
-                  b.c_test, b.in_pos, b.in_mass, b.out_acc, b.out_pot};
+                  b.c_test, b.c_tlo, b.c_thi, b.in_pos, b.in_mass, b.out_acc, b.out_pot};
   for (void *p : ptrs) if (p) cudaFree(p);
   b = Buffers();
 }
 
 static inline void rec(tree_ctx *t, int e) { if (t->ev_valid[e]) cudaEventRecord(t->ev[e], t->stream); }
 
+// tree_build: the sort's payload is the caller index; the particles are gathered from the staging copy posm
 static int build_from_posm(tree_ctx *t) {
-  BH_TRY(run_keys(t));
+  BH_TRY(run_keys(t, t->b.posm));
   rec(t, EV_KEYS);
   BH_TRY(run_sort(t));
   rec(t, EV_SORT);
-  BH_TRY(run_permute(t));
+  BH_TRY(run_permute_build(t));
   rec(t, EV_PERM);
-  BH_TRY(run_tree(t));
+  t->state_valid = true;
+  BH_TRY(run_tree(t, /*async=*/false));
   rec(t, EV_BUILD);
   BH_TRY(run_groups_moments(t));
   rec(t, EV_MOM);
@@ -174,7 +204,8 @@ static int build_from_posm(tree_ctx *t) {
 // First half of a force pass: everything up to and including the fused walk + force kernel.  The pass
 // writes into the result buffers of parity (pass & 1); the other parity still holds the previous pass
 // (its per-group counts schedule this one, and a sharded peer may still be reading it).
-static int force_begin_impl(tree_ctx *t, float theta, float eps) {
+// kick_hdt != 0 (tree_leapfrog on one context): the walk's epilogue also applies the step's closing half kick.
+static int force_begin_impl(tree_ctx *t, float theta, float eps, float kick_hdt) {
   if (t->shard_world > 1)
     for (int r = 0; r < t->shard_world; ++r)
       if (r != t->shard_rank && !t->peer_base[r]) return set_err(t, TREE_ERR_ORDER, "sharded context: a peer is not attached");
@@ -186,15 +217,15 @@ static int force_begin_impl(tree_ctx *t, float theta, float eps) {
   // A force pass after a fresh tree_build normally estimates the cost of every group with a counting walk.  If the
   // previous pass on this context saw the same number of particles and nearly every group's box is where it was (the
   // caller integrates the particles itself and rebuilds every step, or asks for another theta), that pass's exact
-  // counts are the better estimate, as in tree_leapfrog: no counting walk, a better-balanced task list.
-  const bool was_reuse = t->reuse_costs;
-  if (!was_reuse && t->shard_world <= 1 && t->prev_valid && t->prev_N == t->N) {
-    bool same = false;
-    BH_TRY(run_box_check(t, &same));
-    t->reuse_costs = same;
+  // counts are the better estimate, as in tree_leapfrog: no counting walk, a better-balanced task list.  The check and
+  // the decision stay on the device (reuse_mode 2): no read-back.
+  const int mode_in = t->reuse_mode;
+  if (mode_in == 0 && t->shard_world <= 1 && t->prev_valid && t->prev_N == t->N) {
+    BH_TRY(run_box_check(t));
+    t->reuse_mode = 2;
   }
-  const int wrc = run_walk(t, eps);  // records EV_OPEN before and EV_WALK after the walk kernel
-  t->reuse_costs = was_reuse;
+  const int wrc = run_walk(t, eps, kick_hdt);  // records EV_OPEN before and EV_WALK after the walk kernel
+  t->reuse_mode = mode_in;
   if (wrc) return wrc;
   BH_CUDA(cudaMemcpyAsync(t->b.gbox_prev, t->b.gbox, (size_t)t->n_groups * 6 * sizeof(float), cudaMemcpyDeviceToDevice, t->stream));
   t->prev_valid = true;
@@ -205,9 +236,9 @@ static int force_begin_impl(tree_ctx *t, float theta, float eps) {
   return 0;
 }
 
-// Second half: results to caller order (in a sharded pass, after the caller's barrier).
+// Second half: results to the caller's arrays if it gave any (in a sharded pass, after the caller's barrier).
 static int force_end_impl(tree_ctx *t, float *acc, float *pot) {
-  BH_TRY(run_unpermute(t, acc, pot));
+  BH_TRY(run_scatter_out(t, acc, pot));
   rec(t, EV_UNPERM);
   t->force_open = false;
   t->have_force = true;
@@ -215,22 +246,41 @@ static int force_end_impl(tree_ctx *t, float *acc, float *pot) {
 }
 
 static int force_impl(tree_ctx *t, float theta, float eps, float *acc, float *pot) {
-  BH_TRY(force_begin_impl(t, theta, eps));
+  BH_TRY(force_begin_impl(t, theta, eps, 0.0f));
   return force_end_impl(t, acc, pot);
 }
 
+// One step without a host round trip: the state stays in slot order, the cell arrays
+// are used up to a bound the device checks, the cell count travels back asynchronously for the next step.
 static int leapfrog_begin_impl(tree_ctx *t, float dt) {
+  // room for this step's tree: the latest known cell count plus a margin (grown here, synchronously, when the
+  // margin has been used up: the arrays are rebuilt below anyway)
+  poll_cells(t);
+  const long long want = t->n_cells + t->n_cells / 8 + 1024;
+  if (want > t->cell_cap) {
+    BH_CUDA(cudaStreamSynchronize(t->stream));
+    BH_TRY(ensure_cells(t, want));
+  }
   rec(t, EV_I0);
-  BH_TRY(run_kick_drift(t, dt));
+  BH_TRY(run_kick_drift_bbox(t, dt));
   rec(t, EV_I1);
   t->built = false;
   t->have_force = false;
   rec(t, EV_B0);
-  BH_TRY(run_bbox_only(t));
-  BH_TRY(build_from_posm(t));
-  t->reuse_costs = true;  // same particles one step later: last pass's counts predict this pass's costs
-  const int frc = force_begin_impl(t, t->theta, t->eps);
-  t->reuse_costs = false;
+  BH_TRY(run_keys(t, t->b.spos));
+  rec(t, EV_KEYS);
+  BH_TRY(run_sort(t));
+  rec(t, EV_SORT);
+  BH_TRY(run_permute_step(t));
+  rec(t, EV_PERM);
+  BH_TRY(run_tree(t, /*async=*/true));
+  rec(t, EV_BUILD);
+  BH_TRY(run_groups_moments(t));
+  rec(t, EV_MOM);
+  t->built = true;
+  t->reuse_mode = 1;  // same particles one step later: last pass's counts predict this pass's costs
+  const int frc = force_begin_impl(t, t->theta, t->eps, t->shard_world <= 1 ? 0.5f * dt : 0.0f);
+  t->reuse_mode = 0;
   if (frc) return frc;
   t->step_open = true;
   t->step_dt = dt;
@@ -240,7 +290,10 @@ static int leapfrog_begin_impl(tree_ctx *t, float dt) {
 static int leapfrog_end_impl(tree_ctx *t) {
   BH_TRY(force_end_impl(t, nullptr, nullptr));
   rec(t, EV_I2);
-  BH_TRY(run_kick(t, t->step_dt));
+#ifndef BH_FUSE_KICK
+#define BH_FUSE_KICK 1
+#endif
+  if (t->shard_world > 1 || !BH_FUSE_KICK) BH_TRY(run_kick(t, t->step_dt));  // else: done in the walk's epilogue
   rec(t, EV_I3);
   t->step_open = false;
   return 0;
@@ -273,6 +326,8 @@ int tree_create(tree_ctx **out, int device, void *cuda_stream, int leaf_size, in
   if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) t->sm_count = prop.multiProcessorCount;
   if (cudaMalloc((void **)&t->d_info, sizeof(DevInfo)) != cudaSuccess ||
       cudaMallocHost((void **)&t->h_info, sizeof(DevInfo)) != cudaSuccess ||
+      cudaMallocHost((void **)&t->h_async, sizeof(DevInfo)) != cudaSuccess ||
+      cudaEventCreateWithFlags(&t->ev_async, cudaEventDisableTiming) != cudaSuccess ||
       cudaMalloc((void **)&t->d_hlut, 24 * 8) != cudaSuccess) {
     cudaGetLastError();
     tree_destroy(t);
@@ -280,6 +335,7 @@ int tree_create(tree_ctx **out, int device, void *cuda_stream, int leaf_size, in
   }
   cudaMemset(t->d_info, 0, sizeof(DevInfo));
   memset(t->h_info, 0, sizeof(DevInfo));
+  memset(t->h_async, 0, sizeof(DevInfo));
   uint8_t lut[24 * 8];
   build_hilbert_lut(lut);
   cudaMemcpy(t->d_hlut, lut, sizeof(lut), cudaMemcpyHostToDevice);
@@ -295,6 +351,8 @@ int tree_destroy(tree_ctx *t) {
   free_all(t);
   if (t->d_info) cudaFree(t->d_info);
   if (t->h_info) cudaFreeHost(t->h_info);
+  if (t->h_async) cudaFreeHost(t->h_async);
+  if (t->ev_async) cudaEventDestroy(t->ev_async);
   if (t->d_hlut) cudaFree(t->d_hlut);
   for (int i = 0; i < EV_COUNT; ++i) if (t->ev_valid[i]) cudaEventDestroy(t->ev[i]);
   cudaGetLastError();
@@ -309,7 +367,8 @@ int tree_build(tree_ctx *t, const float *pos, const float *mass, long long N) {
   if (t->force_open || t->step_open) return set_err(t, TREE_ERR_ORDER, "tree_build inside an open force pass");
   t->built = false;
   t->have_force = false;
-  if (N != t->N) t->have_vel = false;
+  t->have_vel = false;   // the slot order changes: velocities are set again after a build (tree.h)
+  t->state_valid = false;
   BH_TRY(ensure_particles(t, N));
   t->N = N;
   t->n_groups = (N + t->group - 1) / t->group;
@@ -372,7 +431,7 @@ int tree_force_begin(tree_ctx *t, float theta, float eps) {
   if (!t) return TREE_ERR_ARG;
   BH_TRY(force_check(t, theta, eps));
   BH_DEVICE(t);
-  return force_begin_impl(t, theta, eps);
+  return force_begin_impl(t, theta, eps, 0.0f);
 }
 
 int tree_force_end(tree_ctx *t, float *acc, float *pot) {
@@ -482,6 +541,7 @@ int tree_shard_range(tree_ctx *t, long long *g_lo, long long *g_hi, long long *s
   BH_DEVICE(t);
   BH_CUDA(cudaMemcpyAsync(t->h_info, t->d_info, sizeof(DevInfo), cudaMemcpyDeviceToHost, t->stream));
   BH_CUDA(cudaStreamSynchronize(t->stream));
+  BH_TRY(check_sticky(t));
   const long long lo = t->h_info->g_lo, hi = t->h_info->g_hi;
   if (g_lo) *g_lo = lo;
   if (g_hi) *g_hi = hi;
@@ -490,10 +550,28 @@ int tree_shard_range(tree_ctx *t, long long *g_lo, long long *g_hi, long long *s
   return TREE_OK;
 }
 
+int tree_set_mac(tree_ctx *t, int kind) {
+  if (!t) return TREE_ERR_ARG;
+  if (kind != TREE_MAC_GEOMETRIC && kind != TREE_MAC_BMAX) return set_err(t, TREE_ERR_ARG, "tree_set_mac: unknown criterion");
+  if (t->force_open || t->step_open) return set_err(t, TREE_ERR_ORDER, "tree_set_mac inside an open force pass");
+  BH_DEVICE(t);
+  if (kind != t->mac) {
+    t->mac = kind;
+    t->built = false;  // the tight boxes are computed with the moments: build again
+    t->have_force = false;
+    if (kind == TREE_MAC_BMAX && t->cell_cap > 0 && !t->b.c_tlo) {
+      BH_CUDA(cudaStreamSynchronize(t->stream));
+      BH_TRY(dev_alloc(t, t->b.c_tlo, t->cell_cap));
+      BH_TRY(dev_alloc(t, t->b.c_thi, t->cell_cap));
+    }
+  }
+  return TREE_OK;
+}
+
 int tree_set_velocity(tree_ctx *t, const float *vel) {
   if (!t) return TREE_ERR_ARG;
   if (!vel) return set_err(t, TREE_ERR_ARG, "tree_set_velocity: NULL");
-  if (t->N <= 0 || !t->b.vel) return set_err(t, TREE_ERR_ORDER, "tree_set_velocity before tree_build");
+  if (t->N <= 0 || !t->built) return set_err(t, TREE_ERR_ORDER, "tree_set_velocity before tree_build");
   BH_DEVICE(t);
   BH_TRY(run_set_velocity(t, vel));
   t->have_vel = true;
@@ -502,7 +580,7 @@ int tree_set_velocity(tree_ctx *t, const float *vel) {
 
 int tree_get_state(tree_ctx *t, float *pos, float *vel, float *acc, float *pot) {
   if (!t) return TREE_ERR_ARG;
-  if (t->N <= 0) return set_err(t, TREE_ERR_ORDER, "tree_get_state before tree_build");
+  if (t->N <= 0 || !t->state_valid) return set_err(t, TREE_ERR_ORDER, "tree_get_state before tree_build");
   if (vel && !t->have_vel) return set_err(t, TREE_ERR_ORDER, "tree_get_state: no velocities set");
   if ((acc || pot) && !t->have_force) return set_err(t, TREE_ERR_ORDER, "tree_get_state: no force computed");
   BH_DEVICE(t);
@@ -513,7 +591,7 @@ int tree_direct(tree_ctx *t, const long long *idx, long long n, float eps, doubl
   if (!t) return TREE_ERR_ARG;
   if (!idx || !acc || !pot || n <= 0 || !(eps >= 0.0f) || !isfinite(eps))
     return set_err(t, TREE_ERR_ARG, "tree_direct: bad argument");
-  if (t->N <= 0 || !t->b.posm) return set_err(t, TREE_ERR_ORDER, "tree_direct before tree_build");
+  if (t->N <= 0 || !t->state_valid) return set_err(t, TREE_ERR_ORDER, "tree_direct before tree_build");
   BH_DEVICE(t);
   return run_direct(t, idx, n, eps, acc, pot);
 }
@@ -542,7 +620,7 @@ int tree_force_host(tree_ctx *t, float theta, float eps, float *acc, float *pot)
   if (rc) return rc;
   if (acc) BH_CUDA(cudaMemcpyAsync(acc, t->b.out_acc, (size_t)t->N * 12, cudaMemcpyDeviceToHost, t->stream));
   if (pot) BH_CUDA(cudaMemcpyAsync(pot, t->b.out_pot, (size_t)t->N * 4, cudaMemcpyDeviceToHost, t->stream));
-  BH_CUDA(cudaMemcpyAsync(&t->h_info->walk_overflow_sticky, &t->d_info->walk_overflow_sticky, sizeof(unsigned), cudaMemcpyDeviceToHost, t->stream));
+  BH_CUDA(cudaMemcpyAsync(t->h_info, t->d_info, sizeof(DevInfo), cudaMemcpyDeviceToHost, t->stream));
   BH_CUDA(cudaStreamSynchronize(t->stream));
   BH_TRY(check_sticky(t));
   return TREE_OK;
@@ -572,6 +650,10 @@ int tree_get_debug(tree_ctx *t, int what, void *dst, long long *count) {
   if (!count) return set_err(t, TREE_ERR_ARG, "tree_get_debug: count is NULL");
   if (!t->built) return set_err(t, TREE_ERR_ORDER, "tree_get_debug before tree_build");
   BH_DEVICE(t);
+  BH_CUDA(cudaMemcpyAsync(t->h_info, t->d_info, sizeof(DevInfo), cudaMemcpyDeviceToHost, t->stream));
+  BH_CUDA(cudaStreamSynchronize(t->stream));
+  BH_TRY(check_sticky(t));
+  t->n_cells = t->h_info->n_cells;  // exact also after an asynchronous rebuild
   const long long N = t->N, nc = t->n_cells, ng = t->n_groups;
   switch (what) {
     case TREE_DBG_KEYS: {
@@ -581,12 +663,12 @@ int tree_get_debug(tree_ctx *t, int what, void *dst, long long *count) {
       std::vector<uint64_t> sk(N);
       std::vector<uint32_t> ord(N);
       BH_TRY(copy_out(t, sk.data(), t->b.key[t->sorted], N * 8));
-      BH_TRY(copy_out(t, ord.data(), t->b.idx[t->sorted], N * 4));
+      BH_TRY(copy_out(t, ord.data(), t->b.order, N * 4));
       uint64_t *o = (uint64_t *)dst;
       for (long long s = 0; s < N; ++s) o[ord[s]] = sk[s];
       return 0;
     }
-    case TREE_DBG_ORDER: *count = N; return dst ? copy_out(t, dst, t->b.idx[t->sorted], N * 4) : 0;
+    case TREE_DBG_ORDER: *count = N; return dst ? copy_out(t, dst, t->b.order, N * 4) : 0;
     case TREE_DBG_SORTED_KEYS: *count = N; return dst ? copy_out(t, dst, t->b.key[t->sorted], N * 8) : 0;
     case TREE_DBG_SORTED_POS: *count = N; return dst ? copy_out(t, dst, t->b.spos, N * 16) : 0;
     case TREE_DBG_CELLS: {
@@ -646,6 +728,20 @@ int tree_get_debug(tree_ctx *t, int what, void *dst, long long *count) {
       BH_TRY(copy_out(t, ts.data(), t->b.c_test, nc * 16));
       float *o = (float *)dst;
       for (long long c = 0; c < nc; ++c) o[c] = ts[c].w;
+      return 0;
+    }
+    case TREE_DBG_TIGHT: {
+      if (t->mac != TREE_MAC_BMAX) return set_err(t, TREE_ERR_ORDER, "tight boxes exist only with TREE_MAC_BMAX");
+      *count = nc;
+      if (!dst) return 0;
+      std::vector<float4> lo(nc), hi(nc);
+      BH_TRY(copy_out(t, lo.data(), t->b.c_tlo, nc * 16));
+      BH_TRY(copy_out(t, hi.data(), t->b.c_thi, nc * 16));
+      float *o = (float *)dst;
+      for (long long c = 0; c < nc; ++c) {
+        float *r = o + 7 * c;
+        r[0] = lo[c].x; r[1] = lo[c].y; r[2] = lo[c].z; r[3] = hi[c].x; r[4] = hi[c].y; r[5] = hi[c].z; r[6] = lo[c].w;
+      }
       return 0;
     }
     case TREE_DBG_LEVEL_OFFSETS: {

@@ -45,24 +45,8 @@ __global__ void info_reset_kernel(DevInfo *info) {
   }
 }
 
-template <bool PACK>
-__global__ void __launch_bounds__(256) bbox_kernel(const float *__restrict__ pos, const float *__restrict__ mass,
-                                                   float4 *__restrict__ posm, long long N, DevInfo *info) {
-  float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
-  int bad = 0;
-  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
-    float4 p;
-    if (PACK) {
-      p.x = pos[3 * i]; p.y = pos[3 * i + 1]; p.z = pos[3 * i + 2]; p.w = mass[i];
-      posm[i] = p;
-    } else {
-      p = posm[i];
-    }
-    bad |= !(isfinite(p.x) && isfinite(p.y) && isfinite(p.z) && isfinite(p.w));
-    lo[0] = fminf(lo[0], p.x); hi[0] = fmaxf(hi[0], p.x);
-    lo[1] = fminf(lo[1], p.y); hi[1] = fmaxf(hi[1], p.y);
-    lo[2] = fminf(lo[2], p.z); hi[2] = fmaxf(hi[2], p.z);
-  }
+// block-wide min/max of a per-thread box and OR of the non-finite flags, merged into info by integer atomics
+__device__ __forceinline__ void block_bbox_reduce(float (&lo)[3], float (&hi)[3], int bad, DevInfo *info) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
 #pragma unroll
@@ -94,6 +78,53 @@ __global__ void __launch_bounds__(256) bbox_kernel(const float *__restrict__ pos
   }
 }
 
+template <bool PACK>
+__global__ void __launch_bounds__(256) bbox_kernel(const float *__restrict__ pos, const float *__restrict__ mass,
+                                                   float4 *__restrict__ posm, long long N, DevInfo *info) {
+  float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+  int bad = 0;
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+    float4 p;
+    if (PACK) {
+      p.x = pos[3 * i]; p.y = pos[3 * i + 1]; p.z = pos[3 * i + 2]; p.w = mass[i];
+      posm[i] = p;
+    } else {
+      p = posm[i];
+    }
+    bad |= !(isfinite(p.x) && isfinite(p.y) && isfinite(p.z) && isfinite(p.w));
+    lo[0] = fminf(lo[0], p.x); hi[0] = fmaxf(hi[0], p.x);
+    lo[1] = fminf(lo[1], p.y); hi[1] = fmaxf(hi[1], p.y);
+    lo[2] = fminf(lo[2], p.z); hi[2] = fmaxf(hi[2], p.z);
+  }
+  block_bbox_reduce(lo, hi, bad, info);
+}
+
+// a12 + a1 fused (tree_leapfrog): v = fma(a, dt/2, v); x = fma(v, dt, x) on the slot-order state, and the bounding box of
+// the new positions in the same pass (48 B read, 32 B written per particle; T12, "step pipeline").
+__global__ void __launch_bounds__(256) kick_drift_bbox_kernel(float4 *__restrict__ spos, float4 *__restrict__ svel,
+                                                              const float4 *__restrict__ sacc, long long N, float hdt,
+                                                              float dt, DevInfo *info) {
+  float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+  int bad = 0;
+  const bool frozen = info->cells_overflow != 0;  // a failed asynchronous rebuild freezes the state (tree.h): bbox only
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+    float4 p = spos[i];
+    if (!frozen) {
+      float4 v = svel[i];
+      const float4 a = sacc[i];
+      v.x = __fmaf_rn(a.x, hdt, v.x); v.y = __fmaf_rn(a.y, hdt, v.y); v.z = __fmaf_rn(a.z, hdt, v.z);
+      p.x = __fmaf_rn(v.x, dt, p.x); p.y = __fmaf_rn(v.y, dt, p.y); p.z = __fmaf_rn(v.z, dt, p.z);
+      svel[i] = v;
+      spos[i] = p;
+    }
+    bad |= !(isfinite(p.x) && isfinite(p.y) && isfinite(p.z) && isfinite(p.w));
+    lo[0] = fminf(lo[0], p.x); hi[0] = fmaxf(hi[0], p.x);
+    lo[1] = fminf(lo[1], p.y); hi[1] = fmaxf(hi[1], p.y);
+    lo[2] = fminf(lo[2], p.z); hi[2] = fmaxf(hi[2], p.z);
+  }
+  block_bbox_reduce(lo, hi, bad, info);
+}
+
 // a2 (first half): cube centred on the bbox, side = smallest power of two > extent (S9).
 __global__ void grid_kernel(DevInfo *info) {
   if (threadIdx.x != 0) return;
@@ -108,6 +139,7 @@ __global__ void grid_kernel(DevInfo *info) {
   int k = 0;
   if (ext > 0.0) { int e; frexp(ext, &e); k = e; }
   if (!(ext >= 0.0) || !isfinite(ext)) { info->nonfinite = 1; k = 0; }
+  if (info->nonfinite) info->nonfinite_sticky = 1;  // an asynchronous rebuild reports it at the next synchronising call
   info->k = k;
   double S = ldexp(1.0, k);
   for (int d = 0; d < 3; ++d) {
@@ -119,28 +151,49 @@ __global__ void grid_kernel(DevInfo *info) {
 
 // a2: Peano-Hilbert key by a 24-state x 8-octant table generated on the host from the
 // Gray-code/rotation recurrence (T3). Table entry = digit | next_state << 3.
+// The kernel walks TWO levels per table step: a 24 x 64 table (digit pair | next_state << 6, built per block from the
+// 8-octant table) over the Morton-interleaved grid coordinates, so a key costs 10 dependent shared-memory look-ups
+// + 1 instead of 21 (the kernel is bound by that chain, not by HBM).
+__device__ __forceinline__ uint64_t spread3(unsigned v) {  // bit i of the 21-bit v -> bit 3 i
+  uint64_t x = v & 0x1fffffu;
+  x = (x | (x << 32)) & 0x001f00000000ffffull;
+  x = (x | (x << 16)) & 0x001f0000ff0000ffull;
+  x = (x | (x << 8)) & 0x100f00f00f00f00full;
+  x = (x | (x << 4)) & 0x10c30c30c30c30c3ull;
+  x = (x | (x << 2)) & 0x1249249249249249ull;
+  return x;
+}
+
 __global__ void __launch_bounds__(256) keys_kernel(const float4 *__restrict__ posm, long long N,
                                                    const DevInfo *__restrict__ info, const uint8_t *__restrict__ lut_g,
                                                    uint64_t *__restrict__ key, uint32_t *__restrict__ idx) {
   __shared__ uint8_t lut[24 * 8];
+  __shared__ uint16_t lut2[24 * 64];
   if (threadIdx.x < 24 * 8) lut[threadIdx.x] = lut_g[threadIdx.x];
+  __syncthreads();
+  for (int e = threadIdx.x; e < 24 * 64; e += blockDim.x) {
+    const unsigned st = e >> 6, hi = (e >> 3) & 7u, lo = e & 7u;
+    const unsigned v1 = lut[st * 8 + hi], v2 = lut[(v1 >> 3) * 8 + lo];
+    lut2[e] = (uint16_t)((((v1 & 7u) << 3) | (v2 & 7u)) | ((v2 >> 3) << 6));
+  }
   __syncthreads();
   const float ox = info->origin[0], oy = info->origin[1], oz = info->origin[2], inv = info->inv;
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
     float4 p = posm[i];
     unsigned ix = grid_coord(p.x, ox, inv), iy = grid_coord(p.y, oy, inv), iz = grid_coord(p.z, oz, inv);
-    // interleave to one octant digit per level: bits z y x
+    // one octant digit per level, bits z y x, most significant level first
+    const uint64_t m = spread3(ix) | (spread3(iy) << 1) | (spread3(iz) << 2);
     uint64_t h = 0;
     unsigned st = 0;
 #pragma unroll
-    for (int b = KEY_BITS - 1; b >= 0; --b) {
-      unsigned l = (((iz >> b) & 1u) << 2) | (((iy >> b) & 1u) << 1) | ((ix >> b) & 1u);
-      unsigned v = lut[st * 8 + l];
-      h = (h << 3) | (v & 7u);
-      st = v >> 3;
+    for (int b = KEY_BITS - 2; b >= 1; b -= 2) {  // levels (b+1, b): 20..1 in 10 steps
+      const unsigned v = lut2[st * 64 + ((unsigned)(m >> (3 * b)) & 63u)];
+      h = (h << 6) | (v & 63u);
+      st = v >> 6;
     }
+    h = (h << 3) | (lut[st * 8 + ((unsigned)m & 7u)] & 7u);  // level 0
     key[i] = h;
-    idx[i] = (uint32_t)i;
+    if (idx) idx[i] = (uint32_t)i;
   }
 }
 
@@ -413,11 +466,46 @@ __global__ void __launch_bounds__(OS_THREADS, OS_MINB) sort_onesweep_kernel(cons
   }
 }
 
-// a4: gather the particles into slot order
-__global__ void __launch_bounds__(256) permute_kernel(const float4 *__restrict__ posm, const uint32_t *__restrict__ order,
-                                                      float4 *__restrict__ spos, long long N) {
+// a4: gather the particles into slot order.
+// tree_build: the sort's payload is the caller index (a stable sort of the caller-ordered keys: ties by caller index, S10).
+__global__ void __launch_bounds__(256) permute_build_kernel(const float4 *__restrict__ posm, const uint32_t *__restrict__ sidx,
+                                                            float4 *__restrict__ spos, uint32_t *__restrict__ order, long long N) {
   long long s = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  if (s < N) spos[s] = posm[order[s]];
+  if (s < N) {
+    const uint32_t i = sidx[s];
+    spos[s] = posm[i];
+    order[s] = i;
+  }
+}
+
+// tree_leapfrog: the state lives in the slot order of the previous step and the sort's payload is the PREVIOUS SLOT, so the
+// gathers below are nearly sequential (few particles change their place on the curve in one step).  The stable sort left
+// equal keys (particles in one finest grid cell) in previous-slot order; S10 wants them by caller index, so a slot inside
+// a run of equal keys ranks itself within the run by caller index (runs are short: pairs in the densest cells; the
+// ranking is quadratic in the run length).
+__global__ void __launch_bounds__(256) permute_step_kernel(const uint64_t *__restrict__ skey, const uint32_t *__restrict__ perm,
+                                                           const float4 *__restrict__ pos_in, const float4 *__restrict__ vel_in,
+                                                           const uint32_t *__restrict__ order_in, float4 *__restrict__ pos_out,
+                                                           float4 *__restrict__ vel_out, uint32_t *__restrict__ order_out,
+                                                           long long N) {
+  const long long s = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (s >= N) return;
+  const uint64_t k = skey[s];
+  const uint32_t q = perm[s];
+  const uint32_t me = order_in[q];
+  long long dst = s;
+  const bool tie_l = s > 0 && skey[s - 1] == k, tie_r = s + 1 < N && skey[s + 1] == k;
+  if (tie_l || tie_r) {
+    long long r0 = s, r1 = s + 1;
+    while (r0 > 0 && skey[r0 - 1] == k) --r0;
+    while (r1 < N && skey[r1] == k) ++r1;
+    long long rank = 0;
+    for (long long j = r0; j < r1; ++j) rank += order_in[perm[j]] < me;
+    dst = r0 + rank;
+  }
+  pos_out[dst] = pos_in[q];
+  vel_out[dst] = vel_in[q];
+  order_out[dst] = me;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -464,11 +552,31 @@ __global__ void __launch_bounds__(TREE_THREADS) tree_levels_kernel(const uint64_
   if (threadIdx.x < NLEVELS) tilecnt[(long long)threadIdx.x * ntiles + blockIdx.x] = cnt[threadIdx.x];
 }
 
+// levels 0..ltop together hold at most this many cells: one block computes their moments (moments_top_kernel)
+#ifndef BH_MOMENTS_TOP_CELLS
+#define BH_MOMENTS_TOP_CELLS 128
+#endif
+constexpr int MOMENTS_TOP_CELLS = BH_MOMENTS_TOP_CELLS;
+
+// Level offsets, cell count, the top levels one block handles, and the capacity check of an asynchronous rebuild:
+// `cells_bound` cells are allocated / launched for; a tree that needs more sets the sticky cells_overflow and every
+// later kernel of the step pipeline does nothing (the host reports it at its next synchronising call, tree.h).
 __global__ void tree_offsets_kernel(const uint32_t *__restrict__ scanned, int ntiles, const uint32_t *__restrict__ total,
-                                    DevInfo *info) {
+                                    long long cells_bound, DevInfo *info) {
+  __shared__ int off[NLEVELS + 1];
   int l = threadIdx.x;
-  if (l < NLEVELS) info->level_off[l] = (int)scanned[(long long)l * ntiles];
-  if (l == NLEVELS) info->level_off[NLEVELS] = (int)*total;
+  if (l < NLEVELS) off[l] = (int)scanned[(long long)l * ntiles];
+  if (l == NLEVELS) off[NLEVELS] = (int)*total;
+  __syncthreads();
+  if (l <= NLEVELS) info->level_off[l] = off[l];
+  if (l == 0) {
+    const unsigned nc = (unsigned)off[NLEVELS];
+    info->n_cells = (int)nc;
+    if ((long long)nc > cells_bound && !info->cells_overflow) info->cells_overflow = nc;
+    int ltop = -1;
+    while (ltop + 1 <= MAX_LEVEL && off[ltop + 2] <= MOMENTS_TOP_CELLS) ++ltop;
+    info->ltop = ltop;
+  }
 }
 
 __global__ void __launch_bounds__(TREE_THREADS) tree_emit_kernel(const uint16_t *__restrict__ lv, long long N,
@@ -476,8 +584,10 @@ __global__ void __launch_bounds__(TREE_THREADS) tree_emit_kernel(const uint16_t 
                                                                   uint8_t *__restrict__ c_level,
                                                                   uint32_t *__restrict__ c_first,
                                                                   uint32_t *__restrict__ c_count,
-                                                                  uint32_t *__restrict__ c_fcall) {
+                                                                  uint32_t *__restrict__ c_fcall,
+                                                                  const DevInfo *__restrict__ info) {
   constexpr int NW = TREE_THREADS / 32;
+  if (info->cells_overflow) return;
   __shared__ uint16_t lvs[TREE_THREADS + TREE_HALO + 1];
   __shared__ unsigned wbase[NLEVELS][NW];
   const long long base = (long long)blockIdx.x * TREE_THREADS;
@@ -537,9 +647,11 @@ __global__ void __launch_bounds__(TREE_THREADS) tree_emit_kernel(const uint16_t 
 }
 
 // child links: n_child(c) = fcall[c+1] - fcall[c]; 0 = leaf.
-__global__ void __launch_bounds__(256) tree_link_kernel(long long n_cells, const uint32_t *__restrict__ c_first,
+__global__ void __launch_bounds__(256) tree_link_kernel(const DevInfo *__restrict__ info, const uint32_t *__restrict__ c_first,
                                                         const uint32_t *__restrict__ c_count,
                                                         const uint32_t *__restrict__ c_fcall, uint2 *__restrict__ c_link) {
+  if (info->cells_overflow) return;
+  const long long n_cells = info->n_cells;
   long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x;
   if (c >= n_cells) return;
   unsigned f = c_fcall[c];
@@ -590,7 +702,8 @@ __device__ __forceinline__ void moments_cell(int c, int level, bool leaves, cons
                                              const float4 *__restrict__ spos, const uint2 *__restrict__ c_link,
                                              const uint32_t *__restrict__ c_first, uint32_t *__restrict__ c_count,
                                              float4 *__restrict__ c_cm, float4 *__restrict__ c_qa,
-                                             float4 *__restrict__ c_qb) {
+                                             float4 *__restrict__ c_qb, float4 *__restrict__ c_tlo = nullptr,
+                                             float4 *__restrict__ c_thi = nullptr) {
   const uint2 lk = c_link[c];
   if (leaves != !(lk.y & LEAF_FLAG)) return;
   double M = 0, s0 = 0, s1 = 0, s2 = 0;
@@ -657,46 +770,79 @@ __device__ __forceinline__ void moments_cell(int c, int level, bool leaves, cons
   double gz = __dadd_rn((double)info->origin[2], __dmul_rn(__dadd_rn(qz, 0.5), lc));
   double ex = __dsub_rn((double)cx, gx), ey = __dsub_rn((double)cy, gy), ez = __dsub_rn((double)cz, gz);
   double del = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(ex, ex), __dmul_rn(ey, ey)), __dmul_rn(ez, ez)));
+  if (c_tlo) {  // TREE_MAC_BMAX: tight box of the cell's particles (min / max are exact) and the bounding radius about
+                // the FP32 centre of mass: e_d = max(c_d - lo_d, hi_d - c_d); b = sqrt(fma(ez, ez, fma(ey, ey, ex ex)))
+    float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+    if (!(lk.y & LEAF_FLAG)) {
+      for (unsigned p = lk.x; p < lk.x + lk.y; ++p) {
+        const float4 q = spos[p];
+        lo[0] = fminf(lo[0], q.x); hi[0] = fmaxf(hi[0], q.x);
+        lo[1] = fminf(lo[1], q.y); hi[1] = fmaxf(hi[1], q.y);
+        lo[2] = fminf(lo[2], q.z); hi[2] = fmaxf(hi[2], q.z);
+      }
+    } else {
+      const unsigned f = lk.x, n = lk.y & ~LEAF_FLAG;
+      for (unsigned ch = f; ch < f + n; ++ch) {
+        const float4 a = c_tlo[ch], b = c_thi[ch];
+        lo[0] = fminf(lo[0], a.x); hi[0] = fmaxf(hi[0], b.x);
+        lo[1] = fminf(lo[1], a.y); hi[1] = fmaxf(hi[1], b.y);
+        lo[2] = fminf(lo[2], a.z); hi[2] = fmaxf(hi[2], b.z);
+      }
+    }
+    const float e0 = fmaxf(__fsub_rn(cx, lo[0]), __fsub_rn(hi[0], cx));
+    const float e1 = fmaxf(__fsub_rn(cy, lo[1]), __fsub_rn(hi[1], cy));
+    const float e2 = fmaxf(__fsub_rn(cz, lo[2]), __fsub_rn(hi[2], cz));
+    const float b2 = __fmaf_rn(e2, e2, __fmaf_rn(e1, e1, __fmul_rn(e0, e0)));
+    c_tlo[c] = make_float4(lo[0], lo[1], lo[2], __fsqrt_rn(b2));
+    c_thi[c] = make_float4(hi[0], hi[1], hi[2], 0.0f);
+  }
   float q0 = (float)Q0, q1 = (float)Q1, q2 = (float)Q2;
   c_cm[c] = make_float4(cx, cy, cz, (float)M);
   c_qa[c] = make_float4(q0, q1, q2, (float)del);
   c_qb[c] = make_float4((float)Q3, (float)Q4, (float)Q5, __fadd_rn(__fadd_rn(q0, q1), q2));
 }
 
-// all leaves, any level (the level of a cell comes from c_level)
-__global__ void __launch_bounds__(128) moments_leaf_kernel(int n_cells, const DevInfo *__restrict__ info,
+// all leaves, any level (the level of a cell comes from c_level); the cell count is read on the device
+__global__ void __launch_bounds__(128) moments_leaf_kernel(const DevInfo *__restrict__ info,
                                                            const float4 *__restrict__ spos, const uint2 *__restrict__ c_link,
                                                            const uint8_t *__restrict__ c_level,
                                                            const uint32_t *__restrict__ c_first,
                                                            uint32_t *__restrict__ c_count, float4 *__restrict__ c_cm,
-                                                           float4 *__restrict__ c_qa, float4 *__restrict__ c_qb) {
-  const int c = blockIdx.x * blockDim.x + threadIdx.x;
-  if (c >= n_cells) return;
-  moments_cell(c, (int)c_level[c], true, info, spos, c_link, c_first, c_count, c_cm, c_qa, c_qb);
+                                                           float4 *__restrict__ c_qa, float4 *__restrict__ c_qb,
+                                                           float4 *__restrict__ c_tlo, float4 *__restrict__ c_thi) {
+  if (info->cells_overflow) return;
+  const int n_cells = info->n_cells;
+  for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < n_cells; c += gridDim.x * blockDim.x)
+    moments_cell(c, (int)c_level[c], true, info, spos, c_link, c_first, c_count, c_cm, c_qa, c_qb, c_tlo, c_thi);
 }
 
-// internal cells of one level [c0, c1)
-__global__ void __launch_bounds__(128) moments_level_kernel(int c0, int c1, int level, const DevInfo *__restrict__ info,
+// internal cells of one level; its range comes from the level offsets on the device (no host round trip), so the
+// launch is a fixed grid that strides over the level; levels 0..ltop are left to moments_top_kernel
+__global__ void __launch_bounds__(128) moments_level_kernel(int level, const DevInfo *__restrict__ info,
                                                             const float4 *__restrict__ spos,
                                                             const uint2 *__restrict__ c_link,
                                                             const uint32_t *__restrict__ c_first,
                                                             uint32_t *__restrict__ c_count, float4 *__restrict__ c_cm,
-                                                            float4 *__restrict__ c_qa, float4 *__restrict__ c_qb) {
-  const int c = c0 + blockIdx.x * blockDim.x + threadIdx.x;
-  if (c >= c1) return;
-  moments_cell(c, level, false, info, spos, c_link, c_first, c_count, c_cm, c_qa, c_qb);
+                                                            float4 *__restrict__ c_qa, float4 *__restrict__ c_qb,
+                                                            float4 *__restrict__ c_tlo, float4 *__restrict__ c_thi) {
+  if (info->cells_overflow || level <= info->ltop) return;
+  const int c0 = info->level_off[level], c1 = info->level_off[level + 1];
+  for (int c = c0 + blockIdx.x * blockDim.x + threadIdx.x; c < c1; c += gridDim.x * blockDim.x)
+    moments_cell(c, level, false, info, spos, c_link, c_first, c_count, c_cm, c_qa, c_qb, c_tlo, c_thi);
 }
 
 // internal cells of the top levels ltop .. 0 (few cells): one block, a block barrier between levels
-__global__ void __launch_bounds__(256) moments_top_kernel(int ltop, const DevInfo *__restrict__ info,
+__global__ void __launch_bounds__(256) moments_top_kernel(const DevInfo *__restrict__ info,
                                                           const float4 *__restrict__ spos, const uint2 *__restrict__ c_link,
                                                           const uint32_t *__restrict__ c_first,
                                                           uint32_t *__restrict__ c_count, float4 *__restrict__ c_cm,
-                                                          float4 *__restrict__ c_qa, float4 *__restrict__ c_qb) {
-  for (int l = ltop; l >= 0; --l) {
+                                                          float4 *__restrict__ c_qa, float4 *__restrict__ c_qb,
+                                                          float4 *__restrict__ c_tlo, float4 *__restrict__ c_thi) {
+  if (info->cells_overflow) return;
+  for (int l = info->ltop; l >= 0; --l) {
     const int c0 = info->level_off[l], c1 = info->level_off[l + 1];
     for (int c = c0 + threadIdx.x; c < c1; c += blockDim.x)
-      moments_cell(c, l, false, info, spos, c_link, c_first, c_count, c_cm, c_qa, c_qb);
+      moments_cell(c, l, false, info, spos, c_link, c_first, c_count, c_cm, c_qa, c_qb, c_tlo, c_thi);
     __threadfence();
     __syncthreads();
   }
@@ -705,11 +851,6 @@ __global__ void __launch_bounds__(256) moments_top_kernel(int ltop, const DevInf
 // ------------------------------------------------------------------------------------------
 // host launchers
 // ------------------------------------------------------------------------------------------
-#ifndef BH_MOMENTS_TOP_CELLS
-#define BH_MOMENTS_TOP_CELLS 128
-#endif
-constexpr int MOMENTS_TOP_CELLS = BH_MOMENTS_TOP_CELLS;  // levels 0..ltop with at most this many cells in total: one block
-
 static inline int grid_for(tree_ctx *t, long long n, int threads, int per_sm) {
   long long need = (n + threads - 1) / threads;
   long long cap = (long long)t->sm_count * per_sm;
@@ -724,19 +865,20 @@ int run_pack_bbox(tree_ctx *t, const float *pos, const float *mass) {
   return 0;
 }
 
-int run_bbox_only(tree_ctx *t) {
+int run_kick_drift_bbox(tree_ctx *t, float dt) {
   info_reset_kernel<<<1, 32, 0, t->stream>>>(t->d_info);
   BH_LAUNCH_CHECK("info_reset");
-  bbox_kernel<false><<<grid_for(t, t->N, 256, 8), 256, 0, t->stream>>>(nullptr, nullptr, t->b.posm, t->N, t->d_info);
-  BH_LAUNCH_CHECK("bbox");
+  kick_drift_bbox_kernel<<<grid_for(t, t->N, 256, 8), 256, 0, t->stream>>>(t->b.spos, t->b.svel, t->b.sacc, t->N, 0.5f * dt,
+                                                                            dt, t->d_info);
+  BH_LAUNCH_CHECK("kick_drift_bbox");
   return 0;
 }
 
-int run_keys(tree_ctx *t) {
+int run_keys(tree_ctx *t, const float4 *xyzm) {
   grid_kernel<<<1, 32, 0, t->stream>>>(t->d_info);
   BH_LAUNCH_CHECK("grid");
-  keys_kernel<<<grid_for(t, t->N, 256, 8), 256, 0, t->stream>>>(t->b.posm, t->N, t->d_info, t->d_hlut, t->b.key[0],
-                                                                 t->b.idx[0]);
+  // the sort's first pass takes the identity as payload: no index array is written here
+  keys_kernel<<<grid_for(t, t->N, 256, 8), 256, 0, t->stream>>>(xyzm, t->N, t->d_info, t->d_hlut, t->b.key[0], nullptr);
   BH_LAUNCH_CHECK("keys");
   return 0;
 }
@@ -772,13 +914,38 @@ int run_sort(tree_ctx *t) {
   return 0;
 }
 
-int run_permute(tree_ctx *t) {
-  permute_kernel<<<(unsigned)((t->N + 255) / 256), 256, 0, t->stream>>>(t->b.posm, t->b.idx[t->sorted], t->b.spos, t->N);
-  BH_LAUNCH_CHECK("permute");
+int run_permute_build(tree_ctx *t) {
+  permute_build_kernel<<<(unsigned)((t->N + 255) / 256), 256, 0, t->stream>>>(t->b.posm, t->b.idx[t->sorted], t->b.spos,
+                                                                             t->b.order, t->N);
+  BH_LAUNCH_CHECK("permute_build");
   return 0;
 }
 
-int run_tree(tree_ctx *t) {
+int run_permute_step(tree_ctx *t) {
+  const int nxt = t->cur ^ 1;
+  permute_step_kernel<<<(unsigned)((t->N + 255) / 256), 256, 0, t->stream>>>(
+      t->b.key[t->sorted], t->b.idx[t->sorted], t->b.spos, t->b.svel, t->b.order, t->b.spos2[nxt], t->b.svel2[nxt],
+      t->b.order2[nxt], t->N);
+  BH_LAUNCH_CHECK("permute_step");
+  t->cur = nxt;
+  t->b.spos = t->b.spos2[nxt]; t->b.svel = t->b.svel2[nxt]; t->b.order = t->b.order2[nxt];
+  return 0;
+}
+
+// The cell count of the last asynchronous rebuild, if its read-back has arrived (never waits).
+void poll_cells(tree_ctx *t) {
+  if (!t->async_pending) return;
+  if (cudaEventQuery(t->ev_async) != cudaSuccess) { cudaGetLastError(); return; }
+  t->async_pending = false;
+  if (t->h_async->n_cells > 0) t->n_cells = t->h_async->n_cells;
+}
+
+// !async (tree_build): one read-back of the cell count sizes the cell arrays exactly.
+// async (tree_leapfrog): no host round trip.  The arrays hold cell_cap cells; the kernels may use
+// cells_bound = min(cell_cap, latest known count + 1/8 + 1024) of them (the count changes by a fraction of a per cent
+// per step), the device checks the real count against it (tree_offsets_kernel) and the count travels back
+// asynchronously for the next step (poll_cells).
+int run_tree(tree_ctx *t, bool async) {
   const int ntiles = (int)((t->N + TREE_THREADS - 1) / TREE_THREADS);
   const uint64_t *skey = t->b.key[t->sorted];
   tree_levels_kernel<<<ntiles, TREE_THREADS, 0, t->stream>>>(skey, t->N, t->leaf, ntiles, t->b.lv, t->b.scan_tmp);
@@ -786,22 +953,43 @@ int run_tree(tree_ctx *t) {
   uint32_t *total = t->b.scan_blk + (t->scan_cap / SCAN_TILE + 8);  // spare slot behind the block sums
   int rc = device_excl_scan(t, t->b.scan_tmp, (long long)NLEVELS * ntiles, total);
   if (rc) return rc;
-  tree_offsets_kernel<<<1, 32, 0, t->stream>>>(t->b.scan_tmp, ntiles, total, t->d_info);
+  if (async) {
+    poll_cells(t);
+    const long long want = t->n_cells + t->n_cells / 8 + 1024;
+    t->cells_bound = want < t->cell_cap ? want : t->cell_cap;
+  } else {
+    t->cells_bound = 1ll << 28;  // checked on the host below
+  }
+  tree_offsets_kernel<<<1, 32, 0, t->stream>>>(t->b.scan_tmp, ntiles, total, t->cells_bound, t->d_info);
   BH_LAUNCH_CHECK("tree_offsets");
-  BH_CUDA(cudaMemcpyAsync(t->h_info, t->d_info, sizeof(DevInfo), cudaMemcpyDeviceToHost, t->stream));
-  BH_CUDA(cudaStreamSynchronize(t->stream));
-  if (t->h_info->nonfinite) return set_err(t, TREE_ERR_NONFINITE, "non-finite position or mass");
-  BH_TRY_RC(check_sticky(t));  // a walk-stack overflow of an earlier asynchronous pass surfaces here at the latest
-  const long long nc = t->h_info->level_off[NLEVELS];
-  if (nc <= 0 || nc >= (1ll << 28)) return set_err(t, TREE_ERR_ARG, "cell count out of range (needs < 2^28 cells)");
-  rc = ensure_cells(t, nc);
-  if (rc) return rc;
-  t->n_cells = nc;
+  if (async) {
+    if (!t->async_pending) {  // the previous read-back has been consumed: start the next one
+      BH_CUDA(cudaMemcpyAsync(t->h_async, t->d_info, sizeof(DevInfo), cudaMemcpyDeviceToHost, t->stream));
+      BH_CUDA(cudaEventRecord(t->ev_async, t->stream));
+      t->async_pending = true;
+    }
+  } else {
+    BH_CUDA(cudaMemcpyAsync(t->h_info, t->d_info, sizeof(DevInfo), cudaMemcpyDeviceToHost, t->stream));
+    BH_CUDA(cudaStreamSynchronize(t->stream));
+    if (t->h_info->nonfinite) {  // reported now, not again later
+      t->h_info->nonfinite_sticky = 0;
+      cudaMemsetAsync(&t->d_info->nonfinite_sticky, 0, sizeof(unsigned), t->stream);
+      return set_err(t, TREE_ERR_NONFINITE, "non-finite position or mass");
+    }
+    BH_TRY_RC(check_sticky(t));  // errors of earlier asynchronous passes surface here at the latest
+    const long long nc = t->h_info->level_off[NLEVELS];
+    if (nc <= 0 || nc >= (1ll << 28)) return set_err(t, TREE_ERR_ARG, "cell count out of range (needs < 2^28 cells)");
+    rc = ensure_cells(t, nc);
+    if (rc) return rc;
+    t->n_cells = nc;
+    t->cells_bound = nc;
+    t->async_pending = false;
+  }
   tree_emit_kernel<<<ntiles, TREE_THREADS, 0, t->stream>>>(t->b.lv, t->N, ntiles, t->b.scan_tmp, t->b.c_level,
-                                                           t->b.c_first, t->b.c_count, t->b.c_fcall);
+                                                           t->b.c_first, t->b.c_count, t->b.c_fcall, t->d_info);
   BH_LAUNCH_CHECK("tree_emit");
-  tree_link_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, t->stream>>>(nc, t->b.c_first, t->b.c_count, t->b.c_fcall,
-                                                                        t->b.c_link);
+  tree_link_kernel<<<(unsigned)((t->cells_bound + 255) / 256), 256, 0, t->stream>>>(t->d_info, t->b.c_first, t->b.c_count,
+                                                                                    t->b.c_fcall, t->b.c_link);
   BH_LAUNCH_CHECK("tree_link");
   return 0;
 }
@@ -810,26 +998,21 @@ int run_groups_moments(tree_ctx *t) {
   const long long thr = t->n_groups * 32;
   groups_kernel<<<(unsigned)((thr + 255) / 256), 256, 0, t->stream>>>(t->b.spos, t->N, t->group, t->n_groups, t->b.gbox);
   BH_LAUNCH_CHECK("groups");
-  const int *off = t->h_info->level_off;
-  const int nc = (int)t->n_cells;
-  moments_leaf_kernel<<<(nc + 127) / 128, 128, 0, t->stream>>>(nc, t->d_info, t->b.spos, t->b.c_link, t->b.c_level,
-                                                               t->b.c_first, t->b.c_count, t->b.c_cm, t->b.c_qa, t->b.c_qb);
+  float4 *tlo = t->mac == TREE_MAC_BMAX ? t->b.c_tlo : nullptr, *thi = t->mac == TREE_MAC_BMAX ? t->b.c_thi : nullptr;
+  // all grids below are sized from cells_bound; the kernels read the cell count and the level ranges on the device
+  moments_leaf_kernel<<<grid_for(t, t->cells_bound, 128, 64), 128, 0, t->stream>>>(
+      t->d_info, t->b.spos, t->b.c_link, t->b.c_level, t->b.c_first, t->b.c_count, t->b.c_cm, t->b.c_qa, t->b.c_qb, tlo, thi);
   BH_LAUNCH_CHECK("moments_leaf");
-  int ltop = -1;  // levels 0..ltop together hold at most MOMENTS_TOP_CELLS cells: one block does them
-  while (ltop + 1 <= MAX_LEVEL && off[ltop + 2] <= MOMENTS_TOP_CELLS) ++ltop;
-  for (int l = MAX_LEVEL; l > ltop; --l) {
-    int c0 = off[l], c1 = off[l + 1];
-    if (c1 <= c0) continue;
-    moments_level_kernel<<<(c1 - c0 + 127) / 128, 128, 0, t->stream>>>(c0, c1, l, t->d_info, t->b.spos, t->b.c_link,
-                                                                       t->b.c_first, t->b.c_count, t->b.c_cm, t->b.c_qa,
-                                                                       t->b.c_qb);
+  for (int l = MAX_LEVEL; l >= 1; --l) {  // level 0 (the root) always belongs to the top block
+    long long most = t->cells_bound;      // a level holds at most 8^l cells
+    if (l < 9 && (1ll << (3 * l)) < most) most = 1ll << (3 * l);
+    moments_level_kernel<<<grid_for(t, most, 128, 16), 128, 0, t->stream>>>(l, t->d_info, t->b.spos, t->b.c_link, t->b.c_first,
+                                                                           t->b.c_count, t->b.c_cm, t->b.c_qa, t->b.c_qb, tlo, thi);
     BH_LAUNCH_CHECK("moments_level");
   }
-  if (ltop >= 0) {
-    moments_top_kernel<<<1, 256, 0, t->stream>>>(ltop, t->d_info, t->b.spos, t->b.c_link, t->b.c_first, t->b.c_count,
-                                                 t->b.c_cm, t->b.c_qa, t->b.c_qb);
-    BH_LAUNCH_CHECK("moments_top");
-  }
+  moments_top_kernel<<<1, 256, 0, t->stream>>>(t->d_info, t->b.spos, t->b.c_link, t->b.c_first, t->b.c_count, t->b.c_cm,
+                                               t->b.c_qa, t->b.c_qb, tlo, thi);
+  BH_LAUNCH_CHECK("moments_top");
   return 0;
 }
 

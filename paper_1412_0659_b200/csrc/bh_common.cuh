@@ -36,22 +36,32 @@ struct DevInfo {
   unsigned int g_lo, g_hi;        // groups this context walks in the current force pass (all of them unless sharded)
   double ekin, epot;
   unsigned int moved_groups;      // groups whose box is not where the previous force pass saw it (box_moved_kernel)
+  unsigned int reuse_costs;       // this pass schedules by the previous pass's per-group counts (decided on the device)
+  int n_cells;                    // cells of the current tree (= level_off[NLEVELS])
+  int ltop;                       // levels 0..ltop hold so few cells that one block computes their moments
+  unsigned int nonfinite_sticky;  // sticky: a rebuild saw a non-finite position or mass (asynchronous steps report it late)
+  unsigned int cells_overflow;    // sticky: an asynchronous rebuild needed more cells than allocated; the cell count it
+                                  // needed.  Every later kernel of the step pipeline does nothing while it is set.
 };
 
 struct Buffers {
-  // caller order
-  float4 *posm = nullptr;   // x,y,z,m
-  float4 *vel = nullptr;    // vx,vy,vz,0
-  float4 *acc = nullptr;    // ax,ay,az,phi
-  // sort
+  // caller order: only the staging copy of tree_build's input (x,y,z,m)
+  float4 *posm = nullptr;
+  // sort: key and payload, double-buffered.  Payload = caller index (tree_build) or previous slot (tree_leapfrog)
   uint64_t *key[2] = {nullptr, nullptr};
   uint32_t *idx[2] = {nullptr, nullptr};
   uint32_t *scan_tmp = nullptr;  // tile level counts of the tree build / scheduling scans (scanned in place)
   uint32_t *sort_hist = nullptr;              // [8][256] digit histograms -> global digit offsets, then 8 tile tickets
   unsigned long long *sort_status = nullptr;  // [sort tiles][256] decoupled look-back words of the one-sweep sort
   uint32_t *scan_blk = nullptr;  // block sums for the device-wide scan
-  // slot (sorted) order
-  float4 *spos = nullptr;
+  // slot (sorted) order: the STATE.  It stays in the slot order of the last sort; a leapfrog step gathers it into the
+  // new order (a nearly sequential gather: few particles change their place on the curve in one step), so no array
+  // is kept in caller order and results are scattered to caller order only when the caller asks for them.
+  float4 *spos2[2] = {nullptr, nullptr}, *svel2[2] = {nullptr, nullptr};
+  uint32_t *order2[2] = {nullptr, nullptr};
+  float4 *spos = nullptr;      // = spos2[cur]: x,y,z,m
+  float4 *svel = nullptr;      // = svel2[cur]: vx,vy,vz,0
+  uint32_t *order = nullptr;   // = order2[cur]: order[s] = caller index of the particle in slot s
   void *shard_slab = nullptr;  // one allocation (one IPC handle): sacc2[0] | sacc2[1] | gcount2[0] | gcount2[1]
   float4 *sacc2[2] = {nullptr, nullptr};  // results in slot order, double-buffered by force pass
   float4 *sacc = nullptr;                 // = sacc2[pass & 1], the buffer of the current / last force pass
@@ -78,6 +88,7 @@ struct Buffers {
   float4 *c_qa = nullptr;     // Qxx,Qyy,Qzz,delta
   float4 *c_qb = nullptr;     // Qxy,Qxz,Qyz,tr(Q)
   float4 *c_test = nullptr;   // cx,cy,cz,r_open^2 (per force call)
+  float4 *c_tlo = nullptr, *c_thi = nullptr;  // TREE_MAC_BMAX only: tight box lo x,y,z | b  and  hi x,y,z | -
   // host-call staging
   float *in_pos = nullptr, *in_mass = nullptr, *out_acc = nullptr, *out_pot = nullptr;
 };
@@ -88,8 +99,15 @@ struct tree_ctx {
   int device = 0;
   cudaStream_t stream = nullptr;
   int leaf = 16, group = 64;
+  int mac = TREE_MAC_GEOMETRIC;      // acceptance criterion (tree_set_mac)
   long long N = 0, cap = 0;          // particles, particle capacity
-  long long n_cells = 0, cell_cap = 0;
+  long long n_cells = 0, cell_cap = 0;  // n_cells: exact after tree_build; after an asynchronous rebuild (tree_leapfrog) the
+                                        // latest count read back so far (poll_cells)
+  long long cells_bound = 0;            // cells the kernels of the current tree may use / launch for (<= cell_cap)
+  int cur = 0;                          // which of the state double buffers (spos2, svel2, order2) is current
+  bh::DevInfo *h_async = nullptr;       // pinned: DevInfo copied back after the tree kernels of an asynchronous rebuild
+  cudaEvent_t ev_async = nullptr;
+  bool async_pending = false;
   long long n_groups = 0;
   long long scan_cap = 0;
   long long sort_status_cap = 0;     // words in b.sort_status
@@ -98,9 +116,11 @@ struct tree_ctx {
   bool sort_attr_set = false;        // the sort kernel's shared-memory attributes are set on this context's device
   int sorted = 0;                    // which of key[]/idx[] holds the sorted result
   bool built = false, have_vel = false, have_force = false;
+  bool state_valid = false;          // spos / svel / order hold one consistent particle set (tree_get_state, tree_direct)
   long long staging_cap = 0;         // capacity of the host-call staging buffers
   float theta = 0.f, eps = 0.f;
-  bool reuse_costs = false;          // this force pass may schedule by the previous pass's per-group counts
+  int reuse_mode = 0;                // scheduling of the next force pass: 0 = counting walk, 1 = by the previous pass's
+                                     // per-group counts (tree_leapfrog), 2 = decided on the device by box_moved_kernel
   bool prev_valid = false;           // b.gbox_prev and the other parity's gcount describe a finished pass over prev_N particles
   long long prev_N = 0;
   // sharded force pass: this context walks one contiguous cost-balanced range of groups and
@@ -150,19 +170,20 @@ int check_sticky(tree_ctx *t);
 
 // phases implemented in bh_build.cu / bh_force.cu (host launchers; all enqueue on t->stream)
 int run_pack_bbox(tree_ctx *t, const float *pos, const float *mass);  // caller arrays -> posm + bbox
-int run_bbox_only(tree_ctx *t);                                        // bbox of posm (leapfrog rebuild)
-int run_keys(tree_ctx *t);
+int run_kick_drift_bbox(tree_ctx *t, float dt);                        // leapfrog: kick + drift of the slot-order state + bbox
+int run_keys(tree_ctx *t, const float4 *xyzm);                         // grid + keys of posm (build) or spos (leapfrog)
 int run_sort(tree_ctx *t);
-int run_permute(tree_ctx *t);
-int run_tree(tree_ctx *t);      // octree construction; synchronises once (cell count)
+int run_permute_build(tree_ctx *t);   // tree_build: posm -> spos, order (payload of the sort = caller index)
+int run_permute_step(tree_ctx *t);    // tree_leapfrog: spos, svel, order -> the new slot order (payload = previous slot)
+int run_tree(tree_ctx *t, bool async);  // octree construction; !async: synchronises once and sizes the cell arrays
 int run_groups_moments(tree_ctx *t);
 int run_opening(tree_ctx *t, float theta);
-int run_walk(tree_ctx *t, float eps);
-int run_box_check(tree_ctx *t, bool *same);  // are the group boxes where the previous force pass saw them?
+int run_walk(tree_ctx *t, float eps, float kick_hdt);  // kick_hdt != 0: v += a * kick_hdt in the walk's epilogue
+int run_box_check(tree_ctx *t);  // device-side: are the group boxes where the previous force pass saw them?
 void shard_views(const tree_ctx *t, void *base, int parity, float4 **sacc, uint2 **gcount);
-int run_unpermute(tree_ctx *t, float *acc, float *pot);
-int run_kick_drift(tree_ctx *t, float dt);
+int run_scatter_out(tree_ctx *t, float *acc, float *pot);  // results to the caller's arrays (caller order)
 int run_kick(tree_ctx *t, float dt);
+void poll_cells(tree_ctx *t);  // non-blocking: take over the cell count of the last asynchronous rebuild if it has arrived
 int run_energy(tree_ctx *t);
 int run_set_velocity(tree_ctx *t, const float *vel);
 int run_get_state(tree_ctx *t, float *pos, float *vel, float *acc, float *pot);

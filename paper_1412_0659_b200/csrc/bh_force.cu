@@ -23,15 +23,20 @@ __device__ __forceinline__ unsigned warp_incl_scan_u(unsigned v, int /*lane*/) {
 // a8: opening radius per cell for this theta, packed with the centre of mass into the 16-byte
 // test record (T9): r = l_c / theta; r = r + delta; r_open^2 = r * r, each one IEEE op.
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) opening_kernel(long long n_cells, const DevInfo *__restrict__ info, float theta,
+__global__ void __launch_bounds__(256) opening_kernel(const DevInfo *__restrict__ info, float theta,
                                                       const uint8_t *__restrict__ c_level,
                                                       const float4 *__restrict__ c_cm, const float4 *__restrict__ c_qa,
-                                                      float4 *__restrict__ c_test) {
+                                                      const float4 *__restrict__ c_tlo, float4 *__restrict__ c_test) {
   long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  if (c >= n_cells) return;
-  float lc = ldexpf(1.0f, info->k - (int)c_level[c]);
-  float r = __fdiv_rn(lc, theta);
-  r = __fadd_rn(r, c_qa[c].w);
+  if (info->cells_overflow || c >= info->n_cells) return;
+  float r;
+  if (c_tlo) {  // TREE_MAC_BMAX: r = b / theta (theta = 0 opens everything, also where b = 0)
+    r = theta == 0.0f ? INFINITY : __fdiv_rn(c_tlo[c].w, theta);
+  } else {
+    float lc = ldexpf(1.0f, info->k - (int)c_level[c]);
+    r = __fdiv_rn(lc, theta);
+    r = __fadd_rn(r, c_qa[c].w);
+  }
   float4 cm = c_cm[c];
   c_test[c] = make_float4(cm.x, cm.y, cm.z, __fmul_rn(r, r));
 }
@@ -111,6 +116,9 @@ struct WalkParams {
   long long N;
   unsigned n_groups;
   float eps2;
+  float4 *svel;            // tree_leapfrog on one context: the step's closing half kick, v += a * kick_hdt, is applied here in
+  float kick_hdt;          // the epilogue (nullptr otherwise: a sharded pass kicks after its barrier)
+  int reuse_mode;          // 0: costs from the counting walk; 1: from the previous pass's counts; 2: info->reuse_costs decides
 };
 
 constexpr unsigned TASK_GROUP_BITS = 26;
@@ -243,6 +251,34 @@ __device__ __forceinline__ float rsqrt_fast(float x) {
   return y;
 }
 
+// Measurement switches of round 2 ("Evaluator variants"); both default to the built form.
+//  BH_RSQRT_NR = 1: one Newton-Raphson step on MUFU.RSQ, y' = y + y (0.5 - 0.5 x y^2): 4 more FP32 instructions per pair
+//  BH_SPLIT_AQ = 1: the quadrupole part of the acceleration, rho^5 Q' r, is summed in accumulators of its own within a
+//                   tile and scaled by -0.4 once per tile: one FP32 instruction fewer per p-c interaction
+#ifndef BH_RSQRT_NR
+#define BH_RSQRT_NR 0
+#endif
+#ifndef BH_SPLIT_AQ
+#define BH_SPLIT_AQ 0
+#endif
+__device__ __forceinline__ float rsqrt_eval(float x) {
+  float y = rsqrt_fast(x);
+#if BH_RSQRT_NR
+  const float e = fmaf(x * y * y, -0.5f, 0.5f);
+  y = fmaf(y, e, y);
+#endif
+  return y;
+}
+__device__ __forceinline__ f32x2 rsqrt_eval2(float xa, float xb) {
+  f32x2 y = pk2(rsqrt_fast(xa), rsqrt_fast(xb));
+#if BH_RSQRT_NR
+  const f32x2 x = pk2(xa, xb);
+  const f32x2 e = fma2(mul2(mul2(x, y), y), bc2(-0.5f), bc2(0.5f));
+  y = fma2(y, e, y);
+#endif
+  return y;
+}
+
 template <int TPL, bool MASK>
 __device__ __forceinline__ void pp_one(const float4 s, uint32_t sidx, Targets<TPL> &T, float eps2) {
 #pragma unroll
@@ -255,7 +291,7 @@ __device__ __forceinline__ void pp_one(const float4 s, uint32_t sidx, Targets<TP
     if (MASK) {
       if (sidx == T.slot[t]) { m = 0.0f; r2 = 1.0f; }
     }
-    float ri = rsqrt_fast(r2);
+    float ri = rsqrt_eval(r2);
     float ri2 = ri * ri;
     float mr = m * ri;
     float mr3 = mr * ri2;
@@ -279,7 +315,7 @@ __device__ __forceinline__ void pc_one(const float4 a, const float4 b, const flo
     float r2 = fmaf(dx, dx, eps2);
     r2 = fmaf(dy, dy, r2);
     r2 = fmaf(dz, dz, r2);
-    float ri = rsqrt_fast(r2);
+    float ri = rsqrt_eval(r2);
     float vx = fmaf(c.y, dz, fmaf(c.x, dy, b.x * dx));   // 2.5 Q' r
     float vy = fmaf(c.z, dz, fmaf(b.y, dy, c.x * dx));
     float vz = fmaf(b.z, dz, fmaf(c.z, dy, c.y * dx));
@@ -308,6 +344,9 @@ __device__ __forceinline__ void pc_one(const float4 a, const float4 b, const flo
 // ------------------------------------------------------------------------------------------
 struct Targets2 {  // the packed view of Targets<2> during one tile
   f32x2 x, y, z, ax, ay, az, ph, phq;
+#if BH_SPLIT_AQ
+  f32x2 qx = 0ull, qy = 0ull, qz = 0ull;  // sum of rho^5 (2.5 Q' r) over the tile; -0.4 x is added to a in store()
+#endif
   __device__ __forceinline__ explicit Targets2(const Targets<2> &T)
       :
 #if BH_PACK_HOME
@@ -318,6 +357,10 @@ struct Targets2 {  // the packed view of Targets<2> during one tile
         ax(pk2(T.ax[0], T.ax[1])),
         ay(pk2(T.ay[0], T.ay[1])), az(pk2(T.az[0], T.az[1])), ph(pk2(T.ph[0], T.ph[1])), phq(pk2(T.phq[0], T.phq[1])) {}
   __device__ __forceinline__ void store(Targets<2> &T) const {
+#if BH_SPLIT_AQ
+    const f32x2 m = bc2(-0.4f);
+    const f32x2 ax = fma2(m, qx, this->ax), ay = fma2(m, qy, this->ay), az = fma2(m, qz, this->az);
+#endif
     up2(ax, T.ax[0], T.ax[1]); up2(ay, T.ay[0], T.ay[1]); up2(az, T.az[0], T.az[1]);
     up2(ph, T.ph[0], T.ph[1]); up2(phq, T.phq[0], T.phq[1]);
   }
@@ -335,7 +378,7 @@ __device__ __forceinline__ void pp_one2(const float4 s, uint32_t sidx, const uin
     if (sidx == slot[0]) { m0 = 0.0f; r2a = 1.0f; }
     if (sidx == slot[1]) { m1 = 0.0f; r2b = 1.0f; }
   }
-  const f32x2 ri = pk2(rsqrt_fast(r2a), rsqrt_fast(r2b));
+  const f32x2 ri = rsqrt_eval2(r2a, r2b);
   const f32x2 ri2 = mul2(ri, ri);
   const f32x2 mr = mul2(MASK ? pk2(m0, m1) : bc2(s.w), ri);
   const f32x2 mr3 = mul2(mr, ri2);
@@ -353,7 +396,7 @@ __device__ __forceinline__ void pc_one2(const float4 a, const float4 b, const fl
   r2 = fma2(dz, dz, r2);
   float r2a, r2b;
   up2(r2, r2a, r2b);
-  const f32x2 ri = pk2(rsqrt_fast(r2a), rsqrt_fast(r2b));
+  const f32x2 ri = rsqrt_eval2(r2a, r2b);
   const f32x2 vx = fma2(bc2(c.y), dz, fma2(bc2(c.x), dy, mul2(bc2(b.x), dx)));
   const f32x2 vy = fma2(bc2(c.z), dz, fma2(bc2(b.y), dy, mul2(bc2(c.x), dx)));
   const f32x2 vz = fma2(bc2(b.z), dz, fma2(bc2(c.z), dy, mul2(bc2(c.y), dx)));
@@ -365,10 +408,15 @@ __device__ __forceinline__ void pc_one2(const float4 a, const float4 b, const fl
   T.ph = fma2(bc2(-a.w), ri, T.ph);
   T.phq = fma2(w, ri5, T.phq);
   const f32x2 g = mul2(fma2(w, ri4, bc2(a.w)), ri3);
+#if BH_SPLIT_AQ
+  T.ax = fma2(g, dx, T.ax); T.ay = fma2(g, dy, T.ay); T.az = fma2(g, dz, T.az);
+  T.qx = fma2(ri5, vx, T.qx); T.qy = fma2(ri5, vy, T.qy); T.qz = fma2(ri5, vz, T.qz);
+#else
   const f32x2 k = mul2(bc2(-0.4f), ri5);
   T.ax = fma2(k, vx, fma2(g, dx, T.ax));
   T.ay = fma2(k, vy, fma2(g, dy, T.ay));
   T.az = fma2(k, vz, fma2(g, dz, T.az));
+#endif
 }
 
 template <int TPL>
@@ -511,6 +559,21 @@ __device__ __forceinline__ void flush_queues(WarpSmem &ws, int lane, WalkState<T
     S.pp_pending = 0;
     S.pp_entries = 0;
   }
+}
+
+// a12, second half kick of a step, fused into the walk's epilogue: v = fma(a, dt/2, v) (T12)
+#ifndef BH_KICK_INLINE
+#define BH_KICK_INLINE 1
+#endif
+#if BH_KICK_INLINE
+__device__ __forceinline__
+#else
+__device__ __noinline__
+#endif
+void kick_slot(float4 *v, const float4 a, float hdt) {
+  float4 u = *v;
+  u.x = __fmaf_rn(a.x, hdt, u.x); u.y = __fmaf_rn(a.y, hdt, u.y); u.z = __fmaf_rn(a.z, hdt, u.z);
+  *v = u;
 }
 
 // One work item: group g (part `part` of `nparts`).
@@ -742,6 +805,7 @@ __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, con
       if (j < gsize) {
         P.sacc[g0 + j] = res[t];
         for (int q = 0; q < P.n_peers; ++q) P.peer_sacc[q][g0 + j] = res[t];
+        if (P.svel) kick_slot(P.svel + g0 + j, res[t], P.kick_hdt);
       }
     }
   } else {
@@ -773,6 +837,7 @@ __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, con
                                          __fadd_rn(hi[3], lo[3]));
           P.sacc[g0 + j] = sum;
           for (int q = 0; q < P.n_peers; ++q) P.peer_sacc[q][g0 + j] = sum;
+          if (P.svel) kick_slot(P.svel + g0 + j, sum, P.kick_hdt);
         }
       }
       if (P.n_peers > 0 && lane == 0) {  // every part's counts were added before it signalled gdone
@@ -788,6 +853,8 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, COUNT ? COUNT_MINB : walk_min
   __shared__ WarpSmem smem[WALK_WARPS];
   WarpSmem &ws = smem[threadIdx.x >> 5];
   const int lane = threadIdx.x & 31;
+  if (P.info->cells_overflow) return;  // a failed asynchronous rebuild: there is no tree to walk (tree.h)
+  if (COUNT && (P.reuse_mode == 1 || (P.reuse_mode == 2 && P.info->reuse_costs))) return;  // costs come from the previous pass
   const unsigned n_items = COUNT ? P.n_groups : P.info->n_tasks;
 
   for (;;) {
@@ -866,9 +933,15 @@ __device__ __forceinline__ double prev_cost(const uint2 *__restrict__ gcount, un
 // Cost estimate of every group for this pass (unit: 13 n_pp + 37 n_pc): the counting walk's (left in gdone), or --
 // tree_leapfrog, the same particles one step later -- the exact counts of the previous pass (the neighbours cover a
 // shift of the runs by up to two); in that case their sum is formed here.
+__device__ __forceinline__ bool reuse_decided(int mode, const DevInfo *info) {
+  return mode == 1 || (mode == 2 && info->reuse_costs);
+}
+
 __global__ void __launch_bounds__(256) group_cost_kernel(unsigned n_groups, DevInfo *info, const uint32_t *__restrict__ gdone,
-                                                         const uint2 *__restrict__ prev, double *__restrict__ gcost) {
+                                                         const uint2 *__restrict__ prev_counts, int reuse_mode,
+                                                         double *__restrict__ gcost) {
   const unsigned g = blockIdx.x * blockDim.x + threadIdx.x;
+  const uint2 *prev = reuse_decided(reuse_mode, info) ? prev_counts : nullptr;  // block-uniform
   double own = 0.0;
   if (g < n_groups) {
     double cost;
@@ -1015,9 +1088,10 @@ __device__ __forceinline__ TailPlan tail_plan(const DevInfo *info, const TailLim
 __global__ void __launch_bounds__(256) task_cost_kernel(unsigned n_groups, const DevInfo *__restrict__ info,
                                                         uint32_t *__restrict__ a_cnt, uint32_t *__restrict__ gdone,
                                                         uint32_t *__restrict__ gthresh, const double *__restrict__ gcost,
-                                                        const float *__restrict__ suspect_gbox, const TailLimits lim) {
+                                                        const float *__restrict__ gbox, int reuse_mode, const TailLimits lim) {
   unsigned g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= n_groups) return;
+  const float *suspect_gbox = reuse_decided(reuse_mode, info) ? gbox : nullptr;
   const unsigned tail_parts = tail_plan(info, lim).parts;
   const double mean = (double)info->sched_cost / (double)n_groups;  // over ALL groups, also in a sharded pass
   const double cost = gcost[g];
@@ -1124,57 +1198,45 @@ __global__ void __launch_bounds__(256) task_fill_kernel(unsigned n_groups, const
   }
 }
 
-// a11: results back to caller order
-__global__ void __launch_bounds__(256) unpermute_kernel(const float4 *__restrict__ sacc, const uint32_t *__restrict__ order,
-                                                        long long N, float4 *__restrict__ acc4, float *__restrict__ acc,
-                                                        float *__restrict__ pot) {
+// a11: results to the caller's arrays (caller order), only when the caller gave any; the library itself keeps its
+// state and results in slot order
+__global__ void __launch_bounds__(256) scatter_out_kernel(const float4 *__restrict__ sacc, const uint32_t *__restrict__ order,
+                                                          long long N, float *__restrict__ acc, float *__restrict__ pot) {
   long long s = blockIdx.x * (long long)blockDim.x + threadIdx.x;
   if (s >= N) return;
   const float4 a = sacc[s];
   const long long i = order[s];
-  acc4[i] = a;
   if (acc) { acc[3 * i] = a.x; acc[3 * i + 1] = a.y; acc[3 * i + 2] = a.z; }
   if (pot) pot[i] = a.w;
 }
 
-// a12: leapfrog (T12): v = fma(a, dt/2, v); x = fma(v, dt, x)
-__global__ void __launch_bounds__(256) kick_drift_kernel(float4 *__restrict__ posm, float4 *__restrict__ vel,
-                                                         const float4 *__restrict__ acc, long long N, float hdt, float dt) {
+// a12: the closing half kick of a step as its own pass (sharded passes: after the barrier; otherwise it is fused into the
+// walk's epilogue, kick_slot): v = fma(a, dt/2, v), slot order, sequential
+__global__ void __launch_bounds__(256) kick_kernel(float4 *__restrict__ svel, const float4 *__restrict__ sacc, long long N,
+                                                   float hdt, const DevInfo *__restrict__ info) {
   long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  if (i >= N) return;
-  float4 p = posm[i], v = vel[i];
-  const float4 a = acc[i];
+  if (i >= N || info->cells_overflow) return;
+  float4 v = svel[i];
+  const float4 a = sacc[i];
   v.x = __fmaf_rn(a.x, hdt, v.x); v.y = __fmaf_rn(a.y, hdt, v.y); v.z = __fmaf_rn(a.z, hdt, v.z);
-  p.x = __fmaf_rn(v.x, dt, p.x); p.y = __fmaf_rn(v.y, dt, p.y); p.z = __fmaf_rn(v.z, dt, p.z);
-  vel[i] = v;
-  posm[i] = p;
-}
-
-__global__ void __launch_bounds__(256) kick_kernel(float4 *__restrict__ vel, const float4 *__restrict__ acc, long long N,
-                                                   float hdt) {
-  long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  if (i >= N) return;
-  float4 v = vel[i];
-  const float4 a = acc[i];
-  v.x = __fmaf_rn(a.x, hdt, v.x); v.y = __fmaf_rn(a.y, hdt, v.y); v.z = __fmaf_rn(a.z, hdt, v.z);
-  vel[i] = v;
+  svel[i] = v;
 }
 
 __global__ void energy_reset_kernel(DevInfo *info) {
   if (threadIdx.x == 0) { info->ekin = 0.0; info->epot = 0.0; }
 }
 
-__global__ void __launch_bounds__(256) energy_kernel(const float4 *__restrict__ posm, const float4 *__restrict__ vel,
-                                                     const float4 *__restrict__ acc, long long N, bool have_vel,
+__global__ void __launch_bounds__(256) energy_kernel(const float4 *__restrict__ spos, const float4 *__restrict__ svel,
+                                                     const float4 *__restrict__ sacc, long long N, bool have_vel,
                                                      DevInfo *info) {
   double ke = 0.0, pe = 0.0;
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
-    const double m = (double)posm[i].w;
+    const double m = (double)spos[i].w;
     if (have_vel) {
-      const float4 v = vel[i];
+      const float4 v = svel[i];
       ke += 0.5 * m * ((double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z);
     }
-    pe += 0.5 * m * (double)acc[i].w;
+    pe += 0.5 * m * (double)sacc[i].w;
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
@@ -1192,24 +1254,37 @@ __global__ void __launch_bounds__(256) energy_kernel(const float4 *__restrict__ 
   }
 }
 
-__global__ void __launch_bounds__(256) set_vel_kernel(const float *__restrict__ v3, float4 *__restrict__ vel, long long N) {
-  long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  if (i < N) vel[i] = make_float4(v3[3 * i], v3[3 * i + 1], v3[3 * i + 2], 0.0f);
+// the caller's velocities (caller order) into the slot-order state
+__global__ void __launch_bounds__(256) set_vel_kernel(const float *__restrict__ v3, const uint32_t *__restrict__ order,
+                                                      float4 *__restrict__ svel, long long N) {
+  long long s = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (s >= N) return;
+  const long long i = order[s];
+  svel[s] = make_float4(v3[3 * i], v3[3 * i + 1], v3[3 * i + 2], 0.0f);
 }
 
-__global__ void __launch_bounds__(256) get_state_kernel(const float4 *__restrict__ posm, const float4 *__restrict__ vel,
-                                                        const float4 *__restrict__ acc4, long long N,
-                                                        float *__restrict__ pos, float *__restrict__ v3,
+// the slot-order state and results to the caller's arrays (caller order)
+__global__ void __launch_bounds__(256) get_state_kernel(const float4 *__restrict__ spos, const float4 *__restrict__ svel,
+                                                        const float4 *__restrict__ sacc, const uint32_t *__restrict__ order,
+                                                        long long N, float *__restrict__ pos, float *__restrict__ v3,
                                                         float *__restrict__ acc, float *__restrict__ pot) {
-  long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  if (i >= N) return;
-  if (pos) { float4 p = posm[i]; pos[3 * i] = p.x; pos[3 * i + 1] = p.y; pos[3 * i + 2] = p.z; }
-  if (v3) { float4 v = vel[i]; v3[3 * i] = v.x; v3[3 * i + 1] = v.y; v3[3 * i + 2] = v.z; }
+  long long s = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (s >= N) return;
+  const long long i = order[s];
+  if (pos) { float4 p = spos[s]; pos[3 * i] = p.x; pos[3 * i + 1] = p.y; pos[3 * i + 2] = p.z; }
+  if (v3) { float4 v = svel[s]; v3[3 * i] = v.x; v3[3 * i + 1] = v.y; v3[3 * i + 2] = v.z; }
   if (acc || pot) {
-    float4 a = acc4[i];
+    float4 a = sacc[s];
     if (acc) { acc[3 * i] = a.x; acc[3 * i + 1] = a.y; acc[3 * i + 2] = a.z; }
     if (pot) pot[i] = a.w;
   }
+}
+
+// slot of every caller index (tree_direct looks its targets up by caller index)
+__global__ void __launch_bounds__(256) inverse_order_kernel(const uint32_t *__restrict__ order, long long N,
+                                                            uint32_t *__restrict__ slot_of) {
+  long long s = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (s < N) slot_of[order[s]] = (uint32_t)s;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -1220,12 +1295,13 @@ __global__ void __launch_bounds__(256) get_state_kernel(const float4 *__restrict
 constexpr int DIRECT_THREADS = 128;
 
 __global__ void __launch_bounds__(DIRECT_THREADS) direct_kernel(const float4 *__restrict__ posm, long long N,
-                                                                const long long *__restrict__ idx, long long n,
+                                                                const long long *__restrict__ idx,
+                                                                const uint32_t *__restrict__ slot_of, long long n,
                                                                 double eps2, double *__restrict__ acc,
                                                                 double *__restrict__ pot) {
   __shared__ float4 tile[DIRECT_THREADS];
   const long long k = blockIdx.x * (long long)DIRECT_THREADS + threadIdx.x;
-  const long long i = k < n ? idx[k] : -1;
+  const long long i = k < n ? (long long)slot_of[idx[k]] : -1;  // the sources are summed in slot order
   const float4 pi = i >= 0 ? posm[i] : make_float4(0.f, 0.f, 0.f, 0.f);
   const double xi = pi.x, yi = pi.y, zi = pi.z;
   const long long chunk = (N + gridDim.y - 1) / gridDim.y;
@@ -1309,8 +1385,8 @@ int run_fp32_peak(tree_ctx *t, double *tflops) {
 static inline unsigned blocks_for(long long n, int threads) { return (unsigned)((n + threads - 1) / threads); }
 
 int run_opening(tree_ctx *t, float theta) {
-  opening_kernel<<<blocks_for(t->n_cells, 256), 256, 0, t->stream>>>(t->n_cells, t->d_info, theta, t->b.c_level,
-                                                                     t->b.c_cm, t->b.c_qa, t->b.c_test);
+  opening_kernel<<<blocks_for(t->cells_bound, 256), 256, 0, t->stream>>>(
+      t->d_info, theta, t->b.c_level, t->b.c_cm, t->b.c_qa, t->mac == TREE_MAC_BMAX ? t->b.c_tlo : nullptr, t->b.c_test);
   BH_LAUNCH_CHECK("opening");
   return 0;
 }
@@ -1343,16 +1419,21 @@ __global__ void __launch_bounds__(256) box_moved_kernel(unsigned n_groups, unsig
   if ((threadIdx.x & 31) == 0 && m) atomicAdd(&info->moved_groups, (unsigned)__popc(m));
 }
 
-int run_box_check(tree_ctx *t, bool *same) {
+__global__ void box_decide_kernel(unsigned n_samples, DevInfo *info) {
+  // measured: 0-2 % of the sampled runs moved for a drifted set, 99.7 % for an unrelated one
+  if (threadIdx.x == 0) info->reuse_costs = (unsigned long long)info->moved_groups * 8ull <= n_samples ? 1u : 0u;
+}
+
+// Decides on the device (info->reuse_costs) whether this pass schedules by the previous pass's counts: no read-back.
+int run_box_check(tree_ctx *t) {
   const unsigned ng = (unsigned)t->n_groups;
   const unsigned stride = (ng + 65535u) / 65536u, ns = (ng + stride - 1u) / stride;
   const unsigned window = std::max(8u, (unsigned)(std::sqrt((double)t->N) / 128.0));
   BH_CUDA(cudaMemsetAsync(&t->d_info->moved_groups, 0, sizeof(unsigned), t->stream));
   box_moved_kernel<<<(ns + 255) / 256, 256, 0, t->stream>>>(ng, ns, stride, window, t->b.gbox, t->b.gbox_prev, t->d_info);
   BH_LAUNCH_CHECK("box_moved");
-  BH_CUDA(cudaMemcpyAsync(&t->h_info->moved_groups, &t->d_info->moved_groups, sizeof(unsigned), cudaMemcpyDeviceToHost, t->stream));
-  BH_CUDA(cudaStreamSynchronize(t->stream));
-  *same = (unsigned long long)t->h_info->moved_groups * 8ull <= ns;  // measured: 0-2 % for a drifted set, 99.7 % for an unrelated one
+  box_decide_kernel<<<1, 32, 0, t->stream>>>(ns, t->d_info);
+  BH_LAUNCH_CHECK("box_decide");
   return 0;
 }
 
@@ -1362,14 +1443,13 @@ static int launch_walk(tree_ctx *t, const WalkParams &P, unsigned grid) {
   DevInfo *info = t->d_info;
   uint32_t *tot = info->sched_tot;
   // 1. cost of every group: the walk without the evaluation, or the previous pass's exact counts
-  const bool reuse = t->reuse_costs;
-  if (!reuse) {
+  const int mode = P.reuse_mode;
+  if (mode != 1) {  // mode 2: the kernel returns at once if the device decided to reuse the previous counts
     const long long cwant = (ng + WALK_WARPS - 1) / WALK_WARPS, ccap = (long long)t->sm_count * COUNT_MINB;
     walk_force_kernel<TPL, true><<<(unsigned)(cwant < ccap ? cwant : ccap), WALK_WARPS * 32, 0, t->stream>>>(P);
     BH_LAUNCH_CHECK("walk_count");
   }
-  group_cost_kernel<<<gb, 256, 0, t->stream>>>(ng, info, t->b.gdone, reuse ? t->b.gcount2[(t->pass + 1) & 1] : nullptr,
-                                               t->b.gcost);
+  group_cost_kernel<<<gb, 256, 0, t->stream>>>(ng, info, t->b.gdone, t->b.gcount2[(t->pass + 1) & 1], mode, t->b.gcost);
   BH_LAUNCH_CHECK("group_cost");
   if (t->shard_world > 1) {
     const unsigned nb = (ng + PART_BLOCK - 1) / PART_BLOCK;  // <= 2^16: sched_b (one word per group) has room
@@ -1384,7 +1464,7 @@ static int launch_walk(tree_ctx *t, const WalkParams &P, unsigned grid) {
   TailLimits lim;
   lim.n_tail_max = (unsigned)std::min<long long>(TAIL_PER_SM * t->sm_count, t->tail_cap / (long long)TAIL_PARTS);
   task_cost_kernel<<<gb, 256, 0, t->stream>>>(ng, info, t->b.sched_a, t->b.gdone, t->b.gthresh, t->b.gcost,
-                                              reuse ? t->b.gbox : nullptr, lim);
+                                              t->b.gbox, mode, lim);
   BH_LAUNCH_CHECK("task_cost");
   int rc = device_excl_scan(t, t->b.sched_a, ng, tot);
   if (rc) return rc;
@@ -1403,8 +1483,15 @@ static int launch_walk(tree_ctx *t, const WalkParams &P, unsigned grid) {
   return 0;
 }
 
-int run_walk(tree_ctx *t, float eps) {
+int run_walk(tree_ctx *t, float eps, float kick_hdt) {
   WalkParams P;
+  P.reuse_mode = t->reuse_mode;
+#ifndef BH_FUSE_KICK
+#define BH_FUSE_KICK 1
+#endif
+  const bool fuse_kick = BH_FUSE_KICK && kick_hdt != 0.0f && t->shard_world <= 1;
+  P.svel = fuse_kick ? t->b.svel : nullptr;
+  P.kick_hdt = kick_hdt;
   P.spos = t->b.spos; P.c_test = t->b.c_test; P.c_link = t->b.c_link;
   P.c_cm = t->b.c_cm; P.c_qa = t->b.c_qa; P.c_qb = t->b.c_qb;
   P.gbox = t->b.gbox; P.sacc = t->b.sacc; P.gcount = t->b.gcount; P.info = t->d_info;
@@ -1436,20 +1523,15 @@ int run_walk(tree_ctx *t, float eps) {
   return 0;
 }
 
-int run_unpermute(tree_ctx *t, float *acc, float *pot) {
-  unpermute_kernel<<<blocks_for(t->N, 256), 256, 0, t->stream>>>(t->b.sacc, t->b.idx[t->sorted], t->N, t->b.acc, acc, pot);
-  BH_LAUNCH_CHECK("unpermute");
-  return 0;
-}
-
-int run_kick_drift(tree_ctx *t, float dt) {
-  kick_drift_kernel<<<blocks_for(t->N, 256), 256, 0, t->stream>>>(t->b.posm, t->b.vel, t->b.acc, t->N, 0.5f * dt, dt);
-  BH_LAUNCH_CHECK("kick_drift");
+int run_scatter_out(tree_ctx *t, float *acc, float *pot) {
+  if (!acc && !pot) return 0;
+  scatter_out_kernel<<<blocks_for(t->N, 256), 256, 0, t->stream>>>(t->b.sacc, t->b.order, t->N, acc, pot);
+  BH_LAUNCH_CHECK("scatter_out");
   return 0;
 }
 
 int run_kick(tree_ctx *t, float dt) {
-  kick_kernel<<<blocks_for(t->N, 256), 256, 0, t->stream>>>(t->b.vel, t->b.acc, t->N, 0.5f * dt);
+  kick_kernel<<<blocks_for(t->N, 256), 256, 0, t->stream>>>(t->b.svel, t->b.sacc, t->N, 0.5f * dt, t->d_info);
   BH_LAUNCH_CHECK("kick");
   return 0;
 }
@@ -1458,14 +1540,14 @@ int run_energy(tree_ctx *t) {
   energy_reset_kernel<<<1, 32, 0, t->stream>>>(t->d_info);
   BH_LAUNCH_CHECK("energy_reset");
   long long want = (t->N + 255) / 256, cap = (long long)t->sm_count * 8;
-  energy_kernel<<<(unsigned)(want < cap ? want : cap), 256, 0, t->stream>>>(t->b.posm, t->b.vel, t->b.acc, t->N,
+  energy_kernel<<<(unsigned)(want < cap ? want : cap), 256, 0, t->stream>>>(t->b.spos, t->b.svel, t->b.sacc, t->N,
                                                                           t->have_vel, t->d_info);
   BH_LAUNCH_CHECK("energy");
   return 0;
 }
 
 int run_set_velocity(tree_ctx *t, const float *vel) {
-  set_vel_kernel<<<blocks_for(t->N, 256), 256, 0, t->stream>>>(vel, t->b.vel, t->N);
+  set_vel_kernel<<<blocks_for(t->N, 256), 256, 0, t->stream>>>(vel, t->b.order, t->b.svel, t->N);
   BH_LAUNCH_CHECK("set_velocity");
   return 0;
 }
@@ -1474,20 +1556,25 @@ int run_direct(tree_ctx *t, const long long *idx, long long n, float eps, double
   cudaError_t e = cudaMemsetAsync(acc, 0, (size_t)n * 3 * sizeof(double), t->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(pot, 0, (size_t)n * sizeof(double), t->stream);
   if (e != cudaSuccess) return set_err(t, TREE_ERR_CUDA, "tree_direct: memset", e);
+  // scratch: the key buffer that does not hold the sorted keys is free between two builds
+  uint32_t *slot_of = reinterpret_cast<uint32_t *>(t->b.key[t->sorted ^ 1]);
+  inverse_order_kernel<<<blocks_for(t->N, 256), 256, 0, t->stream>>>(t->b.order, t->N, slot_of);
+  BH_LAUNCH_CHECK("inverse_order");
   const unsigned gx = blocks_for(n, DIRECT_THREADS);
   long long gy = ((long long)t->sm_count * 16 + gx - 1) / gx;  // about 16 blocks per SM in total
   const long long gy_max = (t->N + 4 * DIRECT_THREADS - 1) / (4 * DIRECT_THREADS);
   if (gy > gy_max) gy = gy_max;
   if (gy < 1) gy = 1;
   if (gy > 65535) gy = 65535;
-  direct_kernel<<<dim3(gx, (unsigned)gy), DIRECT_THREADS, 0, t->stream>>>(t->b.posm, t->N, idx, n,
+  direct_kernel<<<dim3(gx, (unsigned)gy), DIRECT_THREADS, 0, t->stream>>>(t->b.spos, t->N, idx, slot_of, n,
                                                                           (double)eps * (double)eps, acc, pot);
   BH_LAUNCH_CHECK("direct");
   return 0;
 }
 
 int run_get_state(tree_ctx *t, float *pos, float *vel, float *acc, float *pot) {
-  get_state_kernel<<<blocks_for(t->N, 256), 256, 0, t->stream>>>(t->b.posm, t->b.vel, t->b.acc, t->N, pos, vel, acc, pot);
+  get_state_kernel<<<blocks_for(t->N, 256), 256, 0, t->stream>>>(t->b.spos, t->b.svel, t->b.sacc, t->b.order, t->N, pos, vel,
+                                                                 acc, pot);
   BH_LAUNCH_CHECK("get_state");
   return 0;
 }
