@@ -49,8 +49,8 @@ FP32_LANES_PER_SM = 128
 SM_MHZ = 1965.0
 # What the evaluators execute per interaction (bh_force.cu pp_one / pc_one): FP32 instructions and flops
 # (an FMA = 2, add / mul / rsqrt = 1).  The paper's CONVENTION is 23 / 65.
-INSTR_PP, INSTR_PC = 13, 33
-XFLOP_PP, XFLOP_PC = 20, 55
+INSTR_PP, INSTR_PC = 13, 32
+XFLOP_PP, XFLOP_PC = 20, 54
 
 
 def _peak_tflops(sm_count: int, sm_mhz: float = SM_MHZ) -> float:

@@ -59,6 +59,7 @@ def lib():
         L.orc_tree_force.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.c_void_p, C.c_int64, C.c_int64]
         L.orc_tree_get_counts.argtypes = [C.c_void_p] * 3
         L.orc_tree_get_ropen2.argtypes = [C.c_void_p] * 2
+        L.orc_tree_abs_sum.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.c_int64, C.c_void_p]
         L.orc_tree_set_mac.argtypes = [C.c_void_p, C.c_int]
         L.orc_tree_get_tight.argtypes = [C.c_void_p] * 2
         L.orc_tree_walk_lists.argtypes = [C.c_void_p, C.c_float, C.c_int64, C.c_void_p, C.POINTER(C.c_int64),
@@ -195,6 +196,18 @@ class Tree:
         npp = np.zeros(self.n_groups, np.uint32); npc = np.zeros(self.n_groups, np.uint32)
         lib().orc_tree_get_counts(self._h, _p(npp), _p(npc))
         return acc, pot, npp, npc
+
+    def abs_sum(self, theta: float, eps: float, particles):
+        """A_i = sum over particle i's interaction list of the magnitudes |a_ij| of its terms (diagnostic: A_i / |a_i| is
+        the cancellation factor of the force sum).  ``particles``: caller indices.  Returns float64 [len(particles)]."""
+        idx = np.asarray(particles, dtype=np.int64)
+        inv = np.empty(self.n, np.int64)
+        inv[self.keys()[1].astype(np.int64)] = np.arange(self.n, dtype=np.int64)
+        slots = np.ascontiguousarray(inv[idx])
+        out = np.zeros(len(slots), np.float64)
+        if lib().orc_tree_abs_sum(self._h, float(theta), float(eps), _p(slots), len(slots), _p(out)):
+            raise ValueError("orc_tree_abs_sum failed")
+        return out
 
     def set_mac(self, kind: int):
         """Acceptance criterion of later force / walk_lists calls: 0 = canonical (S5), 1 = "bmax" (option, NEXT-2)."""

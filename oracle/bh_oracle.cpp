@@ -553,6 +553,40 @@ void orc_tree_get_ropen2(void *h, float *out) {
   Tree *t = (Tree *)h;
   std::memcpy(out, t->ropen2.data(), t->ropen2.size() * sizeof(float));
 }
+// Diagnostic for the tolerance statement of the force parity: for the particles in the given sorted
+// SLOTS, A_i = sum over the interaction list of the MAGNITUDES |a_ij| of the terms whose vector sum is a_i (each term
+// evaluated by eval_pp / eval_pc alone).  A_i / |a_i| is the cancellation factor of the sum.  Adds nothing to T1-T12.
+int orc_tree_abs_sum(void *h, float theta, float eps, const int64_t *slots, int64_t n, double *out) {
+  Tree *t = (Tree *)h;
+  if (!t || !slots || !out || !(theta >= 0.0f) || !(eps >= 0.0f)) return -1;
+  set_opening(*t, theta);
+  const double eps2 = (double)eps * (double)eps;
+  for (int64_t k = 0; k < n; ++k) {
+    const int64_t s = slots[k];
+    if (s < 0 || s >= t->N) return -1;
+    std::vector<int32_t> ac, ol;
+    walk_group(*t, s / t->group_size, ac, ol);
+    const double tx = t->sx[s], ty = t->sy[s], tz = t->sz[s];
+    double A = 0.0;
+    for (int32_t c : ol) {
+      const Cell &cl = t->cells[c];
+      for (uint32_t p = cl.first; p < cl.first + cl.count; ++p) {
+        if ((int64_t)p == s) continue;
+        double a[3] = {0, 0, 0}, phi = 0;
+        eval_pp(tx, ty, tz, t->sx[p], t->sy[p], t->sz[p], t->sm[p], eps2, a, phi);
+        A += std::sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]);
+      }
+    }
+    for (int32_t c : ac) {
+      double a[3] = {0, 0, 0}, phi = 0;
+      eval_pc(*t, c, tx, ty, tz, eps2, a, phi);
+      A += std::sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]);
+    }
+    out[k] = A;
+  }
+  return 0;
+}
+
 // Interaction lists of one group for the last theta set by orc_tree_force / this call (T10).
 // Returns counts through n_acc / n_open; arrays must hold n_cells entries each.
 int orc_tree_walk_lists(void *h, float theta, int64_t g, int32_t *acc_cells, int64_t *n_acc,

@@ -290,10 +290,7 @@ static int leapfrog_begin_impl(tree_ctx *t, float dt) {
 static int leapfrog_end_impl(tree_ctx *t) {
   BH_TRY(force_end_impl(t, nullptr, nullptr));
   rec(t, EV_I2);
-#ifndef BH_FUSE_KICK
-#define BH_FUSE_KICK 1
-#endif
-  if (t->shard_world > 1 || !BH_FUSE_KICK) BH_TRY(run_kick(t, t->step_dt));  // else: done in the walk's epilogue
+  if (t->shard_world > 1) BH_TRY(run_kick(t, t->step_dt));  // one context: done in the walk's epilogue
   rec(t, EV_I3);
   t->step_open = false;
   return 0;

@@ -294,15 +294,9 @@ constexpr int OS_THREADS = 256;
 constexpr int OS_IPT = 8;
 constexpr int OS_TILE = OS_THREADS * OS_IPT;  // 2048
 constexpr int OS_WARPS = OS_THREADS / 32;
-#ifndef BH_OS_MINB
-#define BH_OS_MINB 5
-#endif
-constexpr int OS_MINB = BH_OS_MINB;  // resident blocks per SM (shared memory allows 6)
+constexpr int OS_MINB = 5;  // resident blocks per SM (shared memory allows 6)
 constexpr unsigned long long OS_LOCAL = 1ull << 62, OS_INCL = 2ull << 62;
-#ifndef BH_OS_LOOK
-#define BH_OS_LOOK 4
-#endif
-constexpr int OS_LOOK = BH_OS_LOOK;  // status words one thread keeps in flight during the look-back
+constexpr int OS_LOOK = 4;  // status words one thread keeps in flight during the look-back
 
 __global__ void __launch_bounds__(256) sort_hist8_kernel(const uint64_t *__restrict__ key, long long N,
                                                          uint32_t *__restrict__ ghist /*[8][256]*/) {
@@ -553,10 +547,7 @@ __global__ void __launch_bounds__(TREE_THREADS) tree_levels_kernel(const uint64_
 }
 
 // levels 0..ltop together hold at most this many cells: one block computes their moments (moments_top_kernel)
-#ifndef BH_MOMENTS_TOP_CELLS
-#define BH_MOMENTS_TOP_CELLS 128
-#endif
-constexpr int MOMENTS_TOP_CELLS = BH_MOMENTS_TOP_CELLS;
+constexpr int MOMENTS_TOP_CELLS = 128;
 
 // Level offsets, cell count, the top levels one block handles, and the capacity check of an asynchronous rebuild:
 // `cells_bound` cells are allocated / launched for; a tree that needs more sets the sticky cells_overflow and every

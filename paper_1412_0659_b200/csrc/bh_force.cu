@@ -53,35 +53,14 @@ __global__ void __launch_bounds__(256) opening_kernel(const DevInfo *__restrict_
 // Evaluate: whenever a queue holds >= 32 sources, 32 of them are staged in shared memory as float4
 // and every lane evaluates them against its TPL targets with broadcast LDS.128 loads.
 // ------------------------------------------------------------------------------------------
-#ifndef BH_WALK_MINB
-#define BH_WALK_MINB 5
-#endif
-#ifndef BH_PP_UNROLL
-#define BH_PP_UNROLL 16
-#endif
-#ifndef BH_PC_UNROLL
-#define BH_PC_UNROLL 16
-#endif
-constexpr int PP_UNROLL = BH_PP_UNROLL, PC_UNROLL = BH_PC_UNROLL;  // sources per unrolled evaluator loop body
-#ifndef BH_WALK_WARPS
-#define BH_WALK_WARPS 4
-#endif
-constexpr int WALK_WARPS = BH_WALK_WARPS;  // warps per block of the walk kernels
-constexpr int WALK_MINB = BH_WALK_MINB;  // resident blocks per SM the register budget is sized for
-#ifndef BH_WALK_MINB4
-#define BH_WALK_MINB4 3
-#endif
+constexpr int PP_UNROLL = 16, PC_UNROLL = 16;  // sources per unrolled evaluator loop body
+constexpr int WALK_WARPS = 4;  // warps per block of the walk kernels
+constexpr int WALK_MINB = 5;  // resident blocks per SM the register budget is sized for
 // four targets per lane (group 128) keep twice the per-target state in registers: fewer, fatter blocks
-constexpr int walk_minb(int tpl) { return tpl >= 4 ? BH_WALK_MINB4 : WALK_MINB; }
+constexpr int walk_minb(int tpl) { return tpl >= 4 ? 3 : WALK_MINB; }
 constexpr int COUNT_MINB = 8;            // same for the counting pre-pass (38 registers; shared memory allows 8 blocks)
-#ifndef BH_COUNT_TRUNC
-#define BH_COUNT_TRUNC 1024
-#endif
-constexpr unsigned COUNT_TRUNC = BH_COUNT_TRUNC;  // the counting walk treats cells this small as opened leaves
-#ifndef BH_FOLD_EVERY
-#define BH_FOLD_EVERY 2
-#endif
-constexpr int FOLD_EVERY = BH_FOLD_EVERY;  // tiles (of 32 sources) summed in plain FP32 between compensated folds
+constexpr unsigned COUNT_TRUNC = 1024;  // the counting walk treats cells this small as opened leaves
+constexpr int FOLD_EVERY = 2;  // tiles (of 32 sources) summed in plain FP32 between compensated folds
 constexpr int DEFER_CAP = 256;   // deferred child ranges one part of a split group may own
 constexpr int STACK_CAP = 1024;  // >= 32 per level (depth-first: 32 x 22) + DEFER_CAP
 
@@ -136,24 +115,12 @@ struct Targets {
   unsigned long long xp, yp, zp;             // two targets per lane, packed evaluators: x, y, z as FP32x2 register pairs
 };
 
-// Running totals (S14).  The per-lane FP32 sums over the last FOLD_EVERY tiles are folded into
-// totals that do not drift with the list length: FP64 accumulators (one conversion + one DADD per value; the
-// FP64 pipe of sm_100a is otherwise idle here), or with BH_FOLD_F64 = 0 unevaluated FP32 (hi, lo) pairs
-// updated by an error-free two-sum (7 FADD per value).
-#ifndef BH_FOLD_F64
-#define BH_FOLD_F64 0
-#endif
-#ifndef BH_FOLD_PLAIN_POT
-#define BH_FOLD_PLAIN_POT 1
-#endif
-// FP32x2 register pairs (see "Packed evaluators" below)
+// Running totals (S14).  The per-lane FP32 sums over the last FOLD_EVERY tiles are folded into totals that
+// do not drift with the list length: unevaluated FP32 (hi, lo) pairs updated by an error-free two-sum (7 FADD per value).
+// BH_PACKED = 0 builds the scalar evaluators for group size 64 too (tests/test_gpu_variants.py compares the two forms
+// byte for byte); FP32x2 register pairs: see "Packed evaluators" below.
 #ifndef BH_PACKED
 #define BH_PACKED 1
-#endif
-// 1: the target positions live in aligned register pairs for the whole task (packed once when they are loaded);
-// 0: they live in scalar registers and every tile packs them (ptxas then re-packs them at every use: 6-7 MOV per source)
-#ifndef BH_PACK_HOME
-#define BH_PACK_HOME 1
 #endif
 typedef unsigned long long f32x2;  // (lo = target 0, hi = target 1)
 __device__ __forceinline__ f32x2 pk2(float lo, float hi) { f32x2 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
@@ -173,21 +140,6 @@ __device__ __forceinline__ void two_sum_fold(float &hi, float &lo, float x) {
   lo = __fadd_rn(lo, e);
 }
 
-#if BH_FOLD_F64
-template <int TPL>
-struct Totals {
-  double s[4][TPL];
-  __device__ __forceinline__ void clear() {
-#pragma unroll
-    for (int t = 0; t < TPL; ++t)
-#pragma unroll
-      for (int c = 0; c < 4; ++c) s[c][t] = 0.0;
-  }
-  __device__ __forceinline__ void add(int c, int t, float x) { s[c][t] += (double)x; }
-  __device__ __forceinline__ void add_same_sign(int t, float x) { s[3][t] += (double)x; }
-  __device__ __forceinline__ float get(int c, int t) const { return (float)s[c][t]; }
-};
-#else
 template <int TPL>
 struct Totals {
   float hi[4][TPL], lo[4][TPL];
@@ -200,18 +152,13 @@ struct Totals {
   __device__ __forceinline__ void add(int c, int t, float x) { two_sum_fold(hi[c][t], lo[c][t], x); }
   // the potential is a sum of terms of one sign (the quadrupole part is a small correction): no cancellation, so a
   // plain FP32 total over the folds (one rounding per fold, random sign) stays below 1e-6 relative
-#if BH_FOLD_PLAIN_POT
   __device__ __forceinline__ void add_same_sign(int t, float x) { hi[3][t] = __fadd_rn(hi[3][t], x); }
-#else
-  __device__ __forceinline__ void add_same_sign(int t, float x) { two_sum_fold(hi[3][t], lo[3][t], x); }
-#endif
   __device__ __forceinline__ float get(int c, int t) const { return __fadd_rn(hi[c][t], lo[c][t]); }
 };
-#endif
 
 template <int TPL>
 __device__ __forceinline__ void fold_tile(Targets<TPL> &T, Totals<TPL> &R) {
-#if BH_PACKED && !BH_FOLD_F64
+#if BH_PACKED
   if constexpr (TPL == 2) {  // the same two-sums on register pairs: both targets per instruction
     float *const comp[3] = {T.ax, T.ay, T.az};
 #pragma unroll
@@ -251,34 +198,6 @@ __device__ __forceinline__ float rsqrt_fast(float x) {
   return y;
 }
 
-// Measurement switches of round 2 ("Evaluator variants"); both default to the built form.
-//  BH_RSQRT_NR = 1: one Newton-Raphson step on MUFU.RSQ, y' = y + y (0.5 - 0.5 x y^2): 4 more FP32 instructions per pair
-//  BH_SPLIT_AQ = 1: the quadrupole part of the acceleration, rho^5 Q' r, is summed in accumulators of its own within a
-//                   tile and scaled by -0.4 once per tile: one FP32 instruction fewer per p-c interaction
-#ifndef BH_RSQRT_NR
-#define BH_RSQRT_NR 0
-#endif
-#ifndef BH_SPLIT_AQ
-#define BH_SPLIT_AQ 0
-#endif
-__device__ __forceinline__ float rsqrt_eval(float x) {
-  float y = rsqrt_fast(x);
-#if BH_RSQRT_NR
-  const float e = fmaf(x * y * y, -0.5f, 0.5f);
-  y = fmaf(y, e, y);
-#endif
-  return y;
-}
-__device__ __forceinline__ f32x2 rsqrt_eval2(float xa, float xb) {
-  f32x2 y = pk2(rsqrt_fast(xa), rsqrt_fast(xb));
-#if BH_RSQRT_NR
-  const f32x2 x = pk2(xa, xb);
-  const f32x2 e = fma2(mul2(mul2(x, y), y), bc2(-0.5f), bc2(0.5f));
-  y = fma2(y, e, y);
-#endif
-  return y;
-}
-
 template <int TPL, bool MASK>
 __device__ __forceinline__ void pp_one(const float4 s, uint32_t sidx, Targets<TPL> &T, float eps2) {
 #pragma unroll
@@ -291,7 +210,7 @@ __device__ __forceinline__ void pp_one(const float4 s, uint32_t sidx, Targets<TP
     if (MASK) {
       if (sidx == T.slot[t]) { m = 0.0f; r2 = 1.0f; }
     }
-    float ri = rsqrt_eval(r2);
+    float ri = rsqrt_fast(r2);
     float ri2 = ri * ri;
     float mr = m * ri;
     float mr3 = mr * ri2;
@@ -306,16 +225,27 @@ __device__ __forceinline__ void pp_one(const float4 s, uint32_t sidx, Targets<TP
 // rearranged exactly: with Q' = 3Q - tr(Q) I and w = r^T Q' r - tr(Q) eps^2,
 //   phi = -M rho - 1/2 w rho^5,   a = (M rho^3 + 5/2 w rho^7) r - rho^5 Q' r.
 // Staged per source: a = (cx,cy,cz,M), b = 2.5 (Q'xx,Q'yy,Q'zz, tr(Q) eps^2), c = 2.5 (Q'xy,Q'xz,Q'yz).
-// 33 FP32 instructions + 1 MUFU per target (the paper counts 65 flop for this interaction).
+// The two parts of a are summed separately within a tile, sum g r and sum rho^5 (2.5 Q' r), and joined with the factor
+// -0.4 once per tile: 32 FP32 instructions + 1 MUFU per target (the paper counts 65 flop for this interaction).
 template <int TPL>
-__device__ __forceinline__ void pc_one(const float4 a, const float4 b, const float4 c, Targets<TPL> &T, float eps2) {
+struct QuadAcc {  // sum over one tile of rho^5 (2.5 Q' r) per target; a += -0.4 x that, once per tile (pc_tile_end)
+  float x[TPL], y[TPL], z[TPL];
+  __device__ __forceinline__ QuadAcc() {
+#pragma unroll
+    for (int t = 0; t < TPL; ++t) x[t] = y[t] = z[t] = 0.0f;
+  }
+};
+
+template <int TPL>
+__device__ __forceinline__ void pc_one(const float4 a, const float4 b, const float4 c, Targets<TPL> &T, QuadAcc<TPL> &A,
+                                       float eps2) {
 #pragma unroll
   for (int t = 0; t < TPL; ++t) {
     float dx = a.x - T.x[t], dy = a.y - T.y[t], dz = a.z - T.z[t];
     float r2 = fmaf(dx, dx, eps2);
     r2 = fmaf(dy, dy, r2);
     r2 = fmaf(dz, dz, r2);
-    float ri = rsqrt_eval(r2);
+    float ri = rsqrt_fast(r2);
     float vx = fmaf(c.y, dz, fmaf(c.x, dy, b.x * dx));   // 2.5 Q' r
     float vy = fmaf(c.z, dz, fmaf(b.y, dy, c.x * dx));
     float vz = fmaf(b.z, dz, fmaf(c.z, dy, c.y * dx));
@@ -327,10 +257,22 @@ __device__ __forceinline__ void pc_one(const float4 a, const float4 b, const flo
     T.ph[t] = fmaf(-a.w, ri, T.ph[t]);       // -M rho
     T.phq[t] = fmaf(w, ri5, T.phq[t]);       // 2.5 w rho^5; folded in as -0.2 x
     float g = fmaf(w, ri4, a.w) * ri3;       // M rho^3 + 2.5 w rho^7
-    float k = -0.4f * ri5;                   // - rho^5 Q' r = k (2.5 Q' r)
-    T.ax[t] = fmaf(k, vx, fmaf(g, dx, T.ax[t]));
-    T.ay[t] = fmaf(k, vy, fmaf(g, dy, T.ay[t]));
-    T.az[t] = fmaf(k, vz, fmaf(g, dz, T.az[t]));
+    T.ax[t] = fmaf(g, dx, T.ax[t]);
+    T.ay[t] = fmaf(g, dy, T.ay[t]);
+    T.az[t] = fmaf(g, dz, T.az[t]);
+    A.x[t] = fmaf(ri5, vx, A.x[t]);          // rho^5 (2.5 Q' r): - rho^5 Q' r = -0.4 x this, applied per tile
+    A.y[t] = fmaf(ri5, vy, A.y[t]);
+    A.z[t] = fmaf(ri5, vz, A.z[t]);
+  }
+}
+
+template <int TPL>
+__device__ __forceinline__ void pc_tile_end(Targets<TPL> &T, const QuadAcc<TPL> &A) {
+#pragma unroll
+  for (int t = 0; t < TPL; ++t) {
+    T.ax[t] = fmaf(-0.4f, A.x[t], T.ax[t]);
+    T.ay[t] = fmaf(-0.4f, A.y[t], T.ay[t]);
+    T.az[t] = fmaf(-0.4f, A.z[t], T.az[t]);
   }
 }
 
@@ -344,23 +286,17 @@ __device__ __forceinline__ void pc_one(const float4 a, const float4 b, const flo
 // ------------------------------------------------------------------------------------------
 struct Targets2 {  // the packed view of Targets<2> during one tile
   f32x2 x, y, z, ax, ay, az, ph, phq;
-#if BH_SPLIT_AQ
-  f32x2 qx = 0ull, qy = 0ull, qz = 0ull;  // sum of rho^5 (2.5 Q' r) over the tile; -0.4 x is added to a in store()
-#endif
+  f32x2 qx = 0ull, qy = 0ull, qz = 0ull;  // p-c tiles: sum of rho^5 (2.5 Q' r) over the tile (pc_tile_end2)
   __device__ __forceinline__ explicit Targets2(const Targets<2> &T)
       :
-#if BH_PACK_HOME
-        x(T.xp), y(T.yp), z(T.zp),
-#else
-        x(pk2(T.x[0], T.x[1])), y(pk2(T.y[0], T.y[1])), z(pk2(T.z[0], T.z[1])),
-#endif
+        x(T.xp), y(T.yp), z(T.zp),  // packed once when the task loads its targets (walk_task)
         ax(pk2(T.ax[0], T.ax[1])),
         ay(pk2(T.ay[0], T.ay[1])), az(pk2(T.az[0], T.az[1])), ph(pk2(T.ph[0], T.ph[1])), phq(pk2(T.phq[0], T.phq[1])) {}
-  __device__ __forceinline__ void store(Targets<2> &T) const {
-#if BH_SPLIT_AQ
+  __device__ __forceinline__ void pc_tile_end2() {  // a += -0.4 x the tile's sum of rho^5 (2.5 Q' r)
     const f32x2 m = bc2(-0.4f);
-    const f32x2 ax = fma2(m, qx, this->ax), ay = fma2(m, qy, this->ay), az = fma2(m, qz, this->az);
-#endif
+    ax = fma2(m, qx, ax); ay = fma2(m, qy, ay); az = fma2(m, qz, az);
+  }
+  __device__ __forceinline__ void store(Targets<2> &T) const {
     up2(ax, T.ax[0], T.ax[1]); up2(ay, T.ay[0], T.ay[1]); up2(az, T.az[0], T.az[1]);
     up2(ph, T.ph[0], T.ph[1]); up2(phq, T.phq[0], T.phq[1]);
   }
@@ -378,7 +314,7 @@ __device__ __forceinline__ void pp_one2(const float4 s, uint32_t sidx, const uin
     if (sidx == slot[0]) { m0 = 0.0f; r2a = 1.0f; }
     if (sidx == slot[1]) { m1 = 0.0f; r2b = 1.0f; }
   }
-  const f32x2 ri = rsqrt_eval2(r2a, r2b);
+  const f32x2 ri = pk2(rsqrt_fast(r2a), rsqrt_fast(r2b));
   const f32x2 ri2 = mul2(ri, ri);
   const f32x2 mr = mul2(MASK ? pk2(m0, m1) : bc2(s.w), ri);
   const f32x2 mr3 = mul2(mr, ri2);
@@ -396,7 +332,7 @@ __device__ __forceinline__ void pc_one2(const float4 a, const float4 b, const fl
   r2 = fma2(dz, dz, r2);
   float r2a, r2b;
   up2(r2, r2a, r2b);
-  const f32x2 ri = rsqrt_eval2(r2a, r2b);
+  const f32x2 ri = pk2(rsqrt_fast(r2a), rsqrt_fast(r2b));
   const f32x2 vx = fma2(bc2(c.y), dz, fma2(bc2(c.x), dy, mul2(bc2(b.x), dx)));
   const f32x2 vy = fma2(bc2(c.z), dz, fma2(bc2(b.y), dy, mul2(bc2(c.x), dx)));
   const f32x2 vz = fma2(bc2(b.z), dz, fma2(bc2(c.z), dy, mul2(bc2(c.y), dx)));
@@ -408,15 +344,8 @@ __device__ __forceinline__ void pc_one2(const float4 a, const float4 b, const fl
   T.ph = fma2(bc2(-a.w), ri, T.ph);
   T.phq = fma2(w, ri5, T.phq);
   const f32x2 g = mul2(fma2(w, ri4, bc2(a.w)), ri3);
-#if BH_SPLIT_AQ
   T.ax = fma2(g, dx, T.ax); T.ay = fma2(g, dy, T.ay); T.az = fma2(g, dz, T.az);
   T.qx = fma2(ri5, vx, T.qx); T.qy = fma2(ri5, vy, T.qy); T.qz = fma2(ri5, vz, T.qz);
-#else
-  const f32x2 k = mul2(bc2(-0.4f), ri5);
-  T.ax = fma2(k, vx, fma2(g, dx, T.ax));
-  T.ay = fma2(k, vy, fma2(g, dy, T.ay));
-  T.az = fma2(k, vz, fma2(g, dz, T.az));
-#endif
 }
 
 template <int TPL>
@@ -459,15 +388,18 @@ __device__ __forceinline__ void eval_pc_tile(const WarpSmem &ws, int cnt, Target
     } else {
       for (int j = 0; j < cnt; ++j) pc_one2(ws.pc0[j], ws.pc1[j], ws.pc2[j], P2, e2);
     }
+    P2.pc_tile_end2();
     P2.store(T);
     return;
   }
+  QuadAcc<TPL> A;
   if (cnt == 32) {
 #pragma unroll(PC_UNROLL)
-    for (int j = 0; j < 32; ++j) pc_one<TPL>(ws.pc0[j], ws.pc1[j], ws.pc2[j], T, eps2);
+    for (int j = 0; j < 32; ++j) pc_one<TPL>(ws.pc0[j], ws.pc1[j], ws.pc2[j], T, A, eps2);
   } else {
-    for (int j = 0; j < cnt; ++j) pc_one<TPL>(ws.pc0[j], ws.pc1[j], ws.pc2[j], T, eps2);
+    for (int j = 0; j < cnt; ++j) pc_one<TPL>(ws.pc0[j], ws.pc1[j], ws.pc2[j], T, A, eps2);
   }
+  pc_tile_end<TPL>(T, A);
 }
 
 // Take `want` (<= 32) particles from the back of the p-p range queue; if `load`, stage them.
@@ -562,15 +494,7 @@ __device__ __forceinline__ void flush_queues(WarpSmem &ws, int lane, WalkState<T
 }
 
 // a12, second half kick of a step, fused into the walk's epilogue: v = fma(a, dt/2, v) (T12)
-#ifndef BH_KICK_INLINE
-#define BH_KICK_INLINE 1
-#endif
-#if BH_KICK_INLINE
-__device__ __forceinline__
-#else
-__device__ __noinline__
-#endif
-void kick_slot(float4 *v, const float4 a, float hdt) {
+__device__ __forceinline__ void kick_slot(float4 *v, const float4 a, float hdt) {
   float4 u = *v;
   u.x = __fmaf_rn(a.x, hdt, u.x); u.y = __fmaf_rn(a.y, hdt, u.y); u.z = __fmaf_rn(a.z, hdt, u.z);
   *v = u;
@@ -601,7 +525,7 @@ __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, con
     T.ax[t] = T.ay[t] = T.az[t] = T.ph[t] = T.phq[t] = 0.0f;
     if (j >= gsize) T.slot[t] = 0xffffffffu;
   }
-  if constexpr (TPL == 2 && BH_PACKED && BH_PACK_HOME && !COUNT) {
+  if constexpr (TPL == 2 && BH_PACKED && !COUNT) {
     // scalar loads: the halves of a pair can then be the load destinations themselves (the quad of an LDG.128 cannot be
     // an aligned pair of two different targets, and ptxas would copy quad -> pair before every use)
     const unsigned j0 = lane < gsize ? lane : gsize - 1, j1 = lane + 32u < gsize ? lane + 32u : gsize - 1;
@@ -886,32 +810,14 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, COUNT ? COUNT_MINB : walk_min
 //   body : one task per ordinary group, in Peano-Hilbert order (L1/L2 locality between warps)
 //   tail : the last n_tail groups, TAIL_PARTS parts each, so that the kernel ends on small tasks
 // ------------------------------------------------------------------------------------------
-#ifndef BH_SPLIT_FINE
-#define BH_SPLIT_FINE 1.0
-#endif
-#ifndef BH_SPLIT_AT
-#define BH_SPLIT_AT 2.0
-#endif
-constexpr double SPLIT_FINE = BH_SPLIT_FINE;  // parts per mean-cost unit of an expensive group
-constexpr double SPLIT_AT = BH_SPLIT_AT;      // a group is expensive above this multiple of the mean cost
+constexpr double SPLIT_FINE = 1.0;  // parts per mean-cost unit of an expensive group
+constexpr double SPLIT_AT = 2.0;      // a group is expensive above this multiple of the mean cost
 constexpr unsigned MAX_PARTS = 63;
-#ifndef BH_SUSPECT_AT
-#define BH_SUSPECT_AT 3.0
-#endif
-#ifndef BH_BIG_BOX
-#define BH_BIG_BOX 0.35
-#endif
-constexpr double BIG_BOX = BH_BIG_BOX;  // a run's box diagonal against the bounding box's (task_cost_kernel)
-#ifndef BH_BIG_PARTS
-#define BH_BIG_PARTS 16
-#endif
-constexpr unsigned BIG_PARTS = BH_BIG_PARTS;
-constexpr double SUSPECT_AT = BH_SUSPECT_AT;  // a run's box diagonal against its neighbours' (task_cost_kernel)
-#ifndef BH_TAIL_PER_SM
-#define BH_TAIL_PER_SM 16
-#endif
+constexpr double BIG_BOX = 0.35;  // a run's box diagonal against the bounding box's (task_cost_kernel)
+constexpr unsigned BIG_PARTS = 16;
+constexpr double SUSPECT_AT = 3.0;  // a run's box diagonal against its neighbours' (task_cost_kernel)
 constexpr unsigned TAIL_PARTS = 4;
-constexpr long long TAIL_PER_SM = BH_TAIL_PER_SM;  // groups per SM at the end of the list that are cut into TAIL_PARTS
+constexpr long long TAIL_PER_SM = 16;  // groups per SM at the end of the list that are cut into TAIL_PARTS
 
 __global__ void walk_reset_kernel(DevInfo *info, unsigned n_groups) {
   if (threadIdx.x == 0) {
@@ -1486,10 +1392,7 @@ static int launch_walk(tree_ctx *t, const WalkParams &P, unsigned grid) {
 int run_walk(tree_ctx *t, float eps, float kick_hdt) {
   WalkParams P;
   P.reuse_mode = t->reuse_mode;
-#ifndef BH_FUSE_KICK
-#define BH_FUSE_KICK 1
-#endif
-  const bool fuse_kick = BH_FUSE_KICK && kick_hdt != 0.0f && t->shard_world <= 1;
+  const bool fuse_kick = kick_hdt != 0.0f && t->shard_world <= 1;
   P.svel = fuse_kick ? t->b.svel : nullptr;
   P.kick_hdt = kick_hdt;
   P.spos = t->b.spos; P.c_test = t->b.c_test; P.c_link = t->b.c_link;

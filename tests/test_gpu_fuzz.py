@@ -56,9 +56,15 @@ def _one(rng):
     assert np.array_equal(cnt[:, 0], onpp) and np.array_equal(cnt[:, 1], onpc), tag
     if n > 1:
         an = a.cpu().numpy().astype(np.float64); pn = ph.cpu().numpy().astype(np.float64)
-        rel = (np.linalg.norm(an - oacc, axis=1) / np.linalg.norm(oacc, axis=1)).max()
+        relv = np.linalg.norm(an - oacc, axis=1) / np.linalg.norm(oacc, axis=1)
+        rel = relv.max()
         prel = (np.abs(pn - opot) / np.abs(opot)).max()
         assert rel <= 1e-5 and prel <= 1e-5, (tag, rel, prel)
+        # the form of the bound that holds whatever the cancellation: the absolute error of a_i is
+        # at most 2.5e-7 x A_i, A_i = sum of the magnitudes of the terms of particle i's interaction list
+        i = int(relv.argmax())
+        A = ot.abs_sum(theta, eps, [i])[0]
+        assert np.linalg.norm(an[i] - oacc[i]) <= 2.5e-7 * A, (tag, i, np.linalg.norm(an[i] - oacc[i]) / A)
     for t in trees:
         t.close()
 
