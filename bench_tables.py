@@ -4,6 +4,8 @@
                  (``--from-ncu FILE``: a ``--metrics gpu__time_duration.sum,dram__bytes_read.sum,dram__bytes_write.sum``
                  pass), against the measured copy bandwidth of MEASURED_PEAKS.json and the algorithmic bytes of DESIGN.md §5
   shard-scaling  per-rank cost of the sharded force pass measured on ONE GPU with W contexts
+  sass-histogram instruction classes of the whole kernel and of every innermost loop of a ``cuobjdump -sass`` listing
+                 (``--from-sass FILE``)
   mac-sweep      error versus cost of the acceptance criteria: opening angle x criterion on a
                  BASELINE.json configuration, force error against tree_direct on a 16,384 subsample
 
@@ -207,6 +209,46 @@ def table_mac_sweep(config: int):
             t.close()
 
 
+def table_sass_histogram(path: str):
+    """Instruction histogram of a `cuobjdump -sass -fun KERNEL libbhtree.so` listing: whole kernel and every innermost
+    loop (a backward branch that encloses no other), in the classes the roofline of the fused kernel talks about."""
+    import collections
+    ins = []
+    for ln in open(path).read().splitlines():
+        m = re.match(r"\s+/\*([0-9a-f]{4,})\*/\s+(.*?);", ln)
+        if m:
+            txt = re.sub(r"^@!?U?P\d+\s+", "", m.group(2).strip())
+            ins.append((int(m.group(1), 16), txt.split()[0].split(".")[0], txt))
+    loops = []
+    for a, op, txt in ins:
+        if op == "BRA":
+            m = re.search(r"0x([0-9a-f]+)", txt)
+            if m and int(m.group(1), 16) < a:
+                loops.append((int(m.group(1), 16), a))
+    inner = [l for l in loops if not any(o != l and l[0] <= o[0] and o[1] <= l[1] for o in loops)]
+    scalar = ("FFMA", "FMUL", "FADD", "FSEL", "FSETP", "FMNMX", "FMNMX3")
+
+    def cls(op):
+        return op if op in ("FFMA2", "FMUL2", "FADD2", "MUFU", "LDS") else ("FP32 scalar" if op in scalar else "other")
+
+    cols = ["FFMA2", "FMUL2", "FADD2", "MUFU", "LDS", "FP32 scalar", "other"]
+    print("| region | instructions | " + " | ".join(cols) + " | packed with a .reuse operand | most frequent other |")
+    print("|---|---|" + "---|" * (len(cols) + 2))
+
+    def row(name, body):
+        h = collections.Counter(cls(i[1]) for i in body)
+        oth = collections.Counter(i[1] for i in body if cls(i[1]) == "other").most_common(5)
+        reuse = sum(".reuse" in i[2] for i in body if i[1] in ("FFMA2", "FMUL2", "FADD2"))
+        print(f"| {name} | {len(body)} | " + " | ".join(str(h.get(c, 0)) for c in cols) + f" | {reuse} | "
+              + ", ".join(f"{k} {v}" for k, v in oth) + " |")
+
+    row("whole kernel", ins)
+    for tgt, a in sorted(inner, key=lambda x: -(x[1] - x[0])):
+        body = [i for i in ins if tgt <= i[0] <= a]
+        if len(body) >= 40:
+            row(f"loop 0x{tgt:x}..0x{a:x}", body)
+
+
 def run(args) -> int:
     if args.table == "kernels":
         from nbody_inputs import CONFIGS
@@ -215,6 +257,8 @@ def run(args) -> int:
         table_shard_scaling(args.config, [int(x) for x in args.worlds.split(",")], args.steps)
     elif args.table == "mac-sweep":
         table_mac_sweep(args.config)
+    elif args.table == "sass-histogram":
+        table_sass_histogram(args.from_sass)
     else:
         raise SystemExit(f"unknown table {args.table!r}")
     return 0

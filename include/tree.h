@@ -79,6 +79,9 @@ int tree_build(tree_ctx *t, const float *pos, const float *mass, long long N);
 
 /* Force pass on the last built tree (Eqs. (1),(2) L186-188): opening radii for
  * this theta, fused walk + evaluation, results to caller order.
+ * Accuracy against the FP64 sum of the same interaction lists: |phi - phi_exact| <= 1e-5 |phi|
+ * and |a - a_exact| <= max(1e-5 |a|, 2.5e-7 A), A = sum of the magnitudes of the terms of the particle's list; the
+ * second term only decides where the net force cancels to less than 1/40 of that sum.
  * theta >= 0 (0 = open everything = direct summation, L31); eps >= 0 (Plummer softening).
  * acc: DEV float[N][3] or NULL; pot: DEV float[N] or NULL.  The result is also kept inside the
  * context for tree_leapfrog / tree_get_state.
@@ -185,7 +188,7 @@ int tree_get_stats(tree_ctx *t, double *ms, unsigned long long *n_pp, unsigned l
  * the PH-sorted order with ~1/world of the estimated walk cost, and the walk kernel stores each
  * group's accelerations, potentials and interaction counts straight into the result buffers of
  * every attached context over NVLink (peer stores): there is no separate collective.  The one
- * exchange step is a barrier between the two halves of the pass, which the CALLER provides
+ * exchange step of a force pass is a barrier between its two halves, which the CALLER provides
  * (e.g. one NCCL all-reduce on the contexts' streams; the binding's ShardedTree does that):
  *     tree_force_begin on every context  ->  barrier  ->  tree_force_end on every context.
  * Results are those of the same pass on one context up to the order of a few partial sums (the task
@@ -222,9 +225,19 @@ int tree_shard_attach_local(tree_ctx *t, int peer_rank, tree_ctx *peer);
 int tree_force_begin(tree_ctx *t, float theta, float eps);
 /* Second half, after the caller's barrier: results to caller order (acc, pot as in tree_force). */
 int tree_force_end(tree_ctx *t, float *acc, float *pot);
-/* tree_leapfrog in two halves around the same barrier: kick, drift, rebuild, tree_force_begin |
- * tree_force_end, kick. */
+/* tree_leapfrog of a sharded context, in three parts around TWO barriers of the caller:
+ *     tree_leapfrog_begin  kick, drift, bounding box, keys of all N; then the sort is cut by KEY RANGE (PAPER.md L93-97:
+ *                          contiguous pieces of the PH curve): the keys at the slot boundaries N r / world of the previous
+ *                          sorted order are splitters every context holds, context r sorts only the particles whose new
+ *                          key falls into its range and stores the sorted run at its offset into every context
+ *     -> barrier
+ *     tree_leapfrog_mid    gather into the new order, octree, moments, tree_force_begin
+ *     -> barrier
+ *     tree_leapfrog_end    tree_force_end, kick.
+ * On a context that is not sharded (world = 1) tree_leapfrog_begin does the first two parts and tree_leapfrog_mid
+ * returns at once. */
 int tree_leapfrog_begin(tree_ctx *t, float dt);
+int tree_leapfrog_mid(tree_ctx *t);
 int tree_leapfrog_end(tree_ctx *t);
 /* The range of groups [*g_lo, *g_hi) and of slots [*s_lo, *s_hi) this context walked in the last
  * pass, to HOST memory (any pointer may be NULL).  Synchronises. */

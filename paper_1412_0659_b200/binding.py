@@ -52,6 +52,7 @@ _SIGS = {
     "tree_force_begin": (C.c_int, [C.c_void_p, C.c_float, C.c_float]),
     "tree_force_end": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "tree_leapfrog_begin": (C.c_int, [C.c_void_p, C.c_float]),
+    "tree_leapfrog_mid": (C.c_int, [C.c_void_p]),
     "tree_leapfrog_end": (C.c_int, [C.c_void_p]),
     "tree_shard_range": (C.c_int, [C.c_void_p] + [C.POINTER(C.c_longlong)] * 4),
     "tree_fp32_peak": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
@@ -211,6 +212,9 @@ class Tree:
 
     def leapfrog_begin(self, dt: float):
         _check(self.h, load_library().tree_leapfrog_begin(self.h, float(dt)))
+
+    def leapfrog_mid(self):
+        _check(self.h, load_library().tree_leapfrog_mid(self.h))
 
     def leapfrog_end(self):
         _check(self.h, load_library().tree_leapfrog_end(self.h))

@@ -75,7 +75,18 @@ struct DeviceScope {
   bh::DeviceScope _dev_scope((t)->device);                                                  \
   if (_dev_scope.err != cudaSuccess) return bh::set_err((t), TREE_ERR_CUDA, "cudaSetDevice", _dev_scope.err)
 
-static size_t slab_bytes(long long cap, long long ng) { return 2 * (size_t)cap * sizeof(float4) + 2 * (size_t)ng * sizeof(uint2); }
+static size_t slab_results_bytes(long long cap, long long ng) { return 2 * (size_t)cap * sizeof(float4) + 2 * (size_t)ng * sizeof(uint2); }
+static size_t slab_bytes(long long cap, long long ng) {
+  return slab_results_bytes(cap, ng) + (size_t)cap * sizeof(uint64_t) + (size_t)cap * sizeof(uint32_t);
+}
+
+// the exchanged sorted keys / previous slots of a sharded step inside a slab (8-byte aligned: the results are 16 N + 8 n_g)
+void shard_xviews(const tree_ctx *t, void *base, uint64_t **xkey, uint32_t **xperm) {
+  const long long ng = (t->cap + t->group - 1) / t->group;
+  char *p = (char *)base + slab_results_bytes(t->cap, ng);
+  *xkey = (uint64_t *)p;
+  *xperm = (uint32_t *)(p + (size_t)t->cap * sizeof(uint64_t));
+}
 
 // result buffers inside a slab of `t`'s reserved sizes (the local one or a mapped peer's)
 void shard_views(const tree_ctx *t, void *base, int parity, float4 **sacc, uint2 **gcount) {
@@ -145,6 +156,8 @@ static int ensure_particles(tree_ctx *t, long long N) {
   t->sort_epoch = 0;
   t->cap = cap;
   for (int k = 0; k < 2; ++k) shard_views(t, b.shard_slab, k, &b.sacc2[k], &b.gcount2[k]);
+  shard_xviews(t, b.shard_slab, &b.xkey, &b.xperm);
+  t->split_valid = false;
   b.sacc = b.sacc2[t->pass & 1];
   b.gcount = b.gcount2[t->pass & 1];
   t->have_vel = false;
@@ -190,12 +203,14 @@ static int build_from_posm(tree_ctx *t) {
   rec(t, EV_KEYS);
   BH_TRY(run_sort(t));
   rec(t, EV_SORT);
+  rec(t, EV_SORT2);
   BH_TRY(run_permute_build(t));
   rec(t, EV_PERM);
   t->state_valid = true;
   BH_TRY(run_tree(t, /*async=*/false));
   rec(t, EV_BUILD);
   BH_TRY(run_groups_moments(t));
+  if (t->shard_world > 1) BH_TRY(run_save_splitters(t));
   rec(t, EV_MOM);
   t->built = true;
   return 0;
@@ -252,7 +267,9 @@ static int force_impl(tree_ctx *t, float theta, float eps, float *acc, float *po
 
 // One step without a host round trip: the state stays in slot order, the cell arrays
 // are used up to a bound the device checks, the cell count travels back asynchronously for the next step.
-static int leapfrog_begin_impl(tree_ctx *t, float dt) {
+// Phase 1: kick + drift + bbox, keys, sort.  A sharded context sorts only its own key range and stores the sorted run
+// into every rank (run_sort_bucket); the caller's barrier follows, then phase 2 (tree_leapfrog_mid).
+static int step_phase1(tree_ctx *t, float dt) {
   // room for this step's tree: the latest known cell count plus a margin (grown here, synchronously, when the
   // margin has been used up: the arrays are rebuilt below anyway)
   poll_cells(t);
@@ -260,6 +277,11 @@ static int leapfrog_begin_impl(tree_ctx *t, float dt) {
   if (want > t->cell_cap) {
     BH_CUDA(cudaStreamSynchronize(t->stream));
     BH_TRY(ensure_cells(t, want));
+  }
+  if (t->shard_world > 1) {
+    for (int r = 0; r < t->shard_world; ++r)
+      if (r != t->shard_rank && !t->peer_base[r]) return set_err(t, TREE_ERR_ORDER, "sharded context: a peer is not attached");
+    if (!t->split_valid) BH_TRY(run_save_splitters(t));  // (normally saved by the previous rebuild)
   }
   rec(t, EV_I0);
   BH_TRY(run_kick_drift_bbox(t, dt));
@@ -269,25 +291,41 @@ static int leapfrog_begin_impl(tree_ctx *t, float dt) {
   rec(t, EV_B0);
   BH_TRY(run_keys(t, t->b.spos));
   rec(t, EV_KEYS);
-  BH_TRY(run_sort(t));
+  if (t->shard_world > 1) BH_TRY(run_sort_bucket(t)); else BH_TRY(run_sort(t));
   rec(t, EV_SORT);
+  t->step_open = true;
+  t->step_mid_done = false;
+  t->step_dt = dt;
+  return 0;
+}
+
+// Phase 2: gather the state into the new order, octree, moments, first half of the force pass.
+static int step_phase2(tree_ctx *t) {
+  rec(t, EV_SORT2);
   BH_TRY(run_permute_step(t));
   rec(t, EV_PERM);
   BH_TRY(run_tree(t, /*async=*/true));
   rec(t, EV_BUILD);
   BH_TRY(run_groups_moments(t));
+  if (t->shard_world > 1) BH_TRY(run_save_splitters(t));  // for the next step, before any peer can store new keys here
   rec(t, EV_MOM);
   t->built = true;
   t->reuse_mode = 1;  // same particles one step later: last pass's counts predict this pass's costs
-  const int frc = force_begin_impl(t, t->theta, t->eps, t->shard_world <= 1 ? 0.5f * dt : 0.0f);
+  const int frc = force_begin_impl(t, t->theta, t->eps, t->shard_world <= 1 ? 0.5f * t->step_dt : 0.0f);
   t->reuse_mode = 0;
   if (frc) return frc;
-  t->step_open = true;
-  t->step_dt = dt;
+  t->step_mid_done = true;
+  return 0;
+}
+
+static int leapfrog_begin_impl(tree_ctx *t, float dt) {
+  BH_TRY(step_phase1(t, dt));
+  if (t->shard_world <= 1) BH_TRY(step_phase2(t));
   return 0;
 }
 
 static int leapfrog_end_impl(tree_ctx *t) {
+  if (!t->step_mid_done) return set_err(t, TREE_ERR_ORDER, "sharded context: tree_leapfrog_mid (after the first barrier) is missing");
   BH_TRY(force_end_impl(t, nullptr, nullptr));
   rec(t, EV_I2);
   if (t->shard_world > 1) BH_TRY(run_kick(t, t->step_dt));  // one context: done in the walk's epilogue
@@ -409,6 +447,14 @@ int tree_leapfrog_begin(tree_ctx *t, float dt) {
   return leapfrog_begin_impl(t, dt);
 }
 
+int tree_leapfrog_mid(tree_ctx *t) {
+  if (!t) return TREE_ERR_ARG;
+  if (!t->step_open) return set_err(t, TREE_ERR_ORDER, "tree_leapfrog_mid without tree_leapfrog_begin");
+  if (t->step_mid_done) return TREE_OK;  // one context: tree_leapfrog_begin has done it all
+  BH_DEVICE(t);
+  return step_phase2(t);
+}
+
 int tree_leapfrog_end(tree_ctx *t) {
   if (!t) return TREE_ERR_ARG;
   if (!t->step_open) return set_err(t, TREE_ERR_ORDER, "tree_leapfrog_end without tree_leapfrog_begin");
@@ -464,6 +510,7 @@ int tree_shard_config(tree_ctx *t, int rank, int world) {
   t->b.gcount = t->b.gcount2[0];
   t->prev_valid = false;   // the other parity no longer holds "the previous pass"
   t->have_force = false;
+  t->split_valid = false;
   return TREE_OK;
 }
 
@@ -659,14 +706,14 @@ int tree_get_debug(tree_ctx *t, int what, void *dst, long long *count) {
       // keys live in slot order after the sort: scatter back through `order` on the host
       std::vector<uint64_t> sk(N);
       std::vector<uint32_t> ord(N);
-      BH_TRY(copy_out(t, sk.data(), t->b.key[t->sorted], N * 8));
+      BH_TRY(copy_out(t, sk.data(), t->b.skey, N * 8));
       BH_TRY(copy_out(t, ord.data(), t->b.order, N * 4));
       uint64_t *o = (uint64_t *)dst;
       for (long long s = 0; s < N; ++s) o[ord[s]] = sk[s];
       return 0;
     }
     case TREE_DBG_ORDER: *count = N; return dst ? copy_out(t, dst, t->b.order, N * 4) : 0;
-    case TREE_DBG_SORTED_KEYS: *count = N; return dst ? copy_out(t, dst, t->b.key[t->sorted], N * 8) : 0;
+    case TREE_DBG_SORTED_KEYS: *count = N; return dst ? copy_out(t, dst, t->b.skey, N * 8) : 0;
     case TREE_DBG_SORTED_POS: *count = N; return dst ? copy_out(t, dst, t->b.spos, N * 16) : 0;
     case TREE_DBG_CELLS: {
       *count = nc;
@@ -772,7 +819,7 @@ int tree_get_stats(tree_ctx *t, double *ms, unsigned long long *n_pp, unsigned l
   double *m = t->ms;
   m[TREE_PH_KEYS] = el(EV_B0, EV_KEYS);
   m[TREE_PH_SORT] = el(EV_KEYS, EV_SORT);
-  m[TREE_PH_PERMUTE] = el(EV_SORT, EV_PERM);
+  m[TREE_PH_PERMUTE] = el(EV_SORT2, EV_PERM);
   m[TREE_PH_BUILD] = el(EV_PERM, EV_BUILD);
   m[TREE_PH_MOMENTS] = el(EV_BUILD, EV_MOM);
   m[TREE_PH_OPENING] = t->have_force ? el(EV_F0, EV_OPEN) : 0.0;

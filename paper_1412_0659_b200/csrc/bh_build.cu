@@ -298,9 +298,12 @@ constexpr int OS_MINB = 5;  // resident blocks per SM (shared memory allows 6)
 constexpr unsigned long long OS_LOCAL = 1ull << 62, OS_INCL = 2ull << 62;
 constexpr int OS_LOOK = 4;  // status words one thread keeps in flight during the look-back
 
+// n_dev != nullptr: the number of keys is *n_dev (a bucket of a sharded step, known only on the device)
 __global__ void __launch_bounds__(256) sort_hist8_kernel(const uint64_t *__restrict__ key, long long N,
+                                                         const unsigned *__restrict__ n_dev,
                                                          uint32_t *__restrict__ ghist /*[8][256]*/) {
   __shared__ unsigned h[8 * RADIX];
+  if (n_dev) N = *n_dev;
   for (int i = threadIdx.x; i < 8 * RADIX; i += blockDim.x) h[i] = 0;
   __syncthreads();
   for (long long p = blockIdx.x * (long long)blockDim.x + threadIdx.x; p < N; p += (long long)gridDim.x * blockDim.x) {
@@ -356,16 +359,19 @@ __global__ void __launch_bounds__(OS_THREADS, OS_MINB) sort_onesweep_kernel(cons
                                                                    const uint32_t *__restrict__ gscan /*[256] of this pass*/,
                                                                    uint32_t *__restrict__ ticket,
                                                                    unsigned long long *__restrict__ status /*[tiles][256]*/,
-                                                                   unsigned long long epoch, int shift, long long N) {
+                                                                   unsigned long long epoch, int shift, long long N,
+                                                                   const unsigned *__restrict__ n_dev) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   OsSmem &sm = *reinterpret_cast<OsSmem *>(smem_raw);
   const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const unsigned lt = (1u << lane) - 1u;
+  if (n_dev) N = *n_dev;  // the grid covers an upper bound; tiles past the end take a ticket and leave
   if (threadIdx.x == 0) sm.tile = atomicAdd(ticket, 1u);
   for (int i = lane; i < RADIX; i += 32) sm.wc[w][i] = 0;
   __syncthreads();
   const unsigned tile = sm.tile;
   const long long base = (long long)tile * OS_TILE;
+  if (base >= N) return;  // block-uniform; nobody looks back at a tile that does not exist
   uint64_t key[OS_IPT];
   unsigned rank[OS_IPT];
   // warp-striped: warp w owns items [w*256, w*256+256) of the tile, item k of lane l at k*32+l
@@ -874,21 +880,23 @@ int run_keys(tree_ctx *t, const float4 *xyzm) {
   return 0;
 }
 
-int run_sort(tree_ctx *t) {
+// The eight passes over `bound` keys starting in buffer `start` of key[] / idx[].  n_dev: the real count on the device
+// (<= bound), or nullptr.  explicit_payload: idx[start] holds the payload (otherwise the first pass takes the identity).
+static int sort_passes(tree_ctx *t, int start, long long bound, const unsigned *n_dev, bool explicit_payload) {
   if (!t->sort_attr_set) {  // per context: function attributes are per device
     BH_CUDA(cudaFuncSetAttribute(sort_onesweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(OsSmem)));
     BH_CUDA(cudaFuncSetAttribute(sort_onesweep_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
     t->sort_attr_set = true;
   }
-  const unsigned ntiles = (unsigned)((t->N + OS_TILE - 1) / OS_TILE);
+  const unsigned ntiles = (unsigned)((bound + OS_TILE - 1) / OS_TILE);
   uint32_t *ghist = t->b.sort_hist, *ticket = t->b.sort_hist + 8 * RADIX;
   BH_CUDA(cudaMemsetAsync(ghist, 0, 8 * RADIX * sizeof(uint32_t), t->stream));
-  const long long hwant = (t->N + 256 * 16 - 1) / (256 * 16), hcap = (long long)t->sm_count * 8;
-  sort_hist8_kernel<<<(unsigned)(hwant < hcap ? hwant : hcap), 256, 0, t->stream>>>(t->b.key[0], t->N, ghist);
+  const long long hwant = (bound + 256 * 16 - 1) / (256 * 16), hcap = (long long)t->sm_count * 8;
+  sort_hist8_kernel<<<(unsigned)(hwant < hcap ? hwant : hcap), 256, 0, t->stream>>>(t->b.key[start], bound, n_dev, ghist);
   BH_LAUNCH_CHECK("sort_hist8");
   sort_scan8_kernel<<<8, RADIX, 0, t->stream>>>(ghist, ticket);
   BH_LAUNCH_CHECK("sort_scan8");
-  int cur = 0;
+  int cur = start;
   for (int pass = 0; pass < 8; ++pass) {
     const unsigned long long epoch = (++t->sort_epoch) & 0x3fffffffull;
     if (epoch == 0) {  // wrapped: old words could alias the new epoch
@@ -896,8 +904,8 @@ int run_sort(tree_ctx *t) {
       ++t->sort_epoch;
     }
     sort_onesweep_kernel<<<ntiles, OS_THREADS, sizeof(OsSmem), t->stream>>>(
-        t->b.key[cur], pass == 0 ? nullptr : t->b.idx[cur], t->b.key[cur ^ 1], t->b.idx[cur ^ 1], ghist + pass * RADIX,
-        ticket + pass, t->b.sort_status, t->sort_epoch & 0x3fffffffull, 8 * pass, t->N);
+        t->b.key[cur], (pass == 0 && !explicit_payload) ? nullptr : t->b.idx[cur], t->b.key[cur ^ 1], t->b.idx[cur ^ 1],
+        ghist + pass * RADIX, ticket + pass, t->b.sort_status, t->sort_epoch & 0x3fffffffull, 8 * pass, bound, n_dev);
     BH_LAUNCH_CHECK("sort_onesweep");
     cur ^= 1;
   }
@@ -905,8 +913,121 @@ int run_sort(tree_ctx *t) {
   return 0;
 }
 
+int run_sort(tree_ctx *t) {
+  BH_TRY_RC(sort_passes(t, 0, t->N, nullptr, false));
+  t->b.skey = t->b.key[t->sorted];
+  t->b.sperm = t->b.idx[t->sorted];
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------
+// Sharded step: the sort is cut by KEY RANGE.  The keys found at the slot boundaries N r / world of
+// the previous sorted order are splitters every rank holds; rank r takes the particles whose NEW key lies in
+// [split[r], split[r+1]) -- its own slice of the previous order plus the few neighbours that crossed a boundary
+// (contiguous pieces of the PH curve) -- sorts that bucket alone and stores the sorted (key, previous
+// slot) run at the bucket's offset into every rank's xkey / xperm (peer stores).  After the caller's barrier all ranks
+// hold the complete sorted arrays.  Equal keys all fall into one bucket; their order inside it is left to
+// permute_step_kernel, which ranks ties by caller index anyway, so the compaction need not be stable.
+// ------------------------------------------------------------------------------------------
+__global__ void save_splitters_kernel(const uint64_t *__restrict__ skey, long long N, int world, DevInfo *info) {
+  const int r = threadIdx.x;
+  if (r < world) info->split[r] = r == 0 ? 0ull : skey[(N * r) / world];
+}
+
+__global__ void bucket_reset_kernel(DevInfo *info) {
+  if (threadIdx.x < TREE_SHARD_MAX_WORLD) info->bucket_cnt[threadIdx.x] = 0u;
+  if (threadIdx.x == 0) info->bucket_fill = 0u;
+}
+
+// counts every bucket (all ranks arrive at the same counts) and compacts this rank's bucket: (key, slot)
+__global__ void __launch_bounds__(256) bucket_kernel(const uint64_t *__restrict__ key, long long N, int rank, int world,
+                                                     DevInfo *info, uint64_t *__restrict__ out_key,
+                                                     uint32_t *__restrict__ out_slot) {
+  __shared__ unsigned long long sp[TREE_SHARD_MAX_WORLD];
+  __shared__ unsigned cnt[TREE_SHARD_MAX_WORLD];
+  if (threadIdx.x < TREE_SHARD_MAX_WORLD) {
+    sp[threadIdx.x] = threadIdx.x < world ? info->split[threadIdx.x] : ~0ull;
+    cnt[threadIdx.x] = 0u;
+  }
+  __syncthreads();
+  const int lane = threadIdx.x & 31;
+  for (long long base = (long long)blockIdx.x * blockDim.x; base < N; base += (long long)gridDim.x * blockDim.x) {
+    const long long i = base + threadIdx.x;
+    const bool valid = i < N;
+    unsigned long long k = 0;
+    int b = -1;
+    if (valid) {
+      k = key[i];
+      b = 0;
+      for (int r = 1; r < world; ++r) b += k >= sp[r];  // splitters are non-decreasing: b = last r with split[r] <= k
+    }
+    const unsigned same = __match_any_sync(0xffffffffu, b);  // neighbours on the curve share a bucket: one add per warp
+    if (valid && lane == __ffs(same) - 1) atomicAdd(&cnt[b], (unsigned)__popc(same));
+    const bool mine = b == rank;
+    const unsigned m = __ballot_sync(0xffffffffu, mine);
+    if (m) {
+      unsigned at = 0;
+      if (lane == __ffs(m) - 1) at = atomicAdd(&info->bucket_fill, (unsigned)__popc(m));
+      at = __shfl_sync(0xffffffffu, at, __ffs(m) - 1);
+      if (mine) {
+        const unsigned dst = at + __popc(m & ((1u << lane) - 1u));
+        out_key[dst] = k;
+        out_slot[dst] = (uint32_t)i;
+      }
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x < world && cnt[threadIdx.x]) atomicAdd(&info->bucket_cnt[threadIdx.x], cnt[threadIdx.x]);
+}
+
+struct XDest { uint64_t *key[TREE_SHARD_MAX_WORLD]; uint32_t *perm[TREE_SHARD_MAX_WORLD]; int n; };
+
+// the sorted bucket to its place in every rank's sorted arrays (own copy included)
+__global__ void __launch_bounds__(256) bucket_store_kernel(const uint64_t *__restrict__ skey, const uint32_t *__restrict__ sperm,
+                                                           int rank, const DevInfo *__restrict__ info, const XDest D) {
+  const unsigned n = info->bucket_cnt[rank];
+  unsigned off = 0;
+  for (int r = 0; r < rank; ++r) off += info->bucket_cnt[r];
+  for (unsigned i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    const uint64_t k = skey[i];
+    const uint32_t p = sperm[i];
+    for (int q = 0; q < D.n; ++q) { D.key[q][off + i] = k; D.perm[q][off + i] = p; }
+  }
+}
+
+int run_save_splitters(tree_ctx *t) {
+  save_splitters_kernel<<<1, 32, 0, t->stream>>>(t->b.skey, t->N, t->shard_world, t->d_info);
+  BH_LAUNCH_CHECK("save_splitters");
+  t->split_valid = true;
+  return 0;
+}
+
+int run_sort_bucket(tree_ctx *t) {
+  bucket_reset_kernel<<<1, 32, 0, t->stream>>>(t->d_info);
+  BH_LAUNCH_CHECK("bucket_reset");
+  // new keys of all N are in key[0]; the bucket is compacted into key[1] / idx[1] and sorted from there
+  bucket_kernel<<<grid_for(t, t->N, 256, 8), 256, 0, t->stream>>>(t->b.key[0], t->N, t->shard_rank, t->shard_world, t->d_info,
+                                                                  t->b.key[1], t->b.idx[1]);
+  BH_LAUNCH_CHECK("bucket");
+  // the bucket's size is known on the device only: the grids cover all N, tiles past the end leave at once
+  BH_TRY_RC(sort_passes(t, 1, t->N, &t->d_info->bucket_cnt[t->shard_rank], true));
+  XDest D;
+  D.n = 0;
+  for (int r = 0; r < t->shard_world; ++r) {
+    void *base = r == t->shard_rank ? t->b.shard_slab : t->peer_base[r];
+    shard_xviews(t, base, &D.key[D.n], &D.perm[D.n]);
+    ++D.n;
+  }
+  bucket_store_kernel<<<grid_for(t, (t->N + t->shard_world - 1) / t->shard_world, 256, 8), 256, 0, t->stream>>>(
+      t->b.key[t->sorted], t->b.idx[t->sorted], t->shard_rank, t->d_info, D);
+  BH_LAUNCH_CHECK("bucket_store");
+  t->b.skey = t->b.xkey;
+  t->b.sperm = t->b.xperm;
+  return 0;
+}
+
 int run_permute_build(tree_ctx *t) {
-  permute_build_kernel<<<(unsigned)((t->N + 255) / 256), 256, 0, t->stream>>>(t->b.posm, t->b.idx[t->sorted], t->b.spos,
+  permute_build_kernel<<<(unsigned)((t->N + 255) / 256), 256, 0, t->stream>>>(t->b.posm, t->b.sperm, t->b.spos,
                                                                              t->b.order, t->N);
   BH_LAUNCH_CHECK("permute_build");
   return 0;
@@ -915,7 +1036,7 @@ int run_permute_build(tree_ctx *t) {
 int run_permute_step(tree_ctx *t) {
   const int nxt = t->cur ^ 1;
   permute_step_kernel<<<(unsigned)((t->N + 255) / 256), 256, 0, t->stream>>>(
-      t->b.key[t->sorted], t->b.idx[t->sorted], t->b.spos, t->b.svel, t->b.order, t->b.spos2[nxt], t->b.svel2[nxt],
+      t->b.skey, t->b.sperm, t->b.spos, t->b.svel, t->b.order, t->b.spos2[nxt], t->b.svel2[nxt],
       t->b.order2[nxt], t->N);
   BH_LAUNCH_CHECK("permute_step");
   t->cur = nxt;
@@ -938,7 +1059,7 @@ void poll_cells(tree_ctx *t) {
 // asynchronously for the next step (poll_cells).
 int run_tree(tree_ctx *t, bool async) {
   const int ntiles = (int)((t->N + TREE_THREADS - 1) / TREE_THREADS);
-  const uint64_t *skey = t->b.key[t->sorted];
+  const uint64_t *skey = t->b.skey;
   tree_levels_kernel<<<ntiles, TREE_THREADS, 0, t->stream>>>(skey, t->N, t->leaf, ntiles, t->b.lv, t->b.scan_tmp);
   BH_LAUNCH_CHECK("tree_levels");
   uint32_t *total = t->b.scan_blk + (t->scan_cap / SCAN_TILE + 8);  // spare slot behind the block sums

@@ -40,6 +40,10 @@ struct DevInfo {
   int n_cells;                    // cells of the current tree (= level_off[NLEVELS])
   int ltop;                       // levels 0..ltop hold so few cells that one block computes their moments
   unsigned int nonfinite_sticky;  // sticky: a rebuild saw a non-finite position or mass (asynchronous steps report it late)
+  // sharded step (DESIGN.md §7 "partitioned sort"): key splitters of the previous sorted order and the bucket sizes
+  unsigned long long split[TREE_SHARD_MAX_WORLD];   // split[r] = first key of bucket r (split[0] unused: bucket 0 starts at 0)
+  unsigned int bucket_cnt[TREE_SHARD_MAX_WORLD];    // particles whose new key falls into bucket r
+  unsigned int bucket_fill;                         // compaction cursor of this context's own bucket
   unsigned int cells_overflow;    // sticky: an asynchronous rebuild needed more cells than allocated; the cell count it
                                   // needed.  Every later kernel of the step pipeline does nothing while it is set.
 };
@@ -62,7 +66,11 @@ struct Buffers {
   float4 *spos = nullptr;      // = spos2[cur]: x,y,z,m
   float4 *svel = nullptr;      // = svel2[cur]: vx,vy,vz,0
   uint32_t *order = nullptr;   // = order2[cur]: order[s] = caller index of the particle in slot s
-  void *shard_slab = nullptr;  // one allocation (one IPC handle): sacc2[0] | sacc2[1] | gcount2[0] | gcount2[1]
+  void *shard_slab = nullptr;  // one allocation (one IPC handle): sacc2[0] | sacc2[1] | gcount2[0] | gcount2[1] | xkey | xperm
+  uint64_t *xkey = nullptr;    // sharded step: the sorted keys, every rank's bucket stored at its offset by its owner
+  uint32_t *xperm = nullptr;   //               and the previous slot of each sorted particle
+  const uint64_t *skey = nullptr;   // the sorted keys of the current tree: key[sorted], or xkey after a sharded step
+  const uint32_t *sperm = nullptr;  // payload of the last sort: idx[sorted] or xperm
   float4 *sacc2[2] = {nullptr, nullptr};  // results in slot order, double-buffered by force pass
   float4 *sacc = nullptr;                 // = sacc2[pass & 1], the buffer of the current / last force pass
   uint16_t *lv = nullptr;   // per slot: L0 | Lleaf << 5
@@ -129,6 +137,8 @@ struct tree_ctx {
   unsigned pass = 0;                 // force passes begun; parity selects the result buffers
   bool force_open = false;           // between tree_force_begin and tree_force_end
   bool step_open = false;            // between tree_leapfrog_begin and tree_leapfrog_end
+  bool step_mid_done = false;        // sharded step: tree_leapfrog_mid has run (begin | barrier | mid | barrier | end)
+  bool split_valid = false;          // d_info->split holds the splitters of the current sorted order
   float step_dt = 0.f;
   float *open_acc = nullptr, *open_pot = nullptr;
   void *peer_base[TREE_SHARD_MAX_WORLD] = {};   // mapped result slab of each attached peer (nullptr: not attached)
@@ -148,7 +158,7 @@ struct tree_ctx {
 namespace bh {
 
 // event slots
-enum { EV_B0 = 0, EV_KEYS, EV_SORT, EV_PERM, EV_BUILD, EV_MOM, EV_F0, EV_OPEN, EV_SCHED, EV_WALK, EV_UNPERM,
+enum { EV_B0 = 0, EV_KEYS, EV_SORT, EV_SORT2, EV_PERM, EV_BUILD, EV_MOM, EV_F0, EV_OPEN, EV_SCHED, EV_WALK, EV_UNPERM,
        EV_I0, EV_I1, EV_I2, EV_I3, EV_COUNT };
 
 int set_err(tree_ctx *t, int code, const char *what, cudaError_t ce = cudaSuccess);
@@ -172,7 +182,10 @@ int check_sticky(tree_ctx *t);
 int run_pack_bbox(tree_ctx *t, const float *pos, const float *mass);  // caller arrays -> posm + bbox
 int run_kick_drift_bbox(tree_ctx *t, float dt);                        // leapfrog: kick + drift of the slot-order state + bbox
 int run_keys(tree_ctx *t, const float4 *xyzm);                         // grid + keys of posm (build) or spos (leapfrog)
-int run_sort(tree_ctx *t);
+int run_sort(tree_ctx *t);                            // all N keys of key[0], payload = identity
+int run_sort_bucket(tree_ctx *t);                     // sharded step: count, compact and sort this context's key range, store it to all
+int run_save_splitters(tree_ctx *t);                  // keys at the slot boundaries N r / world of the current sorted order
+void shard_xviews(const tree_ctx *t, void *base, uint64_t **xkey, uint32_t **xperm);
 int run_permute_build(tree_ctx *t);   // tree_build: posm -> spos, order (payload of the sort = caller index)
 int run_permute_step(tree_ctx *t);    // tree_leapfrog: spos, svel, order -> the new slot order (payload = previous slot)
 int run_tree(tree_ctx *t, bool async);  // octree construction; !async: synchronises once and sizes the cell arrays

@@ -4,8 +4,9 @@ DESIGN.md §7; PAPER.md L81-125 is the paper's multi-GPU scheme this replaces on
 Every rank (one process per GPU, ``torch.distributed``) holds all N particles and builds the same
 tree; rank r walks one contiguous, cost-balanced range of the Peano-Hilbert-sorted groups
  and its walk kernel stores the results straight into every rank's result
-buffers (peer stores over NVLink).  The only collective is the barrier between the two halves of a
-pass: one 8-byte all-reduce on the stream the context works on.
+buffers (peer stores over NVLink).  In a leapfrog step the sort is cut as well, by key range: every rank sorts its
+own range and stores the sorted run into every rank.  The only collectives are the barriers between the parts of a
+pass / step: one 8-byte all-reduce each on the stream the context works on.
 
 This module is host logic only: set-up (exchange of the IPC handles), the begin / barrier / end
 sequence, the reduced totals.  It drives any object with the ``Tree`` methods it names, so the
@@ -94,9 +95,11 @@ class ShardedTree:
         self.tree.force_end(acc, pot)
 
     def leapfrog(self, dt: float):
-        self.tree.leapfrog_begin(dt)
+        self.tree.leapfrog_begin(dt)   # kick, drift, keys; this rank's key range sorted and stored into every rank
         self._barrier()
-        self.tree.leapfrog_end()
+        self.tree.leapfrog_mid()       # gather, octree, moments, walk of this rank's groups (results into every rank)
+        self._barrier()
+        self.tree.leapfrog_end()       # kick
 
     def stats(self):
         """Per-phase times of this rank; interaction totals summed over ranks (each rank counts its range)."""
@@ -138,6 +141,9 @@ def force_local(trees, theta, eps, outs=None):
 def leapfrog_local(trees, dt):
     for t in trees:
         t.leapfrog_begin(dt)
+    torch.cuda.synchronize()
+    for t in trees:
+        t.leapfrog_mid()
     torch.cuda.synchronize()
     for t in trees:
         t.leapfrog_end()

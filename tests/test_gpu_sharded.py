@@ -274,7 +274,7 @@ acc = torch.zeros((n, 3), device="cuda"); pot = torch.zeros(n, device="cuda")
 t.build(pos.cuda(), mass.cuda()); t.set_velocity(vel.cuda())
 t.force_begin(theta, eps); host_barrier(); t.force_end(acc, pot)
 for _ in range(2):
-    t.leapfrog_begin(dt); host_barrier(); t.leapfrog_end()
+    t.leapfrog_begin(dt); host_barrier(); t.leapfrog_mid(); host_barrier(); t.leapfrog_end()
 p = torch.empty((n, 3), device="cuda"); a = torch.empty((n, 3), device="cuda"); ph = torch.empty(n, device="cuda")
 t.get_state(p, None, a, ph); torch.cuda.synchronize()
 lo, hi, _, _ = t.shard_range()
@@ -324,4 +324,52 @@ def test_cross_process_ipc_sharded_pass_two_processes_one_gpu(tmp_path):
     assert np.array_equal(r0["counts"][:, 0], onpp) and np.array_equal(r0["counts"][:, 1], onpc)
     rel = np.linalg.norm(r0["a"].astype(np.float64) - oacc, axis=1) / np.linalg.norm(oacc, axis=1)
     assert rel.max() <= TOL
+    _close(trees)
+
+
+@pytest.mark.parametrize("n,world,dt", [(2000, 5, 0.5), (70000, 8, 0.05), (150, 8, 0.2), (30000, 3, 1e-3)])
+def test_sharded_steps_cut_the_sort_by_key_range(n, world, dt):
+    # A sharded step sorts by key range: context r sorts the particles whose new key falls between the splitters of the
+    # previous order and stores the run into every context.  Large dt: particles move far, buckets become very uneven
+    # (some empty); whatever the cut, every context must end with the oracle's order, tree and counts on the final
+    # positions, bit-identical to a single context that sorted everything itself.
+    theta, eps, steps = 0.4, 0.05, 3
+    pos, vel, mass = plummer(n, 41)
+    dpos, dvel, dmass = pos.cuda(), vel.cuda(), mass.cuda()
+    one = Tree(device=0)
+    one.build(dpos, dmass); one.set_velocity(dvel); one.force(theta, eps)
+    trees = _make(world, n)
+    for t in trees:
+        t.build(dpos, dmass); t.set_velocity(dvel)
+    force_local(trees, theta, eps)
+    for _ in range(steps):
+        one.leapfrog(dt)
+        leapfrog_local(trees, dt)
+    torch.cuda.synchronize()
+
+    def state(t):
+        p = torch.empty((n, 3), device="cuda"); v = torch.empty((n, 3), device="cuda")
+        a = torch.empty((n, 3), device="cuda"); ph = torch.empty(n, device="cuda")
+        t.get_state(p, v, a, ph); torch.cuda.synchronize()
+        return p.cpu().numpy(), v.cpu().numpy(), a.cpu().numpy(), ph.cpu().numpy()
+
+    p1, v1, a1, ph1 = state(one)
+    p0, v0, a0, ph0 = state(trees[0])
+    # (the single context's task list differs, so a few partial sums are ordered differently: close, not identical)
+    assert np.abs(p0 - p1).max() <= 1e-5 * np.abs(p1).max()
+    ot = oracle.Tree(p0, mass.numpy())
+    key, order, skey = ot.keys()
+    oacc, opot, onpp, onpc = ot.force(theta, eps)
+    for t in trees:
+        p, v, a, ph = state(t)
+        assert np.array_equal(p, p0) and np.array_equal(v, v0)        # all contexts hold the same bits
+        assert np.array_equal(t.debug("order"), order)
+        assert np.array_equal(t.debug("sorted_keys"), skey)
+        assert np.array_equal(t.debug("cells"), ot.cells())
+        assert np.array_equal(t.debug("moments"), ot.moments())
+        cnt = t.debug("counts")
+        assert np.array_equal(cnt[:, 0], onpp) and np.array_equal(cnt[:, 1], onpc)
+        rel = np.linalg.norm(a.astype(np.float64) - oacc, axis=1) / np.linalg.norm(oacc, axis=1)
+        assert rel.max() <= TOL
+    one.close()
     _close(trees)

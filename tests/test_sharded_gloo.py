@@ -34,21 +34,27 @@ class StandInTree:
     def build(self, pos, mass): self.calls.append(("build",))
     def set_velocity(self, v): self.calls.append(("vel",))
 
-    def _begin(self):
+    def _begin(self, what="pass"):
         self.passes += 1
         if self.rank == 1:
             time.sleep(0.5)  # a slow rank: the others must wait for it at the barrier
-        with open(os.path.join(self.tmp, f"pass{self.passes}_from{self.rank}"), "w") as f:
+        with open(os.path.join(self.tmp, f"{what}{self.passes}_from{self.rank}"), "w") as f:
             f.write("stored")
 
-    def _end(self):
-        # every rank's first half must be complete: its "store" is visible
-        seen = [os.path.exists(os.path.join(self.tmp, f"pass{self.passes}_from{r}")) for r in range(self.world)]
-        self.calls.append(("end_saw_all", all(seen)))
+    def _end(self, what="pass", tag="end_saw_all"):
+        # every rank's preceding part must be complete: its "store" is visible
+        seen = [os.path.exists(os.path.join(self.tmp, f"{what}{self.passes}_from{r}")) for r in range(self.world)]
+        self.calls.append((tag, all(seen)))
 
     def force_begin(self, theta, eps): self.calls.append(("force_begin",)); self._begin()
     def force_end(self, acc=None, pot=None): self._end()
-    def leapfrog_begin(self, dt): self.calls.append(("leapfrog_begin",)); self._begin()
+    def leapfrog_begin(self, dt): self.calls.append(("leapfrog_begin",)); self._begin("sorted")   # sorted run "stored"
+
+    def leapfrog_mid(self):
+        self._end("sorted", "mid_saw_all")      # reads every rank's sorted run: needs the first barrier
+        self.passes -= 1
+        self._begin("pass")                     # the walk "stores" its results
+
     def leapfrog_end(self): self._end()
     def stats(self): return {"walk": 1.0 + self.rank}, 100 * (self.rank + 1), 7 * (self.rank + 1)
     def shard_range(self): return (self.rank, self.rank + 1, 64 * self.rank, 64 * (self.rank + 1))
@@ -88,8 +94,9 @@ def test_two_rank_sharded_sequence(tmp_path):
         assert names[:4] == ["reserve", "config", "export", "attach"]           # set-up order of include/tree.h
         assert calls[1] == ("config", rank, world)
         assert peers == [(1 - rank, bytes([2 - rank]) * 128)]                     # the OTHER rank's handle, under its rank
-        assert names[4:] == ["build", "vel", "force_begin", "end_saw_all", "leapfrog_begin", "end_saw_all", "close"]
-        assert all(c[1] for c in calls if c[0] == "end_saw_all")                 # the barrier sits between the halves
+        assert names[4:] == ["build", "vel", "force_begin", "end_saw_all", "leapfrog_begin", "mid_saw_all", "end_saw_all",
+                             "close"]
+        assert all(c[1] for c in calls if c[0] in ("end_saw_all", "mid_saw_all"))  # a barrier sits between the parts
         assert (pp, pc) == (300, 21)                                             # totals are summed over the ranks
         assert ms["walk"] == 1.0 + rank                                          # times stay per rank
 
