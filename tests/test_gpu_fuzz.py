@@ -128,3 +128,43 @@ def test_degenerate_geometries_against_oracle():
             assert (np.abs(pn - opot) / np.abs(opot)).max() <= 1e-5, tag
             assert np.linalg.norm(an - oacc, axis=1).max() <= 1e-3 * np.linalg.norm(oacc, axis=1).max(), tag
         t.close()
+
+
+def test_error_tail_report():
+    """Random configurations for BH_TAIL_SECONDS (default 20 s; profiles/r2_tolerance_tail.md is a 300 s run with -s):
+    the largest relative acceleration error of each, its cancellation factor kappa = A_i / |a_i| and its error in units
+    of A_i.  Every worst particle must obey |err| <= max(1e-5 |a_i|, 2.5e-7 A_i)."""
+    import os, time
+    budget = float(os.environ.get("BH_TAIL_SECONDS", "20"))
+    rng = np.random.default_rng(int(os.environ.get("BH_TAIL_SEED", "4242")))
+    t0 = time.time(); res = []
+    while time.time() - t0 < budget:
+        n = int(rng.choice([rng.integers(200, 5000), rng.integers(5000, 40000), rng.integers(40000, 250000)]))
+        model = str(rng.choice(["plummer", "mw"]))
+        leaf = int(rng.choice([8, 16, 32]))
+        theta = float(rng.choice([0.3, 0.4, 0.4, 0.6, 0.9])); eps = float(rng.choice([0.002, 0.01, 0.05]))
+        seed = int(rng.integers(1, 10**6))
+        pos, vel, mass = (plummer if model == "plummer" else milky_way)(n, seed)
+        t = Tree(device=0, leaf_size=leaf, group_size=64)
+        a = torch.empty((n, 3), device="cuda"); ph = torch.empty(n, device="cuda")
+        t.build(pos.cuda(), mass.cuda()); t.force(theta, eps, a, ph); torch.cuda.synchronize()
+        ot = oracle.Tree(pos.numpy(), mass.numpy(), leaf_size=leaf, group_size=64)
+        oacc, opot, onpp, onpc = ot.force(theta, eps)
+        an = a.cpu().numpy().astype(np.float64); pn = ph.cpu().numpy().astype(np.float64)
+        rel = np.linalg.norm(an - oacc, axis=1) / np.linalg.norm(oacc, axis=1); prel = np.abs(pn - opot) / np.abs(opot)
+        i = int(rel.argmax())
+        A = ot.abs_sum(theta, eps, [i])[0]
+        err = np.linalg.norm(an[i] - oacc[i])
+        res.append((rel.max(), prel.max(), n, model, leaf, theta, eps, seed, A / np.linalg.norm(oacc[i]), err / A))
+        assert err <= max(1e-5 * np.linalg.norm(oacc[i]), 2.5e-7 * A), res[-1]
+        assert prel.max() <= 1e-5, res[-1]
+        t.close()
+    res.sort(reverse=True)
+    above = sum(r[0] > 1e-5 for r in res)
+    print(f"\n{len(res)} random configurations in {budget:.0f} s; max relative acceleration error above 1e-5 in {above}; "
+          f"median of the maxima {np.median([r[0] for r in res]):.2e}; largest potential error {max(r[1] for r in res):.2e}")
+    print("| max rel acc err | max rel pot err | N | model | leaf | theta | eps | seed | kappa = A_i / |a_i| | err / A_i |")
+    print("|---|---|---|---|---|---|---|---|---|---|")
+    for r in res[:10]:
+        print("| %.2e | %.2e | %d | %s | %d | %.1f | %g | %d | %.1f | %.2e |" % r)
+    assert above <= max(1, len(res) // 200)
