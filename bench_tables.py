@@ -6,6 +6,8 @@
   shard-scaling  per-rank cost of the sharded force pass measured on ONE GPU with W contexts
   sass-histogram instruction classes of the whole kernel and of every innermost loop of a ``cuobjdump -sass`` listing
                  (``--from-sass FILE``)
+  walk-eval-split the fused kernel against its walk alone and its evaluation alone (tree_measure_listeval); ``--worlds``
+                 takes the list of configurations here (default 2,4)
   mac-sweep      error versus cost of the acceptance criteria: opening angle x criterion on a
                  BASELINE.json configuration, force error against tree_direct on a 16,384 subsample
 
@@ -35,7 +37,8 @@ ALGO_BYTES = {
     "tree_emit_kernel": ("N", 2),
     "groups_kernel": ("N", 16),
     "kick_kernel": ("N", 32 + 16),
-    "scatter_out_kernel": ("N", 20 + 16),
+    "gather_out_kernel": ("N", 20 + 16),
+    "inverse_order_kernel": ("N", 4 + 4),
 }
 
 
@@ -249,6 +252,32 @@ def table_sass_histogram(path: str):
             row(f"loop 0x{tgt:x}..0x{a:x}", body)
 
 
+def table_walk_eval_split(configs):
+    """tree_measure_listeval on BASELINE.json configurations: the fused walk+force kernel against the walk alone and the
+    evaluation alone (two kernels, lists through global memory)."""
+    import torch
+    from nbody_inputs import config as make_config
+    from paper_1412_0659_b200 import Tree
+    print("| workload | N | fused walk+force ms | walk alone ms | evaluation alone ms | evaluation / fused | walk / fused | "
+          "max rel deviation of a from the fused pass |")
+    print("|---|---|---|---|---|---|---|---|")
+    for k in configs:
+        cfg, pos, vel, mass = make_config(k, device="cuda")
+        t = Tree(device=0)
+        t.build(pos, mass); t.set_velocity(vel); t.force(cfg["theta"], cfg["eps"])
+        for _ in range(3):
+            t.leapfrog(cfg.get("dt", 1e-3))
+        fused = []
+        for _ in range(3):  # a plain force pass on the current tree, scheduled by the previous pass's counts
+            t.force(cfg["theta"], cfg["eps"]); fused.append(t.stats()[0]["walk"])
+        w, e, dev = t.measure_listeval()
+        f = min(fused)
+        print(f"| {cfg['name']} | {cfg['n']:,} | {f:.3f} | {w:.3f} | {e:.3f} | {e / f:.4f} | {w / f:.4f} | {dev:.2e} |", flush=True)
+        t.close()
+        del pos, vel, mass
+        torch.cuda.empty_cache()
+
+
 def run(args) -> int:
     if args.table == "kernels":
         from nbody_inputs import CONFIGS
@@ -257,6 +286,8 @@ def run(args) -> int:
         table_shard_scaling(args.config, [int(x) for x in args.worlds.split(",")], args.steps)
     elif args.table == "mac-sweep":
         table_mac_sweep(args.config)
+    elif args.table == "walk-eval-split":
+        table_walk_eval_split([int(x) for x in args.worlds.split(",")] if args.worlds != "1,2,4,8" else [2, 4])
     elif args.table == "sass-histogram":
         table_sass_histogram(args.from_sass)
     else:

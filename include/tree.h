@@ -248,6 +248,14 @@ int tree_shard_range(tree_ctx *t, long long *g_lo, long long *g_hi, long long *s
  * reported beside the nominal FP32 peak in the roofline of the fused walk+force kernel.  Synchronises. */
 int tree_fp32_peak(tree_ctx *t, double *tflops);
 
+/* Measurement aid: the walk and the evaluation of the LAST force pass again, as two
+ * kernels with the interaction lists going through global memory (one warp per group, groups in descending cost, no
+ * splitting; needs an unsharded context, group size 64 and lists below 2^32 entries: N <= ~50 M).  ms[0] = the walk
+ * alone (HOST double[2]), ms[1] = the evaluation alone, best of 3; *max_rel = largest relative deviation of its
+ * accelerations from the fused pass's (HOST).  The evaluation alone bounds what separating walker and evaluator warps
+ * could reach.  Allocates and frees its own buffers; synchronises. */
+int tree_measure_listeval(tree_ctx *t, double *ms, double *max_rel);
+
 /* Number of kernels this library launched on the context since tree_create (for accounting). */
 long long tree_launch_count(const tree_ctx *t);
 

@@ -56,6 +56,7 @@ _SIGS = {
     "tree_leapfrog_end": (C.c_int, [C.c_void_p]),
     "tree_shard_range": (C.c_int, [C.c_void_p] + [C.POINTER(C.c_longlong)] * 4),
     "tree_fp32_peak": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
+    "tree_measure_listeval": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     "tree_launch_count": (C.c_longlong, [C.c_void_p]),
     "tree_last_error": (C.c_char_p, [C.c_void_p]),
 }
@@ -265,6 +266,12 @@ class Tree:
         v = C.c_double(0)
         _check(self.h, load_library().tree_fp32_peak(self.h, C.byref(v)))
         return v.value
+
+    def measure_listeval(self):
+        """(walk-alone ms, evaluation-alone ms, max relative deviation from the fused pass): tree_measure_listeval."""
+        ms = (C.c_double * 2)(); mr = C.c_double(0)
+        _check(self.h, load_library().tree_measure_listeval(self.h, ms, C.byref(mr)))
+        return ms[0], ms[1], mr.value
 
     def launch_count(self) -> int:
         return int(load_library().tree_launch_count(self.h))

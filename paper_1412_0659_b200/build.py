@@ -21,6 +21,7 @@ COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas", "-
 UNITS = {
     "bh_build.cu": ["-fmad=false"],
     "bh_force.cu": [],
+    "bh_measure.cu": [],
     "bh_api.cu": [],
 }
 

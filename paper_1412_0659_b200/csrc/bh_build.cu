@@ -910,6 +910,7 @@ static int sort_passes(tree_ctx *t, int start, long long bound, const unsigned *
     cur ^= 1;
   }
   t->sorted = cur;
+  t->slot_of_valid = false;  // the passes used both key buffers, and the order is about to change
   return 0;
 }
 

@@ -138,6 +138,7 @@ struct tree_ctx {
   bool force_open = false;           // between tree_force_begin and tree_force_end
   bool step_open = false;            // between tree_leapfrog_begin and tree_leapfrog_end
   bool step_mid_done = false;        // sharded step: tree_leapfrog_mid has run (begin | barrier | mid | barrier | end)
+  bool slot_of_valid = false;        // the inverse of `order` (caller index -> slot) is in the spare key buffer
   bool split_valid = false;          // d_info->split holds the splitters of the current sorted order
   float step_dt = 0.f;
   float *open_acc = nullptr, *open_pot = nullptr;
