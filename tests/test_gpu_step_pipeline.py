@@ -130,3 +130,29 @@ def test_asynchronous_rebuild_reports_cell_overflow_and_freezes_the_state():
     t.leapfrog(1e-3)
     t.stats()            # no error left over
     t.close()
+
+
+def test_one_step_moves_few_particles_along_the_curve():
+    # What the step pipeline relies on (and what it cannot use): after one step of BASELINE configs[4]'s dt most
+    # particles keep their slot or move by a few slots, so the gather from the previous slot order is nearly sequential;
+    # but almost every KEY changes in its low digits, so no pass of an LSD radix sort can be skipped.
+    n, theta, eps, dt = 1 << 20, 0.4, 0.01, 0.0005
+    pos, vel, mass = milky_way(n, 1005)
+    t = Tree(device=0)
+    t.build(pos.cuda(), mass.cuda()); t.set_velocity(vel.cuda()); t.force(theta, eps)
+    t.leapfrog(dt)
+    order0, key0 = t.debug("order").astype(np.int64), t.debug("sorted_keys")
+    t.leapfrog(dt)
+    order1, key1 = t.debug("order").astype(np.int64), t.debug("sorted_keys")
+    slot0 = np.empty(n, np.int64); slot0[order0] = np.arange(n)
+    slot1 = np.empty(n, np.int64); slot1[order1] = np.arange(n)
+    disp = np.abs(slot1 - slot0)
+    k0 = np.empty(n, np.uint64); k0[order0] = key0
+    k1 = np.empty(n, np.uint64); k1[order1] = key1
+    changed = k0 != k1
+    low_byte_same = ((k0 ^ k1) & np.uint64(0xff)) == 0
+    print(f"\nslots: unchanged {np.mean(disp == 0):.3f}, moved <= 32 {np.mean(disp <= 32):.4f}, <= 2048 {np.mean(disp <= 2048):.5f}, "
+          f"max {disp.max()}; keys changed {changed.mean():.4f}, lowest byte unchanged {low_byte_same.mean():.4f}")
+    assert np.mean(disp <= 32) > 0.97          # the gather reads within a cache line or two of where it writes
+    assert changed.mean() > 0.9                # yet nearly every key differs: nothing for a radix pass to skip
+    t.close()
