@@ -256,6 +256,34 @@ int tree_fp32_peak(tree_ctx *t, double *tflops);
  * could reach.  Allocates and frees its own buffers; synchronises. */
 int tree_measure_listeval(tree_ctx *t, double *ms, double *max_rel);
 
+/* ---- an entry point that allocates nothing -----------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA stream capture, tight serving loops, harnesses that forbid
+ * it): the energy sums of tree_energy -- kinetic = sum 1/2 m v^2, potential = 1/2 sum m phi (the diagnostics of a
+ * leapfrog run), FP64 sums of FP32 inputs -- without a context and without any allocation.  The scratch
+ * tree_energy keeps in the context's cudaMalloc'ed buffers is here a fixed device array inside the library image
+ * (512.25 KiB; every GPU that loads libbhtree.so holds it until the process exits), hence the limit
+ *     N <= TREE_ENERGY_STATIC_MAX_N = 134,217,728 (32,768 partial sums of 4,096 particles each);
+ * a larger N returns TREE_ERR_ARG with a text that says so (use tree_energy there).
+ *   device       CUDA device the pointers live on (0..63); the caller's current device is restored
+ *   cuda_stream  a cudaStream_t (may be NULL); the call enqueues one 4-byte cudaMemsetAsync and one kernel on it and
+ *                returns without waiting; it calls no cudaMalloc, cudaFree or allocating library routine
+ *   mass         DEV float[N]
+ *   vel          DEV float[N][3] or NULL (kinetic = 0)
+ *   pot          DEV float[N] or NULL (potential = 0): phi_i as tree_force / tree_get_state return it, same order as mass
+ *   out          DEV double[2]: out[0] = kinetic, out[1] = potential, overwritten when the kernel has run
+ *   N = 0        set-up only (asks the driver once per device for the scratch address; every pointer may be NULL):
+ *                call it once before a stream capture begins, since the first call on a device may load the module
+ * The sums are added in a fixed order: the same inputs give the same bits on every call, and agree with tree_energy
+ * (atomic FP64 adds in arrival order) to rounding, ~1e-15 relative.
+ * All calls on a device share the one scratch array, which keeps the last call's contents; the call clears the word
+ * that must start at zero.  Calls that OVERLAP on the GPU (different streams, or two host threads on one device) race on
+ * it and give wrong sums: order them on one stream or with events.
+ * Errors: TREE_ERR_ARG / TREE_ERR_CUDA; text via tree_energy_static_error() (per host thread, "" after a success). */
+#define TREE_ENERGY_STATIC_MAX_N 134217728LL
+int tree_energy_static(int device, void *cuda_stream, const float *mass, const float *vel, const float *pot,
+                       long long N, double *out);
+const char *tree_energy_static_error(void);
+
 /* Number of kernels this library launched on the context since tree_create (for accounting). */
 long long tree_launch_count(const tree_ctx *t);
 

@@ -16,6 +16,8 @@ from .binding import (  # noqa: F401
     tree_force,
     tree_leapfrog,
     tree_destroy,
+    tree_energy_static,
+    ENERGY_STATIC_MAX_N,
     PHASES,
     FLOP_PP,
     FLOP_PC,

@@ -57,6 +57,8 @@ _SIGS = {
     "tree_shard_range": (C.c_int, [C.c_void_p] + [C.POINTER(C.c_longlong)] * 4),
     "tree_fp32_peak": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
     "tree_measure_listeval": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
+    "tree_energy_static": (C.c_int, [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_longlong, C.c_void_p]),
+    "tree_energy_static_error": (C.c_char_p, []),
     "tree_launch_count": (C.c_longlong, [C.c_void_p]),
     "tree_last_error": (C.c_char_p, [C.c_void_p]),
 }
@@ -135,6 +137,17 @@ def tree_leapfrog(h, dt: float):
 
 def tree_destroy(h):
     load_library().tree_destroy(h)
+
+
+ENERGY_STATIC_MAX_N = 134217728  # TREE_ENERGY_STATIC_MAX_N of include/tree.h
+
+
+def tree_energy_static(device: int, stream, mass, vel, pot, n: int, out):
+    """tree_energy_static: the energy sums without a context and without any allocation (static device scratch).
+    mass [n], vel [n,3] or None, pot [n] or None: float32 device tensors; out: float64 device tensor [2]; n = 0: set-up."""
+    rc = load_library().tree_energy_static(int(device), _ptr(stream), _ptr(mass), _ptr(vel), _ptr(pot), int(n), _ptr(out))
+    if rc != 0:
+        raise TreeError(rc, (load_library().tree_energy_static_error() or b"").decode())
 
 
 def effective_flops(n_pp: int, n_pc: int) -> int:

@@ -23,6 +23,7 @@ UNITS = {
     "bh_force.cu": [],
     "bh_measure.cu": [],
     "bh_api.cu": [],
+    "bh_noalloc.cu": [],
 }
 
 
