@@ -548,10 +548,28 @@ __global__ void __launch_bounds__(TREE_THREADS) tree_levels_kernel(const uint64_
   if (s < N) {
     int i = threadIdx.x + TREE_HALO;
     int L0 = cd[i] + 1;
-    int lmin = KEY_BITS, rmin = KEY_BITS, li = i, ri = i + 1, v = KEY_BITS;
-    for (int it = 0; it < leaf; ++it) {
-      int cl = min(lmin, (int)cd[li]), cr = min(rmin, (int)cd[ri]);
-      if (cl >= cr) { v = cl; lmin = cl; --li; } else { v = cr; rmin = cr; ++ri; }
+    int v = KEY_BITS;
+    if (leaf == 16) {
+      // the leaf-th largest of the two non-increasing sequences lm[j] = min(cd[i], .., cd[i-j+1]) and
+      // rm[j] = min(cd[i+1], .., cd[i+j]) is max over k of min(lm[k], rm[leaf-k]) (lm[0] = rm[0] = KEY_BITS):
+      // the value the merge walk below ends on, without its data-dependent selects
+      int rm[17];
+      rm[0] = KEY_BITS;
+#pragma unroll
+      for (int j = 1; j <= 16; ++j) rm[j] = min(rm[j - 1], (int)cd[i + j]);
+      v = rm[16];
+      int lm = KEY_BITS;
+#pragma unroll
+      for (int k = 1; k <= 16; ++k) {
+        lm = min(lm, (int)cd[i - k + 1]);
+        v = max(v, min(lm, rm[16 - k]));
+      }
+    } else {
+      int lmin = KEY_BITS, rmin = KEY_BITS, li = i, ri = i + 1;
+      for (int it = 0; it < leaf; ++it) {
+        int cl = min(lmin, (int)cd[li]), cr = min(rmin, (int)cd[ri]);
+        if (cl >= cr) { v = cl; lmin = cl; --li; } else { v = cr; rmin = cr; ++ri; }
+      }
     }
     int Ll = min(MAX_LEVEL, v + 1);
     lv[s] = (uint16_t)(L0 | (Ll << 5));
@@ -596,6 +614,7 @@ __global__ void __launch_bounds__(TREE_THREADS) tree_emit_kernel(const uint16_t 
   if (info->cells_overflow) return;
   __shared__ uint16_t lvs[TREE_THREADS + TREE_HALO + 1];
   __shared__ unsigned wbase[NLEVELS][NW];
+  __shared__ unsigned wleaf[NW + 1];  // per warp: which of its slots start a leaf; [NW]: the same for the halo
   const long long base = (long long)blockIdx.x * TREE_THREADS;
   const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const unsigned lt = (1u << lane) - 1u;
@@ -608,9 +627,29 @@ __global__ void __launch_bounds__(TREE_THREADS) tree_emit_kernel(const uint16_t 
   const bool valid = s < N;
   const int me = lvs[threadIdx.x];
   const int L0 = valid ? (me & 31) : 99, Ll = valid ? (me >> 5) : -1;
-  for (int l = 0; l < NLEVELS; ++l) {
+  // levels at which any slot of this warp starts a cell: [lo, hi] (warp-uniform); the other levels count zero
+  int lo = L0, hi = Ll;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+    hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+  }
+  if (lane < NLEVELS) wbase[lane][w] = 0;
+  __syncwarp();
+  for (int l = lo; l <= hi; ++l) {
     unsigned b = __ballot_sync(0xffffffffu, L0 <= l && l <= Ll);
     if (lane == 0) wbase[l][w] = __popc(b);
+  }
+  // a slot is the first of its leaf iff it starts a cell at all (L0 <= Ll): leaves tile the slots, so a leaf ends where
+  // the next one starts.  One ballot per warp (and one for the halo); slots past N count as starts: they terminate.
+  {
+    const unsigned f = __ballot_sync(0xffffffffu, !valid || L0 <= Ll);
+    if (lane == 0) wleaf[w] = f;
+    if (w == 0) {
+      const int h = lvs[TREE_THREADS + lane];
+      const unsigned fh = __ballot_sync(0xffffffffu, (h & 31) <= (h >> 5));
+      if (lane == 0) wleaf[NW] = fh;
+    }
   }
   __syncthreads();
   if (threadIdx.x < NLEVELS) {
@@ -618,12 +657,6 @@ __global__ void __launch_bounds__(TREE_THREADS) tree_emit_kernel(const uint16_t 
     for (int ww = 0; ww < NW; ++ww) { unsigned c = wbase[threadIdx.x][ww]; wbase[threadIdx.x][ww] = run; run += c; }
   }
   __syncthreads();
-  int lo = L0, hi = Ll;
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o));
-    hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o));
-  }
   if (hi < 0) return;  // whole warp past the end (warp-uniform)
   if (lo > hi) return;
   unsigned bcur = __ballot_sync(0xffffffffu, L0 <= lo && lo <= Ll);
@@ -633,15 +666,20 @@ __global__ void __launch_bounds__(TREE_THREADS) tree_emit_kernel(const uint16_t 
       unsigned id = wbase[l][w] + __popc(bcur & lt);
       unsigned child = wbase[l + 1][w] + __popc(bnext & lt);  // level 22 is empty: = n_cells
       unsigned cnt = 0;
-      if (l == Ll) {  // leaf: extent = up to the next slot that starts a cell at a level <= l
-        long long e = s + 1;
-        int i = threadIdx.x + 1;
-        while (e < N) {
-          int l0 = (i <= TREE_THREADS + TREE_HALO) ? (lvs[i] & 31) : (lv[e] & 31);
-          if (l0 <= l) break;
-          ++e; ++i;
+      if (l == Ll) {  // leaf: extent = up to the next slot that starts a leaf (or N)
+        const unsigned above = lane < 31 ? wleaf[w] >> (lane + 1) : 0u;
+        const unsigned next = wleaf[w + 1];
+        if (above) cnt = (unsigned)__ffs(above);
+        else if (next) cnt = (unsigned)(31 - lane + __ffs(next));
+        else {  // more than 32 slots: only a leaf of the deepest level can be that full (coincident keys)
+          long long e = s + (32 - lane) + 32;
+          while (e < N) {
+            const int m = lv[e];
+            if ((m & 31) <= (m >> 5)) break;
+            ++e;
+          }
+          cnt = (unsigned)(e - s);
         }
-        cnt = (unsigned)(e - s);
       }
       c_level[id] = (uint8_t)l;
       c_first[id] = (uint32_t)s;
