@@ -363,7 +363,7 @@ int tree_create(tree_ctx **out, int device, void *cuda_stream, int leaf_size, in
       cudaMallocHost((void **)&t->h_info, sizeof(DevInfo)) != cudaSuccess ||
       cudaMallocHost((void **)&t->h_async, sizeof(DevInfo)) != cudaSuccess ||
       cudaEventCreateWithFlags(&t->ev_async, cudaEventDisableTiming) != cudaSuccess ||
-      cudaMalloc((void **)&t->d_hlut, 24 * 8) != cudaSuccess) {
+      cudaMalloc((void **)&t->d_hlut, HLUT3_OFFSET + HLUT3_ENTRIES * sizeof(uint16_t)) != cudaSuccess) {
     cudaGetLastError();
     tree_destroy(t);
     return TREE_ERR_NOMEM;
@@ -374,6 +374,11 @@ int tree_create(tree_ctx **out, int device, void *cuda_stream, int leaf_size, in
   uint8_t lut[24 * 8];
   build_hilbert_lut(lut);
   cudaMemcpy(t->d_hlut, lut, sizeof(lut), cudaMemcpyHostToDevice);
+  {
+    std::vector<uint16_t> lut3(HLUT3_ENTRIES);
+    build_hilbert_lut3(lut, lut3.data());
+    cudaMemcpy(t->d_hlut + HLUT3_OFFSET, lut3.data(), HLUT3_ENTRIES * sizeof(uint16_t), cudaMemcpyHostToDevice);
+  }
   for (int i = 0; i < EV_COUNT; ++i) t->ev_valid[i] = cudaEventCreate(&t->ev[i]) == cudaSuccess;
   *out = t;
   return TREE_OK;

@@ -151,48 +151,32 @@ __global__ void grid_kernel(DevInfo *info) {
 
 // a2: Peano-Hilbert key by a 24-state x 8-octant table generated on the host from the
 // Gray-code/rotation recurrence (T3). Table entry = digit | next_state << 3.
-// The kernel walks TWO levels per table step: a 24 x 64 table (digit pair | next_state << 6, built per block from the
-// 8-octant table) over the Morton-interleaved grid coordinates, so a key costs 10 dependent shared-memory look-ups
-// + 1 instead of 21 (the kernel is bound by that chain, not by HBM).
-__device__ __forceinline__ uint64_t spread3(unsigned v) {  // bit i of the 21-bit v -> bit 3 i
-  uint64_t x = v & 0x1fffffu;
-  x = (x | (x << 32)) & 0x001f00000000ffffull;
-  x = (x | (x << 16)) & 0x001f0000ff0000ffull;
-  x = (x | (x << 8)) & 0x100f00f00f00f00full;
-  x = (x | (x << 4)) & 0x10c30c30c30c30c3ull;
-  x = (x | (x << 2)) & 0x1249249249249249ull;
-  return x;
-}
-
+// The kernel walks THREE levels per table step: a 24 x 512 table (three digits | next_state << 9; built once on the
+// host from the 8-octant table, build_hilbert_lut3; every block copies its 24 KB into shared memory) indexed by state
+// and by 3 bits of each grid coordinate, z | y | x, so the coordinates are never interleaved: a key costs 7 dependent
+// shared-memory look-ups of ~12 instructions each (round 2 (a): 10 + 1 look-ups over Morton-interleaved coordinates,
+// 205 instructions per key, of which the interleaving took 120; the kernel is bound by instruction issue, not by HBM).
 __global__ void __launch_bounds__(256) keys_kernel(const float4 *__restrict__ posm, long long N,
-                                                   const DevInfo *__restrict__ info, const uint8_t *__restrict__ lut_g,
+                                                   const DevInfo *__restrict__ info, const uint16_t *__restrict__ lut3_g,
                                                    uint64_t *__restrict__ key, uint32_t *__restrict__ idx) {
-  __shared__ uint8_t lut[24 * 8];
-  __shared__ uint16_t lut2[24 * 64];
-  if (threadIdx.x < 24 * 8) lut[threadIdx.x] = lut_g[threadIdx.x];
-  __syncthreads();
-  for (int e = threadIdx.x; e < 24 * 64; e += blockDim.x) {
-    const unsigned st = e >> 6, hi = (e >> 3) & 7u, lo = e & 7u;
-    const unsigned v1 = lut[st * 8 + hi], v2 = lut[(v1 >> 3) * 8 + lo];
-    lut2[e] = (uint16_t)((((v1 & 7u) << 3) | (v2 & 7u)) | ((v2 >> 3) << 6));
-  }
+  __shared__ __align__(16) uint16_t lut3[HLUT3_ENTRIES];
+  for (int e = threadIdx.x; e < HLUT3_ENTRIES / 8; e += blockDim.x)
+    reinterpret_cast<uint4 *>(lut3)[e] = reinterpret_cast<const uint4 *>(lut3_g)[e];
   __syncthreads();
   const float ox = info->origin[0], oy = info->origin[1], oz = info->origin[2], inv = info->inv;
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
     float4 p = posm[i];
-    unsigned ix = grid_coord(p.x, ox, inv), iy = grid_coord(p.y, oy, inv), iz = grid_coord(p.z, oz, inv);
-    // one octant digit per level, bits z y x, most significant level first
-    const uint64_t m = spread3(ix) | (spread3(iy) << 1) | (spread3(iz) << 2);
-    uint64_t h = 0;
-    unsigned st = 0;
+    const unsigned ix = grid_coord(p.x, ox, inv), iy = grid_coord(p.y, oy, inv) << 3, iz = grid_coord(p.z, oz, inv) << 6;
+    unsigned st = 0, h[3] = {0u, 0u, 0u};  // 27 + 27 + 9 bits of the key
 #pragma unroll
-    for (int b = KEY_BITS - 2; b >= 1; b -= 2) {  // levels (b+1, b): 20..1 in 10 steps
-      const unsigned v = lut2[st * 64 + ((unsigned)(m >> (3 * b)) & 63u)];
-      h = (h << 6) | (v & 63u);
-      st = v >> 6;
+    for (int step = 0; step < 7; ++step) {  // levels (b+2, b+1, b), b = 18, 15, .., 0
+      const int b = 18 - 3 * step;
+      const unsigned t = ((ix >> b) & 7u) | ((iy >> b) & 0x38u) | ((iz >> b) & 0x1c0u);
+      const unsigned v = lut3[st * 512 + t];
+      h[step / 3] = (h[step / 3] << 9) | (v & 511u);
+      st = v >> 9;
     }
-    h = (h << 3) | (lut[st * 8 + ((unsigned)m & 7u)] & 7u);  // level 0
-    key[i] = h;
+    key[i] = ((uint64_t)h[0] << 36) | ((uint64_t)h[1] << 9) | (uint64_t)h[2];
     if (idx) idx[i] = (uint32_t)i;
   }
 }
@@ -755,6 +739,7 @@ __device__ __forceinline__ void moments_cell(int c, int level, bool leaves, cons
   float cx, cy, cz;
   if (!(lk.y & LEAF_FLAG)) {
     const unsigned f = lk.x, n = lk.y;
+#pragma unroll 4
     for (unsigned p = f; p < f + n; ++p) {
       float4 q = spos[p];
       double m = (double)q.w;
@@ -764,6 +749,7 @@ __device__ __forceinline__ void moments_cell(int c, int level, bool leaves, cons
       s2 = __dadd_rn(s2, __dmul_rn(m, (double)q.z));
     }
     cx = (float)(s0 / M); cy = (float)(s1 / M); cz = (float)(s2 / M);
+#pragma unroll 4
     for (unsigned p = f; p < f + n; ++p) {
       float4 q = spos[p];
       double m = (double)q.w;
@@ -922,7 +908,8 @@ int run_keys(tree_ctx *t, const float4 *xyzm) {
   grid_kernel<<<1, 32, 0, t->stream>>>(t->d_info);
   BH_LAUNCH_CHECK("grid");
   // the sort's first pass takes the identity as payload: no index array is written here
-  keys_kernel<<<grid_for(t, t->N, 256, 8), 256, 0, t->stream>>>(xyzm, t->N, t->d_info, t->d_hlut, t->b.key[0], nullptr);
+  keys_kernel<<<grid_for(t, t->N, 256, 8), 256, 0, t->stream>>>(
+      xyzm, t->N, t->d_info, reinterpret_cast<const uint16_t *>(t->d_hlut + HLUT3_OFFSET), t->b.key[0], nullptr);
   BH_LAUNCH_CHECK("keys");
   return 0;
 }
@@ -1199,6 +1186,19 @@ void build_hilbert_lut(uint8_t out[24 * 8]) {
         unsigned d2 = (d + dir + 1u) % 3u;
         out[(e * 3 + d) * 8 + l] = (uint8_t)(w | ((e2 * 3 + d2) << 3));
       }
+}
+
+// Three levels per look-up (keys_kernel): entry [state][z3 y3 x3] = three digits, most significant first, | next state << 9.
+void build_hilbert_lut3(const uint8_t lut[24 * 8], uint16_t out[HLUT3_ENTRIES]) {
+  for (unsigned e = 0; e < (unsigned)HLUT3_ENTRIES; ++e) {
+    const unsigned st = e >> 9, zt = (e >> 6) & 7u, yt = (e >> 3) & 7u, xt = e & 7u;
+    // octant digit of a level = bits z y x of that level
+    const unsigned o1 = ((zt >> 2) & 1u) << 2 | ((yt >> 2) & 1u) << 1 | ((xt >> 2) & 1u);
+    const unsigned o2 = ((zt >> 1) & 1u) << 2 | ((yt >> 1) & 1u) << 1 | ((xt >> 1) & 1u);
+    const unsigned o3 = (zt & 1u) << 2 | (yt & 1u) << 1 | (xt & 1u);
+    const unsigned v1 = lut[st * 8 + o1], v2 = lut[(v1 >> 3) * 8 + o2], v3 = lut[(v2 >> 3) * 8 + o3];
+    out[e] = (uint16_t)(((v1 & 7u) << 6) | ((v2 & 7u) << 3) | (v3 & 7u) | ((v3 >> 3) << 9));
+  }
 }
 
 }  // namespace bh

@@ -14,6 +14,8 @@ constexpr int KEY_BITS = 21;      // bits per dimension -> 63-bit Peano-Hilbert 
 constexpr int MAX_LEVEL = KEY_BITS;
 constexpr int NLEVELS = MAX_LEVEL + 2;  // levels 0..21 exist; level 22 is an always-empty sentinel
 constexpr uint32_t LEAF_FLAG = 0x80000000u;
+constexpr int HLUT3_ENTRIES = 24 * 512;  // Hilbert table over three levels per look-up (keys_kernel), uint16 each
+constexpr int HLUT3_OFFSET = 256;        // its byte offset inside tree_ctx::d_hlut (the 24 x 8 table comes first)
 
 // Device-resident scalars of one build.
 struct DevInfo {
@@ -148,7 +150,7 @@ struct tree_ctx {
   bh::Buffers b;
   bh::DevInfo *d_info = nullptr;
   bh::DevInfo *h_info = nullptr;     // pinned
-  uint8_t *d_hlut = nullptr;         // Hilbert state table (device copy)
+  uint8_t *d_hlut = nullptr;         // Hilbert state tables (device copy): 24 x 8 bytes | at HLUT3_OFFSET: 24 x 512 uint16
   cudaEvent_t ev[24];
   bool ev_valid[24];
   double ms[TREE_NPHASE];
@@ -205,6 +207,7 @@ int run_direct(tree_ctx *t, const long long *idx, long long n, float eps, double
 int run_fp32_peak(tree_ctx *t, double *tflops);
 int ensure_cells(tree_ctx *t, long long n_cells);
 void build_hilbert_lut(uint8_t out[24 * 8]);
+void build_hilbert_lut3(const uint8_t lut[24 * 8], uint16_t out[HLUT3_ENTRIES]);
 int device_excl_scan(tree_ctx *t, uint32_t *a, long long n, uint32_t *total_out);
 
 }  // namespace bh
