@@ -220,7 +220,8 @@ static int build_from_posm(tree_ctx *t) {
 // writes into the result buffers of parity (pass & 1); the other parity still holds the previous pass
 // (its per-group counts schedule this one, and a sharded peer may still be reading it).
 // kick_hdt != 0 (tree_leapfrog on one context): the walk's epilogue also applies the step's closing half kick.
-static int force_begin_impl(tree_ctx *t, float theta, float eps, float kick_hdt) {
+// acc / pot (tree_force on one context): the walk's epilogue writes the results to the caller's arrays as well.
+static int force_begin_impl(tree_ctx *t, float theta, float eps, float kick_hdt, float *acc = nullptr, float *pot = nullptr) {
   if (t->shard_world > 1)
     for (int r = 0; r < t->shard_world; ++r)
       if (r != t->shard_rank && !t->peer_base[r]) return set_err(t, TREE_ERR_ORDER, "sharded context: a peer is not attached");
@@ -239,7 +240,7 @@ static int force_begin_impl(tree_ctx *t, float theta, float eps, float kick_hdt)
     BH_TRY(run_box_check(t));
     t->reuse_mode = 2;
   }
-  const int wrc = run_walk(t, eps, kick_hdt);  // records EV_OPEN before and EV_WALK after the walk kernel
+  const int wrc = run_walk(t, eps, kick_hdt, acc, pot);  // records EV_OPEN before and EV_WALK after the walk kernel
   t->reuse_mode = mode_in;
   if (wrc) return wrc;
   BH_CUDA(cudaMemcpyAsync(t->b.gbox_prev, t->b.gbox, (size_t)t->n_groups * 6 * sizeof(float), cudaMemcpyDeviceToDevice, t->stream));
@@ -261,8 +262,12 @@ static int force_end_impl(tree_ctx *t, float *acc, float *pot) {
 }
 
 static int force_impl(tree_ctx *t, float theta, float eps, float *acc, float *pot) {
-  BH_TRY(force_begin_impl(t, theta, eps, 0.0f));
-  return force_end_impl(t, acc, pot);
+  if (t->shard_world > 1) {
+    BH_TRY(force_begin_impl(t, theta, eps, 0.0f));
+    return force_end_impl(t, acc, pot);
+  }
+  BH_TRY(force_begin_impl(t, theta, eps, 0.0f, acc, pot));  // a11 fused into the walk's epilogue
+  return force_end_impl(t, nullptr, nullptr);
 }
 
 // One step without a host round trip: the state stays in slot order, the cell arrays

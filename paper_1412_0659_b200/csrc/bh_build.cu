@@ -372,11 +372,16 @@ __global__ void __launch_bounds__(OS_THREADS, OS_MINB) sort_onesweep_kernel(cons
     const bool valid = p < N;
     const unsigned d = (unsigned)(key[k] >> shift) & 255u;
     const unsigned act = __ballot_sync(0xffffffffu, valid);
-    unsigned peers = 0, c0 = 0;
-    if (valid) {
-      peers = __match_any_sync(act, d);
-      c0 = sm.wc[w][d];
+    // lanes with the same digit: one ballot per digit bit (MATCH.ANY takes one round per distinct value in the warp: with
+    // 8-bit digits of well-mixed keys that is ~28 rounds, and the warps queued behind it)
+    unsigned peers = act, c0 = 0;
+#pragma unroll
+    for (int b = 0; b < 8; ++b) {
+      const bool bit = (d >> b) & 1u;
+      const unsigned v = __ballot_sync(0xffffffffu, bit);
+      peers &= bit ? v : ~v;
     }
+    if (valid) c0 = sm.wc[w][d];
     __syncwarp();
     if (valid && lane == 31 - __clz(peers)) sm.wc[w][d] = c0 + __popc(peers);
     __syncwarp();

@@ -194,7 +194,8 @@ int run_permute_step(tree_ctx *t);    // tree_leapfrog: spos, svel, order -> the
 int run_tree(tree_ctx *t, bool async);  // octree construction; !async: synchronises once and sizes the cell arrays
 int run_groups_moments(tree_ctx *t);
 int run_opening(tree_ctx *t, float theta);
-int run_walk(tree_ctx *t, float eps, float kick_hdt);  // kick_hdt != 0: v += a * kick_hdt in the walk's epilogue
+// kick_hdt != 0: v += a * kick_hdt in the walk's epilogue; out_acc / out_pot (one context): results also to the caller's arrays there
+int run_walk(tree_ctx *t, float eps, float kick_hdt, float *out_acc, float *out_pot);
 int run_box_check(tree_ctx *t);  // device-side: are the group boxes where the previous force pass saw them?
 void shard_views(const tree_ctx *t, void *base, int parity, float4 **sacc, uint2 **gcount);
 int run_scatter_out(tree_ctx *t, float *acc, float *pot);  // results to the caller's arrays (caller order)

@@ -77,6 +77,8 @@ struct WalkParams {
   float4 *svel;            // tree_leapfrog on one context: the step's closing half kick, v += a * kick_hdt, is applied here in
   float kick_hdt;          // the epilogue (nullptr otherwise: a sharded pass kicks after its barrier)
   int reuse_mode;          // 0: costs from the counting walk; 1: from the previous pass's counts; 2: info->reuse_costs decides
+  const uint32_t *order;   // tree_force with caller arrays on one context: the epilogue also writes each result to the caller's
+  float *out_acc, *out_pot;  // arrays at order[slot] (a11 fused: no separate pass); order = nullptr otherwise
 };
 
 constexpr unsigned TASK_GROUP_BITS = 26;

@@ -76,6 +76,14 @@ __device__ __forceinline__ void flush_queues(WarpSmem &ws, int lane, WalkState<T
 }
 
 // a12, second half kick of a step, fused into the walk's epilogue: v = fma(a, dt/2, v) (T12)
+// a11 fused into the epilogue: the result of `slot` to the caller's arrays (caller order).  12- and 4-byte random writes,
+// spread over the whole walk (as a pass of their own they ran at a third of the gather's speed).
+__device__ __forceinline__ void emit_caller(const WalkParams &P, unsigned slot, const float4 r) {
+  const size_t ci = P.order[slot];
+  if (P.out_acc) { float *a = P.out_acc + 3 * ci; a[0] = r.x; a[1] = r.y; a[2] = r.z; }
+  if (P.out_pot) P.out_pot[ci] = r.w;
+}
+
 __device__ __forceinline__ void kick_slot(float4 *v, const float4 a, float hdt) {
   float4 u = *v;
   u.x = __fmaf_rn(a.x, hdt, u.x); u.y = __fmaf_rn(a.y, hdt, u.y); u.z = __fmaf_rn(a.z, hdt, u.z);
@@ -312,6 +320,7 @@ __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, con
         P.sacc[g0 + j] = res[t];
         for (int q = 0; q < P.n_peers; ++q) P.peer_sacc[q][g0 + j] = res[t];
         if (P.svel) kick_slot(P.svel + g0 + j, res[t], P.kick_hdt);
+        if (P.order) emit_caller(P, g0 + j, res[t]);
       }
     }
   } else {
@@ -344,6 +353,7 @@ __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, con
           P.sacc[g0 + j] = sum;
           for (int q = 0; q < P.n_peers; ++q) P.peer_sacc[q][g0 + j] = sum;
           if (P.svel) kick_slot(P.svel + g0 + j, sum, P.kick_hdt);
+          if (P.order) emit_caller(P, g0 + j, sum);
         }
       }
       if (P.n_peers > 0 && lane == 0) {  // every part's counts were added before it signalled gdone
@@ -972,9 +982,12 @@ static int launch_walk(tree_ctx *t, const WalkParams &P, unsigned grid) {
   return 0;
 }
 
-int run_walk(tree_ctx *t, float eps, float kick_hdt) {
+int run_walk(tree_ctx *t, float eps, float kick_hdt, float *out_acc, float *out_pot) {
   WalkParams P;
   P.reuse_mode = t->reuse_mode;
+  const bool fuse_out = (out_acc || out_pot) && t->shard_world <= 1;  // sharded: most results arrive from peers (force_end gathers)
+  P.order = fuse_out ? t->b.order : nullptr;
+  P.out_acc = out_acc; P.out_pot = out_pot;
   const bool fuse_kick = kick_hdt != 0.0f && t->shard_world <= 1;
   P.svel = fuse_kick ? t->b.svel : nullptr;
   P.kick_hdt = kick_hdt;
