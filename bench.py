@@ -541,7 +541,7 @@ def main():
                     help="N > 1: N independent replicas (weak scaling) instead of ONE problem over all GPUs")
     ap.add_argument("--sharded", action="store_true", help="(default for N > 1; kept for older command lines)")
     ap.add_argument("--table", default="", help="print a measurement table instead (bench_tables.py): kernels | "
-                                                "shard-scaling | mac-sweep | sass-histogram | walk-eval-split")
+                                                "shard-scaling | shard-weak | mac-sweep | sass-histogram | walk-eval-split")
     ap.add_argument("--from-ncu", default="", help="--table kernels: the ncu CSV to read")
     ap.add_argument("--from-sass", default="", help="--table sass-histogram: the cuobjdump -sass listing to read")
     ap.add_argument("--worlds", default="1,2,4,8", help="--table shard-scaling: world sizes")

@@ -4,6 +4,8 @@
                  (``--from-ncu FILE``: a ``--metrics gpu__time_duration.sum,dram__bytes_read.sum,dram__bytes_write.sum``
                  pass), against the measured copy bandwidth of MEASURED_PEAKS.json and the algorithmic bytes of DESIGN.md §5
   shard-scaling  per-rank cost of the sharded force pass measured on ONE GPU with W contexts
+  shard-weak     the same with N = 13 M particles x W (the paper's weak-scaling set-up, Table II): per-rank
+                 phase times in the rows of Table II; ``--n`` overrides the particles per rank
   sass-histogram instruction classes of the whole kernel and of every innermost loop of a ``cuobjdump -sass`` listing
                  (``--from-sass FILE``)
   walk-eval-split the fused kernel against its walk alone and its evaluation alone (tree_measure_listeval); ``--worlds``
@@ -126,7 +128,9 @@ def _measure_shards(cfg, world: int, steps: int):
             # barrier, which on one GPU includes the other contexts' kernels, so it is taken from the W = 1 run
             own = ms["total"] - ms["integrate"] - ms["unpermute"]
             per_rank.append(dict(total=own, walk=ms["walk"], sched=ms["sched"], rest=own - ms["walk"] - ms["sched"],
-                                 groups=g_hi - g_lo, flops=23 * pp + 65 * pc))
+                                 groups=g_hi - g_lo, flops=23 * pp + 65 * pc, pp=pp, pc=pc, sort=ms["sort"],
+                                 tree=ms["build"], moments=ms["moments"],
+                                 other=own - ms["walk"] - ms["sort"] - ms["build"] - ms["moments"]))
         rows.append(per_rank)
     for t in trees:
         t.close()
@@ -171,6 +175,46 @@ def table_shard_scaling(config: int, worlds, steps: int):
         walks = [r["walk"] for r in avg]
         print(f"| {w} | {slow['total']:.3f} | {slow['walk']:.3f} | {slow['rest']:.3f} | {slow['sched']:.3f} | "
               f"{min(walks):.3f} .. {max(walks):.3f} | {share:.3f} | {base / slow['total']:.2f} |", flush=True)
+
+
+def table_shard_weak(n_per_rank: int, worlds, steps: int):
+    """Weak scaling in the paper's set-up (13 million particles per GPU, Milky-Way model, theta = 0.4),
+    emulated on one GPU like table_shard_scaling: W contexts share the steps of ONE problem of N = n_per_rank x W
+    particles; the rows are those of the paper's Table II (L240-258).  NVLink stores and barriers are not in it."""
+    import torch
+    from nbody_inputs import milky_way
+    from paper_1412_0659_b200 import Tree
+    theta, eps, dt = 0.4, 0.01, 5e-4
+    print(f"# weak scaling, {n_per_rank:,} particles per rank (PAPER.md L200), Milky-Way-shaped model, theta {theta}, eps {eps}, "
+          f"dt {dt}: per-rank times of the slowest rank on one GPU, {steps} leapfrog steps averaged")
+    print("| ranks | N total | sorting ms | tree construction ms | tree properties ms | compute gravity (walk + force) ms | "
+          "other (kick/drift, keys, gather, opening, task list) ms | total ms | p-p / particle | p-c / particle | "
+          "GPU TFLOP/s per rank (walk) | application TFLOP/s per rank | step(1) / step(W) |")
+    print("|---|---|---|---|---|---|---|---|---|---|---|---|---|")
+    base = None
+    for w in worlds:
+        n = n_per_rank * w
+        cfg = dict(name=f"mw_weak_{w}", model="milky_way", n=n, seed=1100 + w, theta=theta, eps=eps, dt=dt)
+        t = Tree(device=0)  # the integrate phase of a single context at this N, measured alone (see table_shard_scaling)
+        pos, vel, mass = milky_way(n, cfg["seed"], device="cuda")
+        t.build(pos, mass); t.set_velocity(vel); t.force(theta, eps)
+        t.leapfrog(dt); t.leapfrog(dt)
+        integ = t.stats()[0]["integrate"] * 1.5
+        t.close()
+        del pos, vel, mass
+        torch.cuda.empty_cache()
+        avg = _measure_shards(cfg, w, steps)
+        for r in avg:
+            r["total"] += integ; r["other"] += integ
+        slow = max(avg, key=lambda r: r["total"])
+        if base is None:
+            base = slow["total"]
+        pp = sum(r["pp"] for r in avg) / n
+        pc = sum(r["pc"] for r in avg) / n
+        print(f"| {w} | {n:,} | {slow['sort']:.2f} | {slow['tree']:.2f} | {slow['moments']:.2f} | {slow['walk']:.2f} | "
+              f"{slow['other']:.2f} | {slow['total']:.2f} | {pp:.0f} | {pc:.0f} | {slow['flops'] / slow['walk'] / 1e9:.1f} | "
+              f"{slow['flops'] / slow['total'] / 1e9:.1f} | {base / slow['total']:.3f} |", flush=True)
+        torch.cuda.empty_cache()
 
 
 def table_mac_sweep(config: int):
@@ -284,6 +328,8 @@ def run(args) -> int:
         table_kernels(args.from_ncu, args.n or CONFIGS[args.config]["n"])
     elif args.table == "shard-scaling":
         table_shard_scaling(args.config, [int(x) for x in args.worlds.split(",")], args.steps)
+    elif args.table == "shard-weak":
+        table_shard_weak(args.n or 13_000_000, [int(x) for x in args.worlds.split(",")], args.steps)
     elif args.table == "mac-sweep":
         table_mac_sweep(args.config)
     elif args.table == "walk-eval-split":

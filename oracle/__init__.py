@@ -61,6 +61,7 @@ def lib():
         L.orc_tree_get_ropen2.argtypes = [C.c_void_p] * 2
         L.orc_tree_abs_sum.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.c_int64, C.c_void_p]
         L.orc_tree_set_mac.argtypes = [C.c_void_p, C.c_int]
+        L.orc_tree_set_mac_relative.argtypes = [C.c_void_p, C.c_float, C.c_void_p]
         L.orc_tree_get_tight.argtypes = [C.c_void_p] * 2
         L.orc_tree_walk_lists.argtypes = [C.c_void_p, C.c_float, C.c_int64, C.c_void_p, C.POINTER(C.c_int64),
                                           C.c_void_p, C.POINTER(C.c_int64)]
@@ -213,6 +214,14 @@ class Tree:
         """Acceptance criterion of later force / walk_lists calls: 0 = canonical (S5), 1 = "bmax" (option, NEXT-2)."""
         if lib().orc_tree_set_mac(self._h, int(kind)):
             raise ValueError("unknown criterion")
+
+    def set_mac_relative(self, alpha: float, amag):
+        """Option "relative" (NEXT-2): group g accepts cell c iff the canonical criterion at the force call's theta does
+        (the floor) and D^5 alpha a_g > M l^3, a_g = min of ``amag`` (float32 [N], caller order: |a| of every particle,
+        an input) over the group's particles.  set_mac(0) returns to the canonical criterion."""
+        amag = _f32(amag, (self.n,))
+        if lib().orc_tree_set_mac_relative(self._h, float(alpha), _p(amag)):
+            raise ValueError("bad alpha or amag")
 
     def tight(self):
         """float32 [n_cells,7]: tight bounding box lo, hi of each cell's particles and its bounding radius b."""

@@ -22,6 +22,15 @@
 // radius: accept iff D > b / theta, b = distance from the cell's centre of mass to the farthest corner of the TIGHT
 // bounding box of its particles), selected with orc_tree_set_mac; the canonical criterion (S5) is the default and its
 // arithmetic is untouched.  Pins: b bounds the distance of every particle of the cell from its c.o.m.; boxes nest.
+// Option "relative" (SURVEY.md §8(f) NEXT-2 "per-group theta chosen to hit a force-error target", not in PAPER.md): an
+// error-targeted criterion per group, selected with orc_tree_set_mac_relative(alpha, |a| per particle).  Group g accepts
+// cell c iff the canonical criterion (S5, with the theta of the force call as a floor) accepts it AND
+//     D^5 alpha a_g > M l^3,    a_g = the smallest given |a| among the group's particles,
+// i.e. the first multipole term the evaluation leaves out, ~ M l^3 / D^5, stays below alpha times the group's own
+// acceleration (the relative criterion of the tree-code literature, with the power that fits a quadrupole expansion).
+// FP32, in this order: gscale = alpha * a_g; lhs = sqrt(D2) * D2 * D2 * gscale; q = M * l * l * l; accept iff lhs > q.
+// Pins: alpha = 0 is direct summation; a huge alpha leaves the canonical lists; lists partition; monotone in alpha; the
+// group's scale is the MINIMUM over its particles; lower cost than the canonical criterion at the same median error.
 // Parity unpinned: the MAC formula itself (S5: PAPER.md L31 names an opening angle and defers to its ref. [9]) and the
 // rounding order of T7 (S13: PAPER.md is silent on the precision of the moments) -- recorded readings, pinned only
 // through their consequences (tree-vs-direct error, partition invariant, theta -> 0).
@@ -92,7 +101,8 @@ struct Tree {
   std::vector<Cell> cells;             // BFS order (T5)
   std::vector<float> cM, cx, cy, cz, qxx, qyy, qzz, qxy, qxz, qyz, delta;  // T7, FP32 stored
   std::vector<float> tlo, thi, brad;   // option "bmax": tight box [n_cells][3] x 2 and bounding radius b about the c.o.m.
-  int mac = 0;                         // 0: S5 (l / theta + delta), 1: bmax (b / theta)
+  int mac = 0;                         // 0: S5 (l / theta + delta), 1: bmax (b / theta), 2: relative (S5 as floor + D^5 alpha a_g > M l^3)
+  std::vector<float> gscale;           // option "relative": alpha * min |a| of each group's particles
   std::vector<float> gmin, gmax;       // T8: [n_groups][3]
   std::vector<float> ropen2;           // T9, for the last theta
   std::vector<uint32_t> npp, npc;      // T10 per group
@@ -315,6 +325,17 @@ inline bool mac_accept(const Tree &t, int64_t g, int32_t c) {
     u[d] = std::max(0.0f, std::max(a, b));
   }
   float D2 = std::fmaf(u[2], u[2], std::fmaf(u[1], u[1], u[0] * u[0]));
+  if (t.mac == 2) {  // option "relative": the canonical criterion as a floor, then D^5 alpha a_g > M l^3
+    if (!(D2 > t.ropen2[c])) return false;
+    float lc = std::ldexp(1.0f, t.k - t.cells[c].level);
+    float lhs = std::sqrt(D2) * D2;
+    lhs = lhs * D2;
+    lhs = lhs * t.gscale[g];
+    float q = t.cM[c] * lc;
+    q = q * lc;
+    q = q * lc;
+    return lhs > q;
+  }
   return D2 > t.ropen2[c];
 }
 
@@ -532,6 +553,22 @@ void orc_tree_get_counts(void *h, uint32_t *npp, uint32_t *npc) {
   Tree *t = (Tree *)h;
   std::memcpy(npp, t->npp.data(), t->npp.size() * sizeof(uint32_t));
   std::memcpy(npc, t->npc.data(), t->npc.size() * sizeof(uint32_t));
+}
+// option "relative": amag = |a| of every particle (caller order, FP32: an input, e.g. of an earlier force pass);
+// the scale of group g is alpha * min over its particles (one FP32 multiplication)
+int orc_tree_set_mac_relative(void *h, float alpha, const float *amag) {
+  Tree *t = (Tree *)h;
+  if (!(alpha >= 0.0f) || !amag) return -1;
+  const int64_t ng = t->n_groups();
+  t->gscale.assign(ng, 0.0f);
+  for (int64_t g = 0; g < ng; ++g) {
+    const int64_t a0 = g * t->group_size, b0 = std::min<int64_t>(a0 + t->group_size, t->N);
+    float m = amag[t->order[a0]];
+    for (int64_t s = a0 + 1; s < b0; ++s) m = std::min(m, amag[t->order[s]]);
+    t->gscale[g] = alpha * m;
+  }
+  t->mac = 2;
+  return 0;
 }
 // option "bmax": kind 0 = canonical (S5), 1 = bmax
 int orc_tree_set_mac(void *h, int kind) {
