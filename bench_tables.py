@@ -254,6 +254,23 @@ def table_mac_sweep(config: int):
                       f"{np.median(err):.2e} | {np.percentile(err, 99):.2e} | {err.max():.2e} | "
                       f"{(23 * pp + 65 * pc) / min(ws) / 1e9:.1f} |", flush=True)
             t.close()
+    # the error-targeted criterion (tree_set_mac_relative): theta = 1 as the geometric floor, alpha swept; every pass is
+    # scaled by |a| of the canonical theta = 0.4 pass (handed in, so that the rows differ in alpha only)
+    t = Tree(device=0)
+    t.build(pos, mass)
+    t.force(0.4, eps, acc, pot)
+    amag = acc.norm(dim=1).contiguous()
+    for alpha in (1e-4, 2e-4, 3e-4, 6e-4, 1e-3, 3e-3):
+        ws = []
+        for _ in range(3):
+            t.set_mac_relative(alpha, amag)
+            t.force(1.0, eps, acc, pot); ms, pp, pc = t.stats(); ws.append(ms["walk"] + ms["sched"])
+        a = acc[idx].double().cpu().numpy()
+        err = np.linalg.norm(a - adn, axis=1) / np.linalg.norm(adn, axis=1)
+        print(f"| relative alpha={alpha:g} | 64 | 16 | 1.0 (floor) | {pp / n:.0f} | {pc / n:.0f} | {min(ws):.2f} | "
+              f"{np.median(err):.2e} | {np.percentile(err, 99):.2e} | {err.max():.2e} | "
+              f"{(23 * pp + 65 * pc) / min(ws) / 1e9:.1f} |", flush=True)
+    t.close()
 
 
 def table_sass_histogram(path: str):

@@ -113,6 +113,24 @@ int tree_destroy(tree_ctx *t);
 #define TREE_MAC_BMAX 1
 int tree_set_mac(tree_ctx *t, int kind);
 
+/* Error-targeted acceptance per group (SURVEY.md 8(f) NEXT-2 "per-group theta chosen to hit a force-error target"; not in
+ * PAPER.md, which fixes theta = 0.4 "for accuracy", L133).  On top of TREE_MAC_GEOMETRIC -- which stays necessary, with the
+ * theta of tree_force as a floor (theta = 1 is a sensible one) -- group g accepts cell c only if
+ *     D^5 alpha a_g > M l^3,
+ * a_g = the smallest |a| among the group's particles in the previous force pass on this context: the first multipole
+ * term the evaluation leaves out, ~ M l^3 / D^5, stays below alpha times the group's own acceleration.  FP32, one IEEE
+ * operation each: gscale = alpha * a_g; sqrt(D2) * D2 * D2 * gscale > M * l * l * l.
+ *   alpha : >= 0 (0 opens everything).  Measured (profiles/r2_mac_sweep_*.md): the median error of theta = 0.4 at about
+ *           0.6 x the time, with a smaller 99th percentile.
+ *   amag  : DEV float[N], caller order, |a| of every particle, or NULL.  NULL: the library uses the accelerations of its
+ *           own last force pass; they travel with the particles through tree_leapfrog.  A pass with no accelerations to go
+ *           by (the first one after tree_build) uses the geometric criterion alone with its theta, so the usual sequence is
+ *           tree_build, tree_force(0.4, ...), tree_set_mac_relative(alpha, NULL), tree_force(1.0, ...), tree_leapfrog ...
+ *           Non-NULL (needs a built tree): these values scale the next pass instead (tests: the same input to the oracle).
+ * tree_set_mac(t, kind) switches it off again.  Needs no rebuild.  Not available on a sharded context
+ * (TREE_ERR_ORDER).  Allocates 8 bytes per particle and 4 per cell on first use. */
+int tree_set_mac_relative(tree_ctx *t, float alpha, const float *amag);
+
 /* vel: DEV float[N][3], caller order, N of the last tree_build.  tree_build forgets the velocities (it re-orders the
  * state): set them after every tree_build that is followed by tree_leapfrog. */
 int tree_set_velocity(tree_ctx *t, const float *vel);

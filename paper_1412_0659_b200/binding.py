@@ -37,6 +37,7 @@ _SIGS = {
     "tree_destroy": (C.c_int, [C.c_void_p]),
     "tree_set_velocity": (C.c_int, [C.c_void_p, C.c_void_p]),
     "tree_set_mac": (C.c_int, [C.c_void_p, C.c_int]),
+    "tree_set_mac_relative": (C.c_int, [C.c_void_p, C.c_float, C.c_void_p]),
     "tree_get_state": (C.c_int, [C.c_void_p] * 5),
     "tree_build_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_longlong]),
     "tree_force_host": (C.c_int, [C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.c_void_p]),
@@ -242,6 +243,13 @@ class Tree:
     def set_mac(self, kind):
         """Acceptance criterion (tree_set_mac): 0 / "geometric" (default) or 1 / "bmax"; before build."""
         _check(self.h, load_library().tree_set_mac(self.h, int(MAC_KINDS.get(kind, kind))))
+
+    def set_mac_relative(self, alpha: float, amag=None):
+        """Error-targeted acceptance per group on top of the geometric criterion (tree_set_mac_relative); ``amag``: CUDA
+        float32 [N] in caller order or None (the library's own last force pass)."""
+        if amag is not None:
+            assert amag.is_cuda and str(amag.dtype) == "torch.float32" and amag.is_contiguous() and (not self.n or amag.numel() == self.n)
+        _check(self.h, load_library().tree_set_mac_relative(self.h, float(alpha), _ptr(amag)))
 
     def set_velocity(self, vel):
         assert vel.is_cuda and vel.numel() == 3 * self.n

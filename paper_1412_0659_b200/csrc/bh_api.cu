@@ -184,13 +184,32 @@ int ensure_cells(tree_ctx *t, long long nc) {
   return 0;
 }
 
+// Buffers of the relative criterion (tree_set_mac_relative), sized like the particle and cell arrays they go with.
+static int ensure_relative(tree_ctx *t) {
+  Buffers &b = t->b;
+  if (t->rel_cap != t->cap) {
+    t->rel_cap = 0;
+    t->amag_valid = false;
+    BH_TRY(dev_alloc(t, b.amag2[0], t->cap));
+    BH_TRY(dev_alloc(t, b.amag2[1], t->cap));
+    BH_TRY(dev_alloc(t, b.gscale, (t->cap + t->group - 1) / t->group));
+    t->rel_cap = t->cap;
+  }
+  if (t->rel_cell_cap != t->cell_cap) {
+    t->rel_cell_cap = 0;
+    BH_TRY(dev_alloc(t, b.c_q, t->cell_cap));
+    t->rel_cell_cap = t->cell_cap;
+  }
+  return 0;
+}
+
 static void free_all(tree_ctx *t) {
   detach_peers(t);
   Buffers &b = t->b;
   void *ptrs[] = {b.posm, b.key[0], b.key[1], b.idx[0], b.idx[1], b.spos2[0], b.spos2[1], b.svel2[0], b.svel2[1], b.order2[0], b.order2[1],
                   b.scan_tmp, b.scan_blk, b.sort_hist, b.sort_status, b.shard_slab, b.gcost,
                   b.lv, b.gbox, b.gbox_prev, b.sched_a, b.sched_b, b.gdone, b.gparts, b.gthresh, b.tasks, b.part, b.trace, b.c_level, b.c_first, b.c_count, b.c_fcall, b.c_link, b.c_cm, b.c_qa, b.c_qb,
-                  b.c_test, b.c_tlo, b.c_thi, b.in_pos, b.in_mass, b.out_acc, b.out_pot};
+                  b.c_test, b.c_tlo, b.c_thi, b.in_pos, b.in_mass, b.out_acc, b.out_pot, b.amag2[0], b.amag2[1], b.gscale, b.c_q};
   for (void *p : ptrs) if (p) cudaFree(p);
   b = Buffers();
 }
@@ -225,6 +244,10 @@ static int force_begin_impl(tree_ctx *t, float theta, float eps, float kick_hdt,
   if (t->shard_world > 1)
     for (int r = 0; r < t->shard_world; ++r)
       if (r != t->shard_rank && !t->peer_base[r]) return set_err(t, TREE_ERR_ORDER, "sharded context: a peer is not attached");
+  if (t->rel_on) {  // before the pass moves on to the other result buffer
+    BH_TRY(ensure_relative(t));
+    if (t->amag_valid) BH_TRY(run_group_scale(t));
+  }
   t->pass++;
   t->b.sacc = t->b.sacc2[t->pass & 1];
   t->b.gcount = t->b.gcount2[t->pass & 1];
@@ -255,6 +278,10 @@ static int force_begin_impl(tree_ctx *t, float theta, float eps, float kick_hdt,
 // Second half: results to the caller's arrays if it gave any (in a sharded pass, after the caller's barrier).
 static int force_end_impl(tree_ctx *t, float *acc, float *pot) {
   BH_TRY(run_scatter_out(t, acc, pot));
+  if (t->rel_on) {  // |a| of this pass scales the next one
+    BH_TRY(run_amag_from_acc(t));
+    t->amag_valid = true;
+  }
   rec(t, EV_UNPERM);
   t->force_open = false;
   t->have_force = true;
@@ -414,6 +441,7 @@ int tree_build(tree_ctx *t, const float *pos, const float *mass, long long N) {
   t->have_force = false;
   t->have_vel = false;   // the slot order changes: velocities are set again after a build (tree.h)
   t->state_valid = false;
+  t->amag_valid = false; // and so are the accelerations that scale the relative criterion
   BH_TRY(ensure_particles(t, N));
   t->N = N;
   t->n_groups = (N + t->group - 1) / t->group;
@@ -507,6 +535,7 @@ int tree_shard_config(tree_ctx *t, int rank, int world) {
     return set_err(t, TREE_ERR_ARG, "tree_shard_config: need 0 <= rank < world <= TREE_SHARD_MAX_WORLD");
   if (t->force_open || t->step_open) return set_err(t, TREE_ERR_ORDER, "tree_shard_config inside an open force pass");
   if (world > 1 && t->cap <= 0) return set_err(t, TREE_ERR_ORDER, "tree_shard_config before tree_reserve");
+  if (world > 1 && t->rel_on) return set_err(t, TREE_ERR_ORDER, "tree_shard_config: the relative criterion is not available on a sharded context");
   BH_DEVICE(t);
   BH_CUDA(cudaStreamSynchronize(t->stream));
   if (world != t->shard_world || rank != t->shard_rank) detach_peers(t);
@@ -609,6 +638,7 @@ int tree_set_mac(tree_ctx *t, int kind) {
   if (kind != TREE_MAC_GEOMETRIC && kind != TREE_MAC_BMAX) return set_err(t, TREE_ERR_ARG, "tree_set_mac: unknown criterion");
   if (t->force_open || t->step_open) return set_err(t, TREE_ERR_ORDER, "tree_set_mac inside an open force pass");
   BH_DEVICE(t);
+  t->rel_on = false;
   if (kind != t->mac) {
     t->mac = kind;
     t->built = false;  // the tight boxes are computed with the moments: build again
@@ -618,6 +648,27 @@ int tree_set_mac(tree_ctx *t, int kind) {
       BH_TRY(dev_alloc(t, t->b.c_tlo, t->cell_cap));
       BH_TRY(dev_alloc(t, t->b.c_thi, t->cell_cap));
     }
+  }
+  return TREE_OK;
+}
+
+int tree_set_mac_relative(tree_ctx *t, float alpha, const float *amag) {
+  if (!t) return TREE_ERR_ARG;
+  if (!(alpha >= 0.0f) || !isfinite(alpha)) return set_err(t, TREE_ERR_ARG, "tree_set_mac_relative: alpha must be finite and >= 0");
+  if (t->force_open || t->step_open) return set_err(t, TREE_ERR_ORDER, "tree_set_mac_relative inside an open force pass");
+  if (t->shard_world > 1) return set_err(t, TREE_ERR_ORDER, "tree_set_mac_relative: not available on a sharded context");
+  if (t->mac != TREE_MAC_GEOMETRIC) return set_err(t, TREE_ERR_ORDER, "tree_set_mac_relative: the floor is the geometric criterion (tree_set_mac)");
+  if (amag && !t->built) return set_err(t, TREE_ERR_ORDER, "tree_set_mac_relative with accelerations before tree_build");
+  BH_DEVICE(t);
+  t->rel_on = true;
+  t->rel_alpha = alpha;
+  if (t->cap > 0) BH_TRY(ensure_relative(t));
+  if (amag) {
+    BH_TRY(run_amag_from_caller(t, amag));
+    t->amag_valid = true;
+  } else if (!t->amag_valid && t->built && t->have_force) {
+    BH_TRY(run_amag_from_acc(t));  // the pass before this call provides the scale
+    t->amag_valid = true;
   }
   return TREE_OK;
 }

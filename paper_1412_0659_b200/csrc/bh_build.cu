@@ -485,6 +485,7 @@ __global__ void __launch_bounds__(256) permute_step_kernel(const uint64_t *__res
                                                            const float4 *__restrict__ pos_in, const float4 *__restrict__ vel_in,
                                                            const uint32_t *__restrict__ order_in, float4 *__restrict__ pos_out,
                                                            float4 *__restrict__ vel_out, uint32_t *__restrict__ order_out,
+                                                           const float *__restrict__ amag_in, float *__restrict__ amag_out,
                                                            long long N) {
   const long long s = blockIdx.x * (long long)blockDim.x + threadIdx.x;
   if (s >= N) return;
@@ -504,6 +505,7 @@ __global__ void __launch_bounds__(256) permute_step_kernel(const uint64_t *__res
   pos_out[dst] = pos_in[q];
   vel_out[dst] = vel_in[q];
   order_out[dst] = me;
+  if (amag_in) amag_out[dst] = amag_in[q];  // relative criterion: |a| of the last force pass travels with the particle
 }
 
 // ------------------------------------------------------------------------------------------
@@ -1077,7 +1079,7 @@ int run_permute_step(tree_ctx *t) {
   const int nxt = t->cur ^ 1;
   permute_step_kernel<<<(unsigned)((t->N + 255) / 256), 256, 0, t->stream>>>(
       t->b.skey, t->b.sperm, t->b.spos, t->b.svel, t->b.order, t->b.spos2[nxt], t->b.svel2[nxt],
-      t->b.order2[nxt], t->N);
+      t->b.order2[nxt], t->rel_on && t->amag_valid ? t->b.amag2[t->cur] : nullptr, t->b.amag2[nxt], t->N);
   BH_LAUNCH_CHECK("permute_step");
   t->cur = nxt;
   t->b.spos = t->b.spos2[nxt]; t->b.svel = t->b.svel2[nxt]; t->b.order = t->b.order2[nxt];

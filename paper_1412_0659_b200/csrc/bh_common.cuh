@@ -99,6 +99,9 @@ struct Buffers {
   float4 *c_qb = nullptr;     // Qxy,Qxz,Qyz,tr(Q)
   float4 *c_test = nullptr;   // cx,cy,cz,r_open^2 (per force call)
   float4 *c_tlo = nullptr, *c_thi = nullptr;  // TREE_MAC_BMAX only: tight box lo x,y,z | b  and  hi x,y,z | -
+  // tree_set_mac_relative only: |a| of the last force pass per slot (part of the state: gathered with it by a step),
+  // alpha * min |a| per group, M l^3 per cell (per force call)
+  float *amag2[2] = {nullptr, nullptr}, *gscale = nullptr, *c_q = nullptr;
   // host-call staging
   float *in_pos = nullptr, *in_mass = nullptr, *out_acc = nullptr, *out_pot = nullptr;
 };
@@ -110,6 +113,10 @@ struct tree_ctx {
   cudaStream_t stream = nullptr;
   int leaf = 16, group = 64;
   int mac = TREE_MAC_GEOMETRIC;      // acceptance criterion (tree_set_mac)
+  bool rel_on = false;               // tree_set_mac_relative: the error-targeted condition on top of the geometric one
+  float rel_alpha = 0.f;
+  bool amag_valid = false;           // b.amag2[cur] holds |a| of every particle of the current slot order
+  long long rel_cap = 0, rel_cell_cap = 0;  // capacities b.amag2 / b.gscale and b.c_q were allocated for
   long long N = 0, cap = 0;          // particles, particle capacity
   long long n_cells = 0, cell_cap = 0;  // n_cells: exact after tree_build; after an asynchronous rebuild (tree_leapfrog) the
                                         // latest count read back so far (poll_cells)
@@ -194,6 +201,9 @@ int run_permute_step(tree_ctx *t);    // tree_leapfrog: spos, svel, order -> the
 int run_tree(tree_ctx *t, bool async);  // octree construction; !async: synchronises once and sizes the cell arrays
 int run_groups_moments(tree_ctx *t);
 int run_opening(tree_ctx *t, float theta);
+int run_amag_from_acc(tree_ctx *t);                      // relative criterion: amag[s] = |a| of the last force pass
+int run_amag_from_caller(tree_ctx *t, const float *amag);  // ... or the caller's values (caller order) into slot order
+int run_group_scale(tree_ctx *t);                        // gscale[g] = alpha * min amag over the group's slots
 // kick_hdt != 0: v += a * kick_hdt in the walk's epilogue; out_acc / out_pot (one context): results also to the caller's arrays there
 int run_walk(tree_ctx *t, float eps, float kick_hdt, float *out_acc, float *out_pot);
 int run_box_check(tree_ctx *t);  // device-side: are the group boxes where the previous force pass saw them?

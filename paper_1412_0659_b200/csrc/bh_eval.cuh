@@ -79,6 +79,8 @@ struct WalkParams {
   int reuse_mode;          // 0: costs from the counting walk; 1: from the previous pass's counts; 2: info->reuse_costs decides
   const uint32_t *order;   // tree_force with caller arrays on one context: the epilogue also writes each result to the caller's
   float *out_acc, *out_pot;  // arrays at order[slot] (a11 fused: no separate pass); order = nullptr otherwise
+  const float *c_q;        // relative criterion (walk kernels with REL = true): M l^3 per cell,
+  const float *gscale;     // alpha * min |a| per group
 };
 
 constexpr unsigned TASK_GROUP_BITS = 26;

@@ -15,9 +15,14 @@ namespace bh {
 __global__ void __launch_bounds__(256) opening_kernel(const DevInfo *__restrict__ info, float theta,
                                                       const uint8_t *__restrict__ c_level,
                                                       const float4 *__restrict__ c_cm, const float4 *__restrict__ c_qa,
-                                                      const float4 *__restrict__ c_tlo, float4 *__restrict__ c_test) {
+                                                      const float4 *__restrict__ c_tlo, float4 *__restrict__ c_test,
+                                                      float *__restrict__ c_q) {
   long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x;
   if (info->cells_overflow || c >= info->n_cells) return;
+  if (c_q) {  // relative criterion: q = M l^3, three IEEE multiplications in this order
+    const float lc = ldexpf(1.0f, info->k - (int)c_level[c]);
+    c_q[c] = __fmul_rn(__fmul_rn(__fmul_rn(c_cm[c].w, lc), lc), lc);
+  }
   float r;
   if (c_tlo) {  // TREE_MAC_BMAX: r = b / theta (theta = 0 opens everything, also where b = 0)
     r = theta == 0.0f ? INFINITY : __fdiv_rn(c_tlo[c].w, theta);
@@ -91,7 +96,7 @@ __device__ __forceinline__ void kick_slot(float4 *v, const float4 a, float hdt) 
 }
 
 // One work item: group g (part `part` of `nparts`).
-template <int TPL, bool COUNT>
+template <int TPL, bool COUNT, bool REL>
 __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, const int lane, const unsigned item,
                                           const unsigned g, const unsigned part, const unsigned nparts,
                                           const unsigned long long t_start) {
@@ -130,6 +135,8 @@ __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, con
   }
   const float *gb = P.gbox + 6ll * g;
   const float bx0 = gb[0], by0 = gb[1], bz0 = gb[2], bx1 = gb[3], by1 = gb[4], bz1 = gb[5];
+  float gscale = 0.0f;  // relative criterion: alpha * min |a| over the group's particles
+  if (REL) gscale = P.gscale[g];
 
   int sp = 1;                       // live stack entries are [0, sp)
   if (lane == 0) ws.stack[0] = 0u;  // root: cell 0, one cell
@@ -199,6 +206,10 @@ __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, con
       float uz = fmaxf(0.0f, fmaxf(__fsub_rn(bz0, tr.z), __fsub_rn(tr.z, bz1)));
       float d2 = __fmaf_rn(uz, uz, __fmaf_rn(uy, uy, __fmul_rn(ux, ux)));
       accept = d2 > tr.w;
+      if (REL) {  // error-targeted condition on top of the geometric floor: D^5 alpha a_g > M l^3, one IEEE op each
+        const float lhs = __fmul_rn(__fmul_rn(__fmul_rn(__fsqrt_rn(d2), d2), d2), gscale);
+        accept = accept && lhs > P.c_q[cell];
+      }
       bool leaf = !(lk.y & LEAF_FLAG);
       if (COUNT && !leaf && !accept) {  // cost estimate: do not descend below small cells
         const unsigned cc = P.c_count[cell];
@@ -364,7 +375,7 @@ __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, con
   }
 }
 
-template <int TPL, bool COUNT>
+template <int TPL, bool COUNT, bool REL>
 __global__ void __launch_bounds__(WALK_WARPS * 32, COUNT ? COUNT_MINB : walk_minb(TPL)) walk_force_kernel(const WalkParams P) {
   __shared__ WarpSmem smem[WALK_WARPS];
   WarpSmem &ws = smem[threadIdx.x >> 5];
@@ -379,7 +390,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, COUNT ? COUNT_MINB : walk_min
     item = __shfl_sync(0xffffffffu, item, 0);
     if (item >= n_items) break;
     if (COUNT) {
-      walk_task<TPL, true>(P, ws, lane, item, item, 0u, 1u, 0ull);
+      walk_task<TPL, true, REL>(P, ws, lane, item, item, 0u, 1u, 0ull);
       continue;
     }
     unsigned long long t_start;
@@ -388,7 +399,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, COUNT ? COUNT_MINB : walk_min
     if (tk == TASK_NONE) continue;  // hole in the tail region of the task list
     const unsigned g = tk & TASK_GROUP_MASK, part = tk >> TASK_GROUP_BITS;
     const unsigned nparts = P.gparts[g] & PARTS_MASK;
-    walk_task<TPL, false>(P, ws, lane, item, g, part, nparts, t_start);
+    walk_task<TPL, false, REL>(P, ws, lane, item, g, part, nparts, t_start);
   }
 }
 
@@ -885,8 +896,57 @@ static inline unsigned blocks_for(long long n, int threads) { return (unsigned)(
 
 int run_opening(tree_ctx *t, float theta) {
   opening_kernel<<<blocks_for(t->cells_bound, 256), 256, 0, t->stream>>>(
-      t->d_info, theta, t->b.c_level, t->b.c_cm, t->b.c_qa, t->mac == TREE_MAC_BMAX ? t->b.c_tlo : nullptr, t->b.c_test);
+      t->d_info, theta, t->b.c_level, t->b.c_cm, t->b.c_qa, t->mac == TREE_MAC_BMAX ? t->b.c_tlo : nullptr, t->b.c_test,
+      t->rel_on && t->amag_valid ? t->b.c_q : nullptr);
   BH_LAUNCH_CHECK("opening");
+  return 0;
+}
+
+// Relative criterion (tree_set_mac_relative): |a| per slot, one IEEE operation each in this order, and the group's scale
+// alpha * min |a| (one warp per group; min is exact, one multiplication).
+__global__ void __launch_bounds__(256) amag_acc_kernel(const float4 *__restrict__ sacc, long long N, float *__restrict__ amag) {
+  long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  const float4 a = sacc[i];
+  amag[i] = __fsqrt_rn(__fmaf_rn(a.z, a.z, __fmaf_rn(a.y, a.y, __fmul_rn(a.x, a.x))));
+}
+
+__global__ void __launch_bounds__(256) amag_caller_kernel(const float *__restrict__ given, const uint32_t *__restrict__ order,
+                                                          long long N, float *__restrict__ amag) {
+  long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (i < N) amag[i] = given[order[i]];
+}
+
+__global__ void __launch_bounds__(256) group_scale_kernel(const float *__restrict__ amag, long long N, int group, float alpha,
+                                                          long long n_groups, float *__restrict__ gscale) {
+  const long long g = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (g >= n_groups) return;
+  const long long s0 = g * group;
+  float m = INFINITY;
+  for (int j = lane; j < group; j += 32)
+    if (s0 + j < N) m = fminf(m, amag[s0 + j]);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = fminf(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if (lane == 0) gscale[g] = __fmul_rn(alpha, m);
+}
+
+int run_amag_from_acc(tree_ctx *t) {
+  amag_acc_kernel<<<blocks_for(t->N, 256), 256, 0, t->stream>>>(t->b.sacc, t->N, t->b.amag2[t->cur]);
+  BH_LAUNCH_CHECK("amag_acc");
+  return 0;
+}
+
+int run_amag_from_caller(tree_ctx *t, const float *amag) {
+  amag_caller_kernel<<<blocks_for(t->N, 256), 256, 0, t->stream>>>(amag, t->b.order, t->N, t->b.amag2[t->cur]);
+  BH_LAUNCH_CHECK("amag_caller");
+  return 0;
+}
+
+int run_group_scale(tree_ctx *t) {
+  group_scale_kernel<<<blocks_for(t->n_groups * 32, 256), 256, 0, t->stream>>>(t->b.amag2[t->cur], t->N, t->group, t->rel_alpha,
+                                                                               t->n_groups, t->b.gscale);
+  BH_LAUNCH_CHECK("group_scale");
   return 0;
 }
 
@@ -936,7 +996,7 @@ int run_box_check(tree_ctx *t) {
   return 0;
 }
 
-template <int TPL>
+template <int TPL, bool REL>
 static int launch_walk(tree_ctx *t, const WalkParams &P, unsigned grid) {
   const unsigned ng = P.n_groups, gb = (ng + 255) / 256;
   DevInfo *info = t->d_info;
@@ -945,7 +1005,7 @@ static int launch_walk(tree_ctx *t, const WalkParams &P, unsigned grid) {
   const int mode = P.reuse_mode;
   if (mode != 1) {  // mode 2: the kernel returns at once if the device decided to reuse the previous counts
     const long long cwant = (ng + WALK_WARPS - 1) / WALK_WARPS, ccap = (long long)t->sm_count * COUNT_MINB;
-    walk_force_kernel<TPL, true><<<(unsigned)(cwant < ccap ? cwant : ccap), WALK_WARPS * 32, 0, t->stream>>>(P);
+    walk_force_kernel<TPL, true, REL><<<(unsigned)(cwant < ccap ? cwant : ccap), WALK_WARPS * 32, 0, t->stream>>>(P);
     BH_LAUNCH_CHECK("walk_count");
   }
   group_cost_kernel<<<gb, 256, 0, t->stream>>>(ng, info, t->b.gdone, t->b.gcount2[(t->pass + 1) & 1], mode, t->b.gcost);
@@ -977,7 +1037,7 @@ static int launch_walk(tree_ctx *t, const WalkParams &P, unsigned grid) {
   BH_LAUNCH_CHECK("task_fill");
   if (t->ev_valid[EV_SCHED]) cudaEventRecord(t->ev[EV_SCHED], t->stream);
   // 3. the fused walk + force over the task list
-  walk_force_kernel<TPL, false><<<grid, WALK_WARPS * 32, 0, t->stream>>>(P);
+  walk_force_kernel<TPL, false, REL><<<grid, WALK_WARPS * 32, 0, t->stream>>>(P);
   BH_LAUNCH_CHECK("walk_force");
   return 0;
 }
@@ -1011,10 +1071,12 @@ int run_walk(tree_ctx *t, float eps, float kick_hdt, float *out_acc, float *out_
   unsigned grid = (unsigned)(want < cap ? want : cap);
   if (t->ev_valid[EV_OPEN]) cudaEventRecord(t->ev[EV_OPEN], t->stream);
   int rc;
+  const bool rel = t->rel_on && t->amag_valid;  // no |a| yet (first pass after tree_build): the geometric criterion alone
+  P.c_q = rel ? t->b.c_q : nullptr; P.gscale = rel ? t->b.gscale : nullptr;
   switch (t->group) {
-    case 32: rc = launch_walk<1>(t, P, grid); break;
-    case 64: rc = launch_walk<2>(t, P, grid); break;
-    case 128: rc = launch_walk<4>(t, P, grid); break;
+    case 32: rc = rel ? launch_walk<1, true>(t, P, grid) : launch_walk<1, false>(t, P, grid); break;
+    case 64: rc = rel ? launch_walk<2, true>(t, P, grid) : launch_walk<2, false>(t, P, grid); break;
+    case 128: rc = rel ? launch_walk<4, true>(t, P, grid) : launch_walk<4, false>(t, P, grid); break;
     default: return set_err(t, TREE_ERR_ARG, "group size");
   }
   if (rc) return rc;

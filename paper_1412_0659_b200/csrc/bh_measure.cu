@@ -233,7 +233,7 @@ extern "C" int tree_measure_listeval(tree_ctx *t, double *ms /*[2]: list walk, e
   P.c_cm = t->b.c_cm; P.c_qa = t->b.c_qa; P.c_qb = t->b.c_qb;
   P.gbox = t->b.gbox; P.sacc = t->b.sacc; P.gcount = t->b.gcount; P.info = t->d_info; P.n_peers = 0;
   P.N = t->N; P.n_groups = ng; P.eps2 = t->eps * t->eps; P.svel = nullptr; P.kick_hdt = 0.f; P.reuse_mode = 0;
-  P.order = nullptr; P.out_acc = nullptr; P.out_pot = nullptr;
+  P.order = nullptr; P.out_acc = nullptr; P.out_pot = nullptr; P.c_q = nullptr; P.gscale = nullptr;
   L.gorder = d_gorder; L.pc_off = d_pc_off; L.pp_off = d_pp_off; L.pc_list = d_pc; L.pp_list = d_pp; L.out = d_out;
   L.ticket = d_ticket;
   cudaEvent_t e0, e1, e2;

@@ -1,0 +1,144 @@
+"""GPU parity of the error-targeted acceptance criterion (tree_set_mac_relative) against the oracle's
+option "relative": with the SAME per-particle |a| given to both sides, per-group interaction counts are bit-exact and
+forces agree to 1e-5; the library's own bookkeeping (|a| of its last pass, carried through tree_leapfrog) gives the same
+lists as handing those values in; the criterion buys the canonical median error with fewer interactions."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from nbody_inputs import plummer, milky_way
+from paper_1412_0659_b200 import Tree, TreeError
+
+pytestmark = pytest.mark.gpu
+
+
+def _amag_like_the_kernel(a32):
+    """|a| as amag_acc_kernel forms it: sqrt(fma(az, az, fma(ay, ay, ax * ax))), FP32, one rounding each (long double holds
+    the exact products and sums of FP32 operands here up to a 2^-40 chance of a double rounding)."""
+    a = a32.astype(np.longdouble)
+    x = (a[:, 0] * a[:, 0]).astype(np.float32).astype(np.longdouble)
+    y = (a[:, 1] * a[:, 1] + x).astype(np.float32).astype(np.longdouble)
+    z = (a[:, 2] * a[:, 2] + y).astype(np.float32)
+    return np.sqrt(z)  # IEEE sqrt of an FP32 value in FP32
+
+
+@pytest.mark.parametrize("model,n,seed,alpha,floor,leaf,group", [
+    ("plummer", 16384, 1001, 1e-3, 1.0, 16, 64),
+    ("mw", 100000 + 13, 3, 3e-4, 1.0, 16, 64),
+    ("mw", 40000, 5, 3e-3, 0.7, 16, 64),
+    ("plummer", 5000, 7, 1e-3, 1.0, 8, 32),
+    ("mw", 30000, 9, 1e-3, 1.0, 16, 128),
+    ("plummer", 3000, 11, 0.0, 1.0, 16, 64),
+])
+def test_relative_parity_with_the_same_accelerations_on_both_sides(model, n, seed, alpha, floor, leaf, group):
+    eps = 0.01
+    pos, _, mass = (plummer if model == "plummer" else milky_way)(n, seed, with_vel=False)
+    ot = oracle.Tree(pos.numpy(), mass.numpy(), leaf_size=leaf, group_size=group)
+    a0, _, pp0, pc0 = ot.force(0.4, eps)                           # the oracle's own canonical pass provides |a|
+    amag = np.linalg.norm(a0, axis=1).astype(np.float32)
+    ot.set_mac_relative(alpha, amag)
+    oacc, opot, onpp, onpc = ot.force(floor, eps)
+    t = Tree(device=0, leaf_size=leaf, group_size=group)
+    acc = torch.empty((n, 3), device="cuda"); pot = torch.empty(n, device="cuda")
+    t.build(pos.cuda(), mass.cuda())
+    t.set_mac_relative(alpha, torch.from_numpy(amag).cuda())
+    t.force(floor, eps, acc, pot)
+    torch.cuda.synchronize()
+    cnt = t.debug("counts")
+    assert np.array_equal(cnt[:, 0], onpp) and np.array_equal(cnt[:, 1], onpc)
+    if alpha > 0:
+        assert (13.0 * onpp + 32.0 * onpc).sum() > 0 and not np.array_equal(onpc, pc0)   # the condition really decided
+    a = acc.cpu().numpy().astype(np.float64); p = pot.cpu().numpy().astype(np.float64)
+    assert (np.linalg.norm(a - oacc, axis=1) / np.linalg.norm(oacc, axis=1)).max() <= 1e-5
+    assert (np.abs(p - opot) / np.abs(opot)).max() <= 1e-5
+    # switched off again: the canonical lists, no rebuild needed
+    t.set_mac("geometric")
+    t.force(0.4, eps)
+    cnt = t.debug("counts")
+    assert np.array_equal(cnt[:, 0], pp0) and np.array_equal(cnt[:, 1], pc0)
+    t.close()
+
+
+def test_own_accelerations_travel_with_the_particles_through_leapfrog_steps():
+    n, alpha, floor, eps, dt = 60000, 1e-3, 1.0, 0.01, 0.002
+    pos, vel, mass = milky_way(n, 21)
+    t = Tree(device=0)
+    t.build(pos.cuda(), mass.cuda()); t.set_velocity(vel.cuda())
+    t.force(0.4, eps)                      # no accelerations yet: the geometric criterion
+    t.set_mac_relative(alpha)              # from here on scaled by the last pass
+    t.force(floor, eps)
+    for _ in range(2):
+        t.leapfrog(dt)
+    a_prev = torch.empty((n, 3), device="cuda")
+    t.get_state(None, None, a_prev, None); torch.cuda.synchronize()
+    amag = _amag_like_the_kernel(a_prev.cpu().numpy())
+    t.leapfrog(dt)                         # this step's pass is scaled by |a_prev|, gathered into the new slot order
+    p = torch.empty((n, 3), device="cuda"); a = torch.empty((n, 3), device="cuda")
+    t.get_state(p, None, a, None); torch.cuda.synchronize()
+    cnt = t.debug("counts")
+    # the same pass with the values handed in: a second context built on the step's positions ...
+    t2 = Tree(device=0)
+    t2.build(p, mass.cuda())
+    t2.set_mac_relative(alpha, torch.from_numpy(amag).cuda())
+    t2.force(floor, eps)
+    assert np.array_equal(t2.debug("counts"), cnt)
+    t2.close()
+    # ... and the oracle on the same input
+    ot = oracle.Tree(p.cpu().numpy(), mass.numpy())
+    ot.set_mac_relative(alpha, amag)
+    oacc, _, onpp, onpc = ot.force(floor, eps)
+    assert np.array_equal(cnt[:, 0], onpp) and np.array_equal(cnt[:, 1], onpc)
+    rel = np.linalg.norm(a.cpu().numpy().astype(np.float64) - oacc, axis=1) / np.linalg.norm(oacc, axis=1)
+    assert rel.max() <= 1e-5
+    t.close()
+
+
+def test_relative_criterion_buys_the_canonical_error_with_fewer_interactions():
+    n, eps = 400000, 0.01
+    pos, _, mass = milky_way(n, 33, with_vel=False)
+    idx = torch.from_numpy(np.sort(np.random.default_rng(2001).choice(n, 8192, replace=False)).astype(np.int64)).cuda()
+    t = Tree(device=0)
+    acc = torch.empty((n, 3), device="cuda")
+    t.build(pos.cuda(), mass.cuda())
+    dacc = torch.empty((idx.numel(), 3), dtype=torch.float64, device="cuda")
+    dpot = torch.empty(idx.numel(), dtype=torch.float64, device="cuda")
+    t.direct(idx, eps, dacc, dpot)
+    dn = dacc.norm(dim=1)
+
+    def err():
+        e = ((acc[idx].double() - dacc).norm(dim=1) / dn).cpu().numpy()
+        _, pp, pc = t.stats()
+        return np.median(e), np.percentile(e, 99), 13.0 * pp + 32.0 * pc
+    t.force(0.4, eps, acc)
+    m0, p0, c0 = err()
+    t.set_mac_relative(3e-4)
+    t.force(1.0, eps, acc)
+    m1, p1, c1 = err()
+    assert m1 <= m0 and p1 < p0 and c1 < 0.75 * c0, (m0, p0, m1, p1, c1 / c0)
+    t.close()
+
+
+def test_relative_criterion_argument_and_order_errors():
+    pos, _, mass = plummer(2000, 3, with_vel=False)
+    t = Tree(device=0)
+    with pytest.raises(TreeError):
+        t.set_mac_relative(-1.0)
+    with pytest.raises(TreeError):                       # accelerations handed in before there is a slot order to put them in
+        t.set_mac_relative(1e-3, torch.ones(2000, device="cuda"))
+    t.set_mac("bmax")
+    with pytest.raises(TreeError) as e:                  # the floor is the geometric criterion
+        t.set_mac_relative(1e-3)
+    assert e.value.code == -4
+    t.set_mac("geometric")
+    t.set_mac_relative(1e-3)                             # before any build: allowed, takes effect once a pass has run
+    t.build(pos.cuda(), mass.cuda()); t.force(0.4, 0.01)
+    c_geo = t.debug("counts").copy()
+    t.force(1.0, 0.01)
+    assert not np.array_equal(t.debug("counts"), c_geo)
+    t.close()
+    t = Tree(device=0)
+    t.reserve(2000); t.shard_config(0, 2)
+    with pytest.raises(TreeError):
+        t.set_mac_relative(1e-3)
+    t.close()
