@@ -423,6 +423,36 @@ def run_ours(args):
               "rel_drift": abs((ke1 + pe1) - (ke0 + pe0)) / abs(ke0 + pe0)}
     clocks = sampler.stop()
     step_ms = sum(a.elapsed_time(b) for a, b in ev)
+
+    # ---- beside the headline (not part of `value`): the same steps with the error-targeted acceptance criterion
+    # (tree_set_mac_relative): time per step and error against direct summation on the same workload
+    relative = None
+    if world == 1 and not args.no_accuracy:
+        alpha, floor, rsteps = 3e-4, 1.0, min(args.steps, 5)
+        acc_r = torch.empty((n, 3), device=dev)
+        t.set_mac_relative(alpha)                      # scaled by |a| of the last pass of the steps above
+        t.force(floor, cfg["eps"], acc_r)
+        acc_rel = _accuracy(t, n, cfg["eps"], acc_r, nsub=16384)
+        del acc_r
+        t.leapfrog(dt)
+        rev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(rsteps)]
+        rpp = rpc = 0
+        rwalk = 0.0
+        for k in range(rsteps):
+            flush.fill_(k & 0xff)
+            rev[k][0].record(stream)
+            t.leapfrog(dt)
+            rev[k][1].record(stream)
+            ms, pp, pc = t.stats()
+            rpp += pp; rpc += pc; rwalk += ms["walk"]
+        rms = sum(a.elapsed_time(b) for a, b in rev)
+        relative = {"criterion": f"tree_set_mac_relative(alpha={alpha:g}), geometric floor theta={floor:g}; |a| of the previous pass",
+                    "steps": rsteps, "ms_per_step": rms / rsteps, "walk_ms": rwalk / rsteps,
+                    "value": (rpp + rpc) / (rms * 1e-3), "unit": UNIT,
+                    "pp_per_particle": rpp / rsteps / n, "pc_per_particle": rpc / rsteps / n,
+                    "roofline_frac": effective_flops(rpp, rpc) / (rwalk * 1e-3) / 1e12 / _peak_tflops(torch.cuda.get_device_properties(dev).multi_processor_count),
+                    "accuracy": acc_rel, "speedup_of_step_vs_headline": (step_ms / args.steps) / (rms / rsteps)}
+        t.set_mac("geometric")
     mx, sm = reduce_max_sum([step_ms, float(pp_tot), float(pc_tot), phase_ms["walk"]], dev)
     step_ms_max = mx[0]
     pp_all, pc_all = sm[1], sm[2]
@@ -512,6 +542,7 @@ def run_ours(args):
             "phase_ms": {k: v / args.steps for k, v in phase_ms.items()},
             "roofline": roof,
             "accuracy": accuracy,
+            "relative_mac": relative,
             "energy": energy,
             "cpu_baseline": cpu,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 16 * n,

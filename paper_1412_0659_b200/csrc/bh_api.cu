@@ -535,7 +535,6 @@ int tree_shard_config(tree_ctx *t, int rank, int world) {
     return set_err(t, TREE_ERR_ARG, "tree_shard_config: need 0 <= rank < world <= TREE_SHARD_MAX_WORLD");
   if (t->force_open || t->step_open) return set_err(t, TREE_ERR_ORDER, "tree_shard_config inside an open force pass");
   if (world > 1 && t->cap <= 0) return set_err(t, TREE_ERR_ORDER, "tree_shard_config before tree_reserve");
-  if (world > 1 && t->rel_on) return set_err(t, TREE_ERR_ORDER, "tree_shard_config: the relative criterion is not available on a sharded context");
   BH_DEVICE(t);
   BH_CUDA(cudaStreamSynchronize(t->stream));
   if (world != t->shard_world || rank != t->shard_rank) detach_peers(t);
@@ -656,7 +655,6 @@ int tree_set_mac_relative(tree_ctx *t, float alpha, const float *amag) {
   if (!t) return TREE_ERR_ARG;
   if (!(alpha >= 0.0f) || !isfinite(alpha)) return set_err(t, TREE_ERR_ARG, "tree_set_mac_relative: alpha must be finite and >= 0");
   if (t->force_open || t->step_open) return set_err(t, TREE_ERR_ORDER, "tree_set_mac_relative inside an open force pass");
-  if (t->shard_world > 1) return set_err(t, TREE_ERR_ORDER, "tree_set_mac_relative: not available on a sharded context");
   if (t->mac != TREE_MAC_GEOMETRIC) return set_err(t, TREE_ERR_ORDER, "tree_set_mac_relative: the floor is the geometric criterion (tree_set_mac)");
   if (amag && !t->built) return set_err(t, TREE_ERR_ORDER, "tree_set_mac_relative with accelerations before tree_build");
   BH_DEVICE(t);

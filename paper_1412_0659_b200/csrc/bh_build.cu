@@ -431,6 +431,7 @@ __global__ void __launch_bounds__(OS_THREADS, OS_MINB) sort_onesweep_kernel(cons
     const unsigned d = threadIdx.x;
     unsigned long long *mine = status + (size_t)tile * RADIX + d;
     const unsigned long long tag = epoch << 32;
+    const unsigned tag_hi = (unsigned)epoch;  // epoch < 2^30: the high word of a status word of this pass is flag << 30 | epoch
     unsigned excl = 0;
     if (tile > 0) {
       bool done = false;
@@ -439,6 +440,22 @@ __global__ void __launch_bounds__(OS_THREADS, OS_MINB) sort_onesweep_kernel(cons
 #pragma unroll
         for (int j = 0; j < OS_LOOK; ++j)
           v[j] = (q - j >= 0) ? ld_status(status + (size_t)(q - j) * RADIX + d) : (OS_INCL | tag);
+        // the usual case: all OS_LOOK words were published long ago (a tile walks back over ~40 predecessors): sum the
+        // local counts up to the first inclusive prefix without a branch per word
+        bool all_ok = true;
+#pragma unroll
+        for (int j = 0; j < OS_LOOK; ++j) {
+          const unsigned hi = (unsigned)(v[j] >> 32);
+          all_ok = all_ok && (hi & 0x3fffffffu) == tag_hi && (hi >> 30) != 0u;
+        }
+        if (all_ok) {
+#pragma unroll
+          for (int j = 0; j < OS_LOOK; ++j) {
+            excl += done ? 0u : (unsigned)v[j];
+            done = done || (unsigned)(v[j] >> 62) == 2u;
+          }
+          continue;
+        }
 #pragma unroll
         for (int j = 0; j < OS_LOOK; ++j) {
           if (done) break;

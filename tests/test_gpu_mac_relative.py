@@ -137,8 +137,103 @@ def test_relative_criterion_argument_and_order_errors():
     t.force(1.0, 0.01)
     assert not np.array_equal(t.debug("counts"), c_geo)
     t.close()
-    t = Tree(device=0)
-    t.reserve(2000); t.shard_config(0, 2)
-    with pytest.raises(TreeError):
-        t.set_mac_relative(1e-3)
-    t.close()
+
+
+def test_relative_criterion_on_sharded_contexts_equals_one_context():
+    # every rank holds the complete results of every pass, so all ranks derive the same group scales: a sharded run in this
+    # mode must reproduce the single context's lists and forces bit for bit, through force passes and leapfrog steps
+    from paper_1412_0659_b200.sharded import connect_local, force_local, leapfrog_local
+    n, alpha, eps, dt = 50000, 1e-3, 0.01, 0.002
+    pos, vel, mass = milky_way(n, 17)
+    dpos, dvel, dmass = pos.cuda(), vel.cuda(), mass.cuda()
+
+    def run(world):
+        trees = [Tree(device=0) for _ in range(world)]
+        if world > 1:
+            for t in trees:
+                t.reserve(n)
+            connect_local(trees)
+        for t in trees:
+            t.build(dpos, dmass); t.set_velocity(dvel)
+        force_local(trees, 0.4, eps)
+        for t in trees:
+            t.set_mac_relative(alpha)
+        force_local(trees, 1.0, eps)
+        for _ in range(3):
+            leapfrog_local(trees, dt)
+        torch.cuda.synchronize()
+        res = []
+        for t in trees:
+            p = torch.empty((n, 3), device="cuda"); a = torch.empty((n, 3), device="cuda")
+            t.get_state(p, None, a, None); torch.cuda.synchronize()
+            res.append((p.cpu(), a.cpu(), t.debug("counts").copy()))
+            t.close()
+        return res
+    one = run(1)[0]
+    for world in (2, 5):
+        for p, a, c in run(world):
+            assert torch.equal(p, one[0]) and torch.equal(a, one[1]) and np.array_equal(c, one[2])
+
+
+def test_energy_drift_with_the_relative_criterion_is_no_worse_than_with_the_canonical_one():
+    n, eps, dt, steps = 100000, 0.01, 0.001, 24
+    pos, vel, mass = milky_way(n, 41)
+
+    def drift(relative):
+        t = Tree(device=0)
+        t.build(pos.cuda(), mass.cuda()); t.set_velocity(vel.cuda()); t.force(0.4, eps)
+        if relative:
+            t.set_mac_relative(3e-4); t.force(1.0, eps)
+        k0, p0 = t.energy()
+        for _ in range(steps):
+            t.leapfrog(dt)
+        k1, p1 = t.energy()
+        t.close()
+        return abs((k1 + p1) - (k0 + p0)) / abs(k0 + p0)
+    d_geo, d_rel = drift(False), drift(True)
+    assert d_rel < max(3.0 * d_geo, 1e-6), (d_geo, d_rel)
+
+
+def test_random_configurations_with_the_relative_criterion_against_oracle():
+    """Seeded sweep: size, model, leaf and group size, alpha (0 and huge included), the geometric floor, eps, 1-3 sharded
+    contexts, and the per-particle |a| either of the oracle's canonical pass or log-uniform random numbers (the scale is an
+    input: any positive array must give the same lists on both sides)."""
+    from paper_1412_0659_b200.sharded import connect_local, force_local
+    rng = np.random.default_rng(20141207)
+    for _ in range(24):
+        n = int(rng.choice([rng.integers(2, 200), rng.integers(200, 5000), rng.integers(5000, 30000)]))
+        model = str(rng.choice(["plummer", "mw"])) if n >= 100 else "plummer"
+        leaf = int(rng.choice([1, 8, 16, 32])); group = int(rng.choice([32, 64, 64, 128]))
+        alpha = float(rng.choice([0.0 if n < 3000 else 1e-4, 1e-4, 1e-3, 1e-2, 1e30]))
+        floor = float(rng.choice([0.5, 1.0, 1.0, 1.5])); eps = float(rng.choice([0.002, 0.01, 0.05]))
+        world = int(rng.choice([1, 1, 2, 3])); seed = int(rng.integers(1, 10**6))
+        pos, _, mass = (plummer if model == "plummer" else milky_way)(n, seed, with_vel=False)
+        tag = f"n={n} {model} leaf={leaf} group={group} alpha={alpha} floor={floor} eps={eps} world={world} seed={seed}"
+        ot = oracle.Tree(pos.numpy(), mass.numpy(), leaf_size=leaf, group_size=group)
+        if rng.random() < 0.5:
+            amag = np.linalg.norm(ot.force(0.4, eps)[0], axis=1).astype(np.float32)
+        else:
+            amag = (10.0 ** rng.uniform(-6, 3, n)).astype(np.float32)
+        ot.set_mac_relative(alpha, amag)
+        oacc, opot, onpp, onpc = ot.force(floor, eps)
+        trees = [Tree(device=0, leaf_size=leaf, group_size=group) for _ in range(world)]
+        for t in trees:
+            t.reserve(n)
+        if world > 1:
+            connect_local(trees)
+        damag = torch.from_numpy(amag).cuda()
+        outs = [(torch.zeros((n, 3), device="cuda"), torch.zeros(n, device="cuda")) for _ in range(world)]
+        for t in trees:
+            t.build(pos.cuda(), mass.cuda()); t.set_mac_relative(alpha, damag)
+        force_local(trees, floor, eps, outs)
+        torch.cuda.synchronize()
+        for t, (acc, pot) in zip(trees, outs):
+            cnt = t.debug("counts")
+            assert np.array_equal(cnt[:, 0], onpp) and np.array_equal(cnt[:, 1], onpc), tag
+            a = acc.cpu().numpy().astype(np.float64); p = pot.cpu().numpy().astype(np.float64)
+            relv = np.linalg.norm(a - oacc, axis=1) / np.linalg.norm(oacc, axis=1)
+            i = int(relv.argmax())
+            A = ot.abs_sum(floor, eps, [i])[0]
+            assert relv.max() <= 1e-5 or np.linalg.norm(a[i] - oacc[i]) <= 2.5e-7 * A, (tag, relv.max())
+            assert (np.abs(p - opot) / np.abs(opot)).max() <= 1e-5, tag
+            t.close()
