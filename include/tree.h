@@ -127,6 +127,8 @@ int tree_set_mac(tree_ctx *t, int kind);
  *           by (the first one after tree_build) uses the geometric criterion alone with its theta, so the usual sequence is
  *           tree_build, tree_force(0.4, ...), tree_set_mac_relative(alpha, NULL), tree_force(1.0, ...), tree_leapfrog ...
  *           Non-NULL (needs a built tree): these values scale the next pass instead (tests: the same input to the oracle).
+ * A group one of whose particles has |a| = 0 opens every cell (direct summation for that group): for systems whose net forces
+ * cancel by symmetry (lattices, uniform boxes) use the geometric criterion.
  * tree_set_mac(t, kind) switches it off again.  Needs no rebuild.  Sharded contexts: every rank makes the same call at the
  * same point of the sequence (every rank holds the complete results of every pass, so all ranks derive the same scales and
  * the same lists; nothing more is communicated).  Allocates 8 bytes per particle and 4 per cell on first use. */

@@ -638,6 +638,7 @@ int tree_set_mac(tree_ctx *t, int kind) {
   if (t->force_open || t->step_open) return set_err(t, TREE_ERR_ORDER, "tree_set_mac inside an open force pass");
   BH_DEVICE(t);
   t->rel_on = false;
+  t->amag_valid = false;  // steps taken from here on do not carry |a| along: a later tree_set_mac_relative starts from the last pass
   if (kind != t->mac) {
     t->mac = kind;
     t->built = false;  // the tight boxes are computed with the moments: build again

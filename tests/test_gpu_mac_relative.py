@@ -237,3 +237,28 @@ def test_random_configurations_with_the_relative_criterion_against_oracle():
             assert relv.max() <= 1e-5 or np.linalg.norm(a[i] - oacc[i]) <= 2.5e-7 * A, (tag, relv.max())
             assert (np.abs(p - opot) / np.abs(opot)).max() <= 1e-5, tag
             t.close()
+
+
+def test_switching_the_relative_criterion_off_and_on_again_starts_from_the_last_pass():
+    # while it is off, steps do not carry |a| along; switching it on again must scale the next pass by the last pass's
+    # accelerations in the CURRENT slot order, exactly as if those values were handed in
+    n, alpha, eps, dt = 30000, 1e-3, 0.01, 0.002
+    pos, vel, mass = milky_way(n, 23)
+    t = Tree(device=0)
+    t.build(pos.cuda(), mass.cuda()); t.set_velocity(vel.cuda())
+    t.force(0.4, eps); t.set_mac_relative(alpha); t.force(1.0, eps); t.leapfrog(dt)
+    t.set_mac("geometric")
+    t.force(0.4, eps)
+    for _ in range(2):
+        t.leapfrog(dt)                      # canonical steps: the order changes, |a| is not gathered
+    p = torch.empty((n, 3), device="cuda"); a = torch.empty((n, 3), device="cuda")
+    t.get_state(p, None, a, None); torch.cuda.synchronize()
+    t.set_mac_relative(alpha)               # NULL: |a| of the last (canonical) pass
+    t.force(1.0, eps)
+    cnt = t.debug("counts")
+    t2 = Tree(device=0)
+    t2.build(p, mass.cuda())
+    t2.set_mac_relative(alpha, torch.from_numpy(_amag_like_the_kernel(a.cpu().numpy())).cuda())
+    t2.force(1.0, eps)
+    assert np.array_equal(t2.debug("counts"), cnt)
+    t.close(); t2.close()
