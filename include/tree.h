@@ -191,7 +191,7 @@ int tree_get_debug(tree_ctx *t, int what, void *dst, long long *count);
 #define TREE_PH_MOMENTS 4  /* groups + multipole moments         */
 #define TREE_PH_OPENING 5  /* opening radii for theta            */
 #define TREE_PH_WALK 6     /* the fused walk + force kernel only */
-#define TREE_PH_UNPERMUTE 7 /* results to the caller's arrays (only if tree_force was given any) */
+#define TREE_PH_UNPERMUTE 7 /* results to the caller's arrays as a pass of its own (sharded passes; tree_force on one context writes them in the walk's epilogue: 0) */
 #define TREE_PH_INTEGRATE 8 /* leapfrog: kick + drift + bbox pass (the closing kick runs in the walk's epilogue; sharded
                                passes kick in a pass of their own after the barrier) */
 #define TREE_PH_SCHED 9    /* counting walk + task list (cost-aware scheduling of the force walk) */

@@ -262,3 +262,36 @@ def test_switching_the_relative_criterion_off_and_on_again_starts_from_the_last_
     t2.force(1.0, eps)
     assert np.array_equal(t2.debug("counts"), cnt)
     t.close(); t2.close()
+
+
+def test_relative_parity_at_bench_size_config3_sampled_groups():
+    # BASELINE config 3 (Milky-Way-shaped, N = 8,388,608, eps = 0.01), the launch configuration bench.py times for it:
+    # counts and forces against the oracle's option on every 509th group, with a smooth synthetic |a| as the common input
+    # (enclosed mass of the three components over r^2 + 1: the scale is an input, any positive array will do)
+    from nbody_inputs import config
+    cfg, pos, vel, mass = config(2, with_vel=False)
+    n, eps, alpha = cfg["n"], cfg["eps"], 3e-4
+    r = pos.double().norm(dim=1).numpy()
+    menc = 80.0 * np.minimum(r / 200.0, 1.0) + 5.0 * (1.0 - np.exp(-r / 2.5)) + 1.0 * (r / (r + 0.7)) ** 2
+    amag = (menc / (r * r + 1.0)).astype(np.float32)
+    t = Tree(device=0)
+    acc = torch.empty((n, 3), device="cuda"); pot = torch.empty(n, device="cuda")
+    t.build(pos.cuda(), mass.cuda())
+    t.set_mac_relative(alpha, torch.from_numpy(amag).cuda())
+    t.force(1.0, eps, acc, pot)
+    torch.cuda.synchronize()
+    ot = oracle.Tree(pos.numpy(), mass.numpy())
+    order = ot.keys()[1]
+    ot.set_mac_relative(alpha, amag)
+    stride = 509
+    oacc, opot, onpp, onpc = ot.force(1.0, eps, g0=3, stride=stride)
+    gsel = np.arange(3, ot.n_groups, stride)
+    cnt = t.debug("counts")
+    assert np.array_equal(cnt[gsel, 0], onpp[gsel]) and np.array_equal(cnt[gsel, 1], onpc[gsel])
+    sel = np.concatenate([order[64 * g: 64 * g + 64] for g in gsel])
+    a = acc.cpu().numpy().astype(np.float64)[sel]; p = pot.cpu().numpy().astype(np.float64)[sel]
+    assert (np.linalg.norm(a - oacc[sel], axis=1) / np.linalg.norm(oacc[sel], axis=1)).max() <= 1e-5
+    assert (np.abs(p - opot[sel]) / np.abs(opot[sel])).max() <= 1e-5
+    ms, pp, pc = t.stats()
+    assert 2000 < (pp + pc) / n < 6000          # the condition is at work: the canonical theta = 1 lists are ~1500 long
+    t.close()
