@@ -120,8 +120,9 @@ int tree_set_mac(tree_ctx *t, int kind);
  * a_g = the smallest |a| among the group's particles in the previous force pass on this context: the first multipole
  * term the evaluation leaves out, ~ M l^3 / D^5, stays below alpha times the group's own acceleration.  FP32, one IEEE
  * operation each: gscale = alpha * a_g; sqrt(D2) * D2 * D2 * gscale > M * l * l * l.
- *   alpha : >= 0 (0 opens everything).  Measured (profiles/r2_mac_sweep_*.md): the median error of theta = 0.4 at about
- *           0.6 x the time, with a smaller 99th percentile.
+ *   alpha : >= 0 (0 opens everything).  Measured (profiles/r2_mac_sweep_*.md): the median error of theta = 0.4 in 0.44 x the
+ *           time on the Milky-Way-shaped model, with a smaller 99th percentile; alpha = 3e-4 is better than theta = 0.4 in
+ *           every error figure at about half the time.
  *   amag  : DEV float[N], caller order, |a| of every particle, or NULL.  NULL: the library uses the accelerations of its
  *           own last force pass; they travel with the particles through tree_leapfrog.  A pass with no accelerations to go
  *           by (the first one after tree_build) uses the geometric criterion alone with its theta, so the usual sequence is

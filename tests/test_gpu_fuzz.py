@@ -70,8 +70,9 @@ def _one(rng):
 
 
 def test_random_configurations_against_oracle():
+    import os
     rng = np.random.default_rng(20141206)
-    for _ in range(48):
+    for _ in range(int(os.environ.get("BH_FUZZ_CONFIGS", "48"))):  # a longer sweep of the same sequence: BH_FUZZ_CONFIGS=3000
         _one(rng)
 
 

@@ -199,8 +199,9 @@ def test_random_configurations_with_the_relative_criterion_against_oracle():
     contexts, and the per-particle |a| either of the oracle's canonical pass or log-uniform random numbers (the scale is an
     input: any positive array must give the same lists on both sides)."""
     from paper_1412_0659_b200.sharded import connect_local, force_local
+    import os
     rng = np.random.default_rng(20141207)
-    for _ in range(24):
+    for _ in range(int(os.environ.get("BH_FUZZ_CONFIGS", "24"))):  # a longer sweep of the same sequence: BH_FUZZ_CONFIGS=1000
         n = int(rng.choice([rng.integers(2, 200), rng.integers(200, 5000), rng.integers(5000, 30000)]))
         model = str(rng.choice(["plummer", "mw"])) if n >= 100 else "plummer"
         leaf = int(rng.choice([1, 8, 16, 32])); group = int(rng.choice([32, 64, 64, 128]))
