@@ -14,7 +14,7 @@ from paper_1412_0659_b200.sharded import connect_local, force_local, leapfrog_lo
 pytestmark = pytest.mark.gpu
 
 
-def _one(rng):
+def _one(rng, strict=True):
     n = int(rng.choice([rng.integers(1, 200), rng.integers(200, 5000), rng.integers(5000, 40000)]))
     model = str(rng.choice(["plummer", "mw"])) if n >= 100 else "plummer"
     leaf = int(rng.choice([1, 4, 8, 16, 32])); group = int(rng.choice([32, 64, 64, 128]))
@@ -59,12 +59,18 @@ def _one(rng):
         relv = np.linalg.norm(an - oacc, axis=1) / np.linalg.norm(oacc, axis=1)
         rel = relv.max()
         prel = (np.abs(pn - opot) / np.abs(opot)).max()
-        assert rel <= 1e-5 and prel <= 1e-5, (tag, rel, prel)
-        # the form of the bound that holds whatever the cancellation: the absolute error of a_i is
-        # at most 2.5e-7 x A_i, A_i = sum of the magnitudes of the terms of particle i's interaction list
+        # the statement of DESIGN.md "Tolerance": |a_gpu - a_oracle| <= max(1e-5 |a_i|, 2.5e-7 A_i), A_i = sum of the
+        # magnitudes of the terms of particle i's interaction list (the second term decides only where the sum cancels);
+        # the committed 48 configurations (strict) meet both the plain 1e-5 bound and the A_i form for their worst particle
         i = int(relv.argmax())
         A = ot.abs_sum(theta, eps, [i])[0]
-        assert np.linalg.norm(an[i] - oacc[i]) <= 2.5e-7 * A, (tag, i, np.linalg.norm(an[i] - oacc[i]) / A)
+        err = np.linalg.norm(an[i] - oacc[i])
+        assert prel <= 1e-5, (tag, prel)
+        if strict:
+            assert rel <= 1e-5, (tag, rel)
+            assert err <= 2.5e-7 * A, (tag, i, err / A)
+        else:
+            assert rel <= 1e-5 or err <= 2.5e-7 * A, (tag, i, rel, err / A)
     for t in trees:
         t.close()
 
@@ -72,8 +78,8 @@ def _one(rng):
 def test_random_configurations_against_oracle():
     import os
     rng = np.random.default_rng(20141206)
-    for _ in range(int(os.environ.get("BH_FUZZ_CONFIGS", "48"))):  # a longer sweep of the same sequence: BH_FUZZ_CONFIGS=3000
-        _one(rng)
+    for k in range(int(os.environ.get("BH_FUZZ_CONFIGS", "48"))):  # a longer sweep of the same sequence: BH_FUZZ_CONFIGS=3000
+        _one(rng, strict=k < 48)
 
 
 def _degenerate(rng, kind, n):
