@@ -311,6 +311,26 @@ def table_sass_histogram(path: str):
         body = [i for i in ins if tgt <= i[0] <= a]
         if len(body) >= 40:
             row(f"loop 0x{tgt:x}..0x{a:x}", body)
+    # straight-line blocks (no branch, no branch target inside) of 400 instructions or more that are not innermost loops
+    # themselves: a fully unrolled tile evaluator has no loop of its own
+    targets = set()
+    for a, op, txt in ins:
+        if op in ("BRA", "BSSY", "CALL", "JMP", "BRX"):
+            m = re.search(r"0x([0-9a-f]+)", txt)
+            if m:
+                targets.add(int(m.group(1), 16))
+    blocks, cur = [], []
+    for i in ins:
+        if i[0] in targets and cur:
+            blocks.append(cur); cur = []
+        cur.append(i)
+        if i[1] in ("BRA", "EXIT", "RET", "BRX", "JMP", "CALL"):
+            blocks.append(cur); cur = []
+    if cur:
+        blocks.append(cur)
+    for b in sorted(blocks, key=lambda b: -len(b)):
+        if len(b) >= 400 and not any(tgt <= b[0][0] and b[-1][0] <= a for tgt, a in inner):
+            row(f"block 0x{b[0][0]:x}..0x{b[-1][0]:x}", b)
 
 
 def table_walk_eval_split(configs):

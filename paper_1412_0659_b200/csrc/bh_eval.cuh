@@ -32,7 +32,11 @@ __device__ __forceinline__ unsigned warp_incl_scan_u(unsigned v, int /*lane*/) {
 // Evaluate: whenever a queue holds >= 32 sources, 32 of them are staged in shared memory as float4
 // and every lane evaluates them against its TPL targets with broadcast LDS.128 loads.
 // ------------------------------------------------------------------------------------------
-constexpr int PP_UNROLL = 16, PC_UNROLL = 16;  // sources per unrolled evaluator loop body
+// sources per unrolled evaluator loop body.  p-c: the whole tile (32 x 32 packed instructions, no loop): 970.8 ms against 976.2 ms with
+// 16 at N = 134 M, 55.36 / 55.56 ms at 8.4 M; p-p stays at 16 (32 for both: 1015 ms, the two bodies no longer fit the instruction cache).
+// With the relative criterion the lists are half as long and the kernel changes between walking and evaluating twice as often: there
+// the 19 KB tile costs more than it gains (459.5 against 453.6 ms per step at 134 M), so those kernels keep 16.
+constexpr int PP_UNROLL = 16, PC_UNROLL = 32, PC_UNROLL_REL = 16;
 constexpr int WALK_WARPS = 4;  // warps per block of the walk kernels
 constexpr int WALK_MINB = 5;  // resident blocks per SM the register budget is sized for
 // four targets per lane (group 128) keep twice the per-target state in registers: fewer, fatter blocks
@@ -360,13 +364,13 @@ __device__ __forceinline__ void eval_pp_tile(const WarpSmem &ws, int cnt, bool m
   }
 }
 
-template <int TPL>
+template <int TPL, int PCU = PC_UNROLL>
 __device__ __forceinline__ void eval_pc_tile(const WarpSmem &ws, int cnt, Targets<TPL> &T, float eps2) {
   if constexpr (TPL == 2 && BH_PACKED) {
     Targets2 P2(T);
     const f32x2 e2 = bc2(eps2);
     if (cnt == 32) {
-#pragma unroll(PC_UNROLL)
+#pragma unroll(PCU)
       for (int j = 0; j < 32; ++j) pc_one2(ws.pc0[j], ws.pc1[j], ws.pc2[j], P2, e2);
     } else {
       for (int j = 0; j < cnt; ++j) pc_one2(ws.pc0[j], ws.pc1[j], ws.pc2[j], P2, e2);
@@ -377,7 +381,7 @@ __device__ __forceinline__ void eval_pc_tile(const WarpSmem &ws, int cnt, Target
   }
   QuadAcc<TPL> A;
   if (cnt == 32) {
-#pragma unroll(PC_UNROLL)
+#pragma unroll(PCU)
     for (int j = 0; j < 32; ++j) pc_one<TPL>(ws.pc0[j], ws.pc1[j], ws.pc2[j], T, A, eps2);
   } else {
     for (int j = 0; j < cnt; ++j) pc_one<TPL>(ws.pc0[j], ws.pc1[j], ws.pc2[j], T, A, eps2);

@@ -52,7 +52,7 @@ struct WalkState {
 };
 
 // Evaluate what is left in the two queues as partial tiles (tile ownership by the counter rule).
-template <int TPL>
+template <int TPL, int PCU>
 __device__ __forceinline__ void flush_queues(WarpSmem &ws, int lane, WalkState<TPL> &S, Targets<TPL> &T, Totals<TPL> &R,
                                              const WalkParams &P, uint32_t g0, uint32_t gsize) {
   if (S.pc_pending > 0) {
@@ -60,7 +60,7 @@ __device__ __forceinline__ void flush_queues(WarpSmem &ws, int lane, WalkState<T
     S.tile_wait = mine ? S.tile_parts - 1 : S.tile_wait - 1;
     if (mine) {
       stage_pc(ws, lane, S.pc_pending, P);
-      eval_pc_tile<TPL>(ws, S.pc_pending, T, P.eps2);
+      eval_pc_tile<TPL, PCU>(ws, S.pc_pending, T, P.eps2);
       if (++S.unfolded >= FOLD_EVERY) { fold_tile<TPL>(T, R); S.unfolded = 0; }
       __syncwarp();
     }
@@ -155,7 +155,7 @@ __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, con
     //      evaluators). A part of a split group has then finished the skeleton all parts walk alike and
     //      continues with its own share of the deferred child ranges, evaluating every tile itself.
     if (sp == 0) {
-      if (!COUNT) flush_queues<TPL>(ws, lane, S, T, R, P, (uint32_t)g0, gsize);
+      if (!COUNT) flush_queues<TPL, REL ? PC_UNROLL_REL : PC_UNROLL>(ws, lane, S, T, R, P, (uint32_t)g0, gsize);
       if (!(SPLIT && prefix)) break;
       if constexpr (!COUNT) {
         for (int base = 0; base < dp; base += 32) {
@@ -268,7 +268,7 @@ __device__ __forceinline__ void walk_task(const WalkParams &P, WarpSmem &ws, con
       S.tile_wait = mine ? S.tile_parts - 1 : S.tile_wait - 1;
       if (mine) {
         stage_pc(ws, lane, 32, P);
-        eval_pc_tile<TPL>(ws, 32, T, P.eps2);
+        eval_pc_tile<TPL, REL ? PC_UNROLL_REL : PC_UNROLL>(ws, 32, T, P.eps2);
         if (++S.unfolded >= FOLD_EVERY) { fold_tile<TPL>(T, R); S.unfolded = 0; }
         __syncwarp();
       }
