@@ -156,3 +156,32 @@ def test_one_step_moves_few_particles_along_the_curve():
     assert np.mean(disp <= 32) > 0.97          # the gather reads within a cache line or two of where it writes
     assert changed.mean() > 0.9                # yet nearly every key differs: nothing for a radix pass to skip
     t.close()
+
+
+def test_caller_order_results_from_the_walk_epilogue_equal_the_state_also_for_split_groups():
+    # tree_force with caller arrays on one context writes them in the walk's epilogue (a11 fused): the arrays must hold exactly
+    # what tree_get_state returns afterwards, also for groups whose walk was cut into parts (their results are written by the part
+    # that combines the partial sums) and for acc-only / pot-only calls
+    n, theta, eps = 200_000, 0.4, 0.01
+    pos, _, mass = plummer(n, 91, with_vel=False)
+    idx = torch.arange(0, n, 1500)   # a few particles far out: their runs of 64 have boxes over dense regions and are split
+    d = torch.randn(len(idx), 3, generator=torch.Generator().manual_seed(6), dtype=torch.float64)
+    pos[idx] = (25.0 * d / d.norm(dim=1, keepdim=True)).float()
+    t = Tree(device=0)
+    acc = torch.full((n, 3), float("nan"), device="cuda"); pot = torch.full((n,), float("nan"), device="cuda")
+    t.build(pos.cuda(), mass.cuda())
+    t.force(theta, eps, acc, pot)
+    tr = t.debug("task_trace")
+    assert ((tr[:, 3] >> 26) > 0).any()          # some groups were walked in parts
+    a2 = torch.empty((n, 3), device="cuda"); p2 = torch.empty(n, device="cuda")
+    t.get_state(None, None, a2, p2); torch.cuda.synchronize()
+    assert torch.equal(acc, a2) and torch.equal(pot, p2)
+    # acc only / pot only (a later pass is scheduled by the previous one's counts: other parts, other last bits, so every
+    # pass is compared with its own state)
+    acc.fill_(float("nan")); t.force(theta, eps, acc, None)
+    t.get_state(None, None, a2, p2); torch.cuda.synchronize()
+    assert torch.equal(acc, a2)
+    pot.fill_(float("nan")); t.force(theta, eps, None, pot)
+    t.get_state(None, None, a2, p2); torch.cuda.synchronize()
+    assert torch.equal(pot, p2)
+    t.close()
