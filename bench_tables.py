@@ -36,7 +36,7 @@ ALGO_BYTES = {
     "permute_step_kernel": ("N", 8 + 4 + 36 + 36),
     "permute_build_kernel": ("N", 4 + 16 + 20),
     "tree_levels_kernel": ("N", 8 + 2),
-    "tree_emit_kernel": ("N", 2),
+    "tree_emit_kernel": ("N", 2 + 3),  # level / leaf words read + 13 B per cell written (c_level, c_first, c_count, c_fcall), 0.234 cells per particle
     "groups_kernel": ("N", 16),
     "kick_kernel": ("N", 32 + 16),
     "gather_out_kernel": ("N", 20 + 16),
